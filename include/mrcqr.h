@@ -1,0 +1,135 @@
+/*
+ * mrcqr.h -- C ABI of the B200-native (sm_100a) MRCQR library: FP64 thin QR  A = Q R  of a
+ * tall-skinny m x n matrix by mixed-precision randomized-preconditioned Cholesky-QR
+ * (arxiv/paper_2606_18411, Algorithm 2; Algorithm 1).
+ *
+ * Conventions (all entry points)
+ *   Layout     column-major; A is m x n with leading dimension lda >= m (the paper's libraries
+ *              and its "column-wise" FFT are column-major).  R, Rs, Rc, G are
+ *              n x n, ld = n, upper triangle meaningful, strictly-lower part written as zero
+ *              (G is written full symmetric).
+ *   Pointers   DEVICE pointers unless the argument name ends in _host.  The caller owns every
+ *              buffer it passes; A is never modified; Q must not overlap A.
+ *   Workspace  the library owns one grow-only device workspace (sketch partials, A_s, R_s, Gram
+ *              partials, status word), allocated on first use, freed by mrcqr_shutdown().
+ *              Not thread-safe: one call at a time per process.
+ *   stream     a cudaStream_t passed as void* (NULL = default stream).  Kernels are enqueued on
+ *              it; the call then reads back an 8-byte status word and synchronises the stream, so
+ *              the return value is final when the call returns.
+ *   Returns    0 ok.  -k: the k-th argument is illegal (LAPACK style).  Positive codes below.
+ *              On a positive code Q and R are unspecified.  Nothing is retried, shifted or
+ *              hidden (breakdown is a reported event).
+ *   No CPU fallback exists: without a CUDA device every compute entry point returns MRCQR_ERR_CUDA.
+ */
+#ifndef MRCQR_H
+#define MRCQR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* sketch precision p of Algorithm 2: half, single, double */
+typedef enum { MRCQR_FP16 = 16, MRCQR_FP32 = 32, MRCQR_FP64 = 64 } mrcqr_prec_t;
+
+enum {
+    MRCQR_OK            = 0,
+    MRCQR_ERR_NONFINITE = 1,  /* non-finite value in the sketch (e.g. FP16 overflow of fl_p(D A))        */
+    MRCQR_ERR_SINGULAR  = 2,  /* R_s has a zero / non-finite diagonal: A rank deficient   */
+    MRCQR_ERR_BREAKDOWN = 3,  /* Cholesky pivot <= 0 or NaN; index: mrcqr_last_info() */
+    MRCQR_ERR_CUDA      = 4   /* CUDA runtime error, or no device                                        */
+};
+
+/*
+ * Algorithm 2 step 1: draw the Rademacher diagonal D and the sampled bins S from a
+ * splitmix64 stream (BASELINE.json configs).  HOST function, integer arithmetic only.
+ *   X(k) = k-th output of splitmix64 seeded with `seed`.
+ *   signs_host: ceil(m/64) words; d_t = -1 iff bit (t mod 64) of word floor(t/64) = X(floor(t/64)) is 1.
+ *   idx_host:   s distinct 0-based bins in [0, floor(m/2)], ascending.  Candidates
+ *               floor(X(k) * (floor(m/2)+1) / 2^64) for k = ceil(m/64), ceil(m/64)+1, ...;
+ *               a candidate is kept if new, until s are kept.
+ * Returns 0, -1 (m < 1), -2 (s < 0 or s > floor(m/2)+1), -4/-5 (null pointer).
+ */
+int mrcqr_draw(int64_t m, int s, uint64_t seed, uint64_t* signs_host, int64_t* idx_host);
+
+/*
+ * Stage 1, Algorithm 2 steps 2-6: the subsampled randomized trigonometric
+ * transform and the sketch QR.
+ *   x~ = fl_p(D a_j) (sign-bit flip + round to p), X = DFT_m(x~) down each column,
+ *   A_s[i,j] = sqrt(s/m) Re X[idx[i]], A_s stored in precision p;
+ *   R_s = R-factor of the Householder QR of A_s with rows sign-normalised to diag > 0, in FP64.
+ * Arithmetic is at least precision p (FP16: FP16 input/output rounding, FP32 arithmetic).
+ *   m       power of two, m >= n            signs  ceil(m/64) uint64 words (device)
+ *   s       n <= s <= m/2+1                 idx    s ascending bins, int64 (device)
+ *   As_out  nullable; s x n, ld = s, FP64 container holding the precision-p values exactly
+ *   Rs      n x n, ld = n (out)
+ * Positive returns: 1 (non-finite sketch), 2 (singular R_s; index via mrcqr_last_info()).
+ */
+int mrcqr_sketch(int64_t m, int n, int64_t lda, const double* A, mrcqr_prec_t prec, int s,
+                 const uint64_t* signs, const int64_t* idx, double* As_out, double* Rs,
+                 void* stream);
+
+/*
+ * Stage 2a, Algorithm 2 step 7 fused with Algorithm 1 steps 1-2.
+ * For every row a of A: y R_s = a by forward substitution in FP64 (R_s^-1 is never formed,
+ * PAPER.md:121); G = sum_rows y^T y on FP64 tensor cores (DMMA) with a deterministic split-m
+ * reduction; Y = A R_s^-1 is never written to memory.  Then G = Rc^T Rc (Cholesky, Rc upper,
+ * diag > 0).  Any m >= n.  G_out nullable (n x n full symmetric).  Rc: n x n (out).
+ * Positive returns: 2 (Rs diagonal zero/non-finite), 3 (Cholesky breakdown, pivot index via
+ * mrcqr_last_info()).
+ */
+int mrcqr_precondition_gram(int64_t m, int n, int64_t lda, const double* A, const double* Rs,
+                            double* G_out, double* Rc, void* stream);
+
+/*
+ * Stage 2b + 3, Algorithm 1 step 3 and Algorithm 2 step 9.
+ * For every row: y = a R_s^-1 recomputed bit-identically to stage 2a, then q R_c = y; Q written
+ * (m x n, ldq >= m).  R = R_c R_s (n x n, nullable).
+ */
+int mrcqr_form_q(int64_t m, int n, int64_t lda, const double* A, const double* Rs,
+                 const double* Rc, int64_t ldq, double* Q, double* R, void* stream);
+
+/*
+ * Whole Algorithm 2 = draw(seed) -> mrcqr_sketch -> mrcqr_precondition_gram ->
+ * mrcqr_form_q on one stream with a single status read-back at the end.
+ *   Q uses the same leading dimension lda as A.   s <= 0 selects the paper default 3n.
+ *   sketch_prec: the caller's choice by the rule of PAPER.md:163 (half if kappa < 1e4, single if
+ *   kappa < 1e8, double otherwise).
+ * Argument errors: -1 m (not a power of two or < n), -2 n, -3 lda, -4 A, -5 Q, -6 R, -7 prec, -8 s.
+ */
+int mrcqr_factor(int64_t m, int n, int64_t lda, const double* A, double* Q, double* R,
+                 mrcqr_prec_t sketch_prec, int s, uint64_t seed, void* stream);
+
+/*
+ * mrcqr_factor with HOST buffers: copies A to the device (library-owned buffers), factors,
+ * copies Q and R back; synchronous.  This is the end-to-end path bench.py times as `e2e`.
+ */
+int mrcqr_factor_host(int64_t m, int n, int64_t lda, const double* A_host, double* Q_host,
+                      double* R_host, mrcqr_prec_t sketch_prec, int s, uint64_t seed);
+
+/* Bytes of library-owned device workspace a factorization of this shape uses. */
+size_t mrcqr_workspace_bytes(int64_t m, int n, int s, mrcqr_prec_t prec);
+
+/* Detail of the last positive return code: 0-based pivot / diagonal index (codes 2, 3), else 0. */
+int mrcqr_last_info(void);
+
+/* Number of kernel launches enqueued by the last compute call (bench.py's gpu_launches). */
+int mrcqr_last_launch_count(void);
+
+/*
+ * Test hook for the "bit-identical Y" requirement: runs the stage-2a and the stage-2b
+ * tile solves and dumps the Y = A R_s^-1 each of them computed (m x n, ld = m).  The two dumps
+ * must be equal bit for bit.
+ */
+int mrcqr_debug_dump_y(int64_t m, int n, int64_t lda, const double* A, const double* Rs,
+                       double* Y_stage2a, double* Y_stage2b, void* stream);
+
+/* Frees the workspace (and the host-path device buffers). */
+void mrcqr_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MRCQR_H */

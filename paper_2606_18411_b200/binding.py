@@ -1,0 +1,175 @@
+"""Thin ctypes binding of the C ABI in include/mrcqr.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libmrcqr.so; there is no Python or CPU
+fallback: a missing library or a missing device raises.  PyTorch is used for device memory and
+streams only.
+
+Matrices are torch float64 CUDA tensors of shape (n, m), C-contiguous = the m x n column-major
+matrix with leading dimension m (see inputs.py).  n x n factors are (n, n) tensors holding the
+column-major matrix, i.e. tensor[j, i] = R[i, j]; use `.t()` to read them as R[i, j].
+"""
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+FP16, FP32, FP64 = 16, 32, 64
+ERRORS = {1: "non-finite value in the sketch", 2: "R_s singular (A rank deficient)",
+          3: "Cholesky breakdown", 4: "CUDA error / no device"}
+
+_lib = None
+
+
+class MrcqrError(RuntimeError):
+    def __init__(self, code, info=0):
+        self.code, self.info = code, info
+        what = ERRORS.get(code, "illegal argument %d" % (-code) if code < 0 else "unknown")
+        super().__init__("mrcqr: code %d (%s), info %d" % (code, what, info))
+
+
+def lib():
+    """Loads (building if needed) libmrcqr.so.  Raises if it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if not os.path.exists(path) or os.environ.get("MRCQR_REBUILD"):
+            path = _build.build()
+        L = C.CDLL(path)
+        i64, u64, vp, ci = C.c_int64, C.c_uint64, C.c_void_p, C.c_int
+        L.mrcqr_draw.argtypes = [i64, ci, u64, vp, vp]
+        L.mrcqr_sketch.argtypes = [i64, ci, i64, vp, ci, ci, vp, vp, vp, vp, vp]
+        L.mrcqr_precondition_gram.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
+        L.mrcqr_form_q.argtypes = [i64, ci, i64, vp, vp, vp, i64, vp, vp, vp]
+        L.mrcqr_factor.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64, vp]
+        L.mrcqr_factor_host.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64]
+        L.mrcqr_workspace_bytes.restype = C.c_size_t
+        L.mrcqr_workspace_bytes.argtypes = [i64, ci, ci, ci]
+        L.mrcqr_debug_dump_y.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
+        L.mrcqr_shutdown.restype = None
+        for f in ("mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
+                  "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y"):
+            getattr(L, f).restype = ci
+        _lib = L
+    return _lib
+
+
+EXPORTS = ["mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
+           "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
+           "mrcqr_debug_dump_y", "mrcqr_shutdown"]
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _chk(rc):
+    if rc != 0:
+        raise MrcqrError(rc, lib().mrcqr_last_info())
+
+
+def _mat(AT):
+    assert AT.is_cuda and AT.dtype == torch.float64 and AT.dim() == 2 and AT.stride(1) == 1
+    n, m = AT.shape
+    return m, n, AT.stride(0), AT.data_ptr()
+
+
+def mrcqr_draw(m, s, seed):
+    """Host draw (Algorithm 2 step 1): returns (signs uint64-as-int64 tensor, idx int64 tensor) on CPU."""
+    signs = torch.zeros((m + 63) // 64, dtype=torch.int64)
+    idx = torch.zeros(max(s, 1), dtype=torch.int64)
+    rc = lib().mrcqr_draw(m, s, seed, signs.data_ptr(), idx.data_ptr())
+    if rc != 0:
+        raise MrcqrError(rc)
+    return signs, idx[:s].clone()
+
+
+def mrcqr_sketch(AT, prec, signs, idx, want_As=False, stream=None):
+    """Stage 1.  signs/idx: device tensors.  Returns (Rs (n,n) col-major, As (n,s) col-major or None)."""
+    m, n, lda, pA = _mat(AT)
+    s = idx.numel()
+    Rs = torch.empty((n, n), dtype=torch.float64, device=AT.device)
+    As = torch.empty((n, s), dtype=torch.float64, device=AT.device) if want_As else None
+    rc = lib().mrcqr_sketch(m, n, lda, pA, prec, s, signs.data_ptr(), idx.data_ptr(),
+                            As.data_ptr() if want_As else None, Rs.data_ptr(), _stream(stream))
+    _chk(rc)
+    return Rs, As
+
+
+def mrcqr_precondition_gram(AT, Rs, want_G=False, stream=None):
+    """Stage 2a.  Returns (Rc, G or None), both (n,n) col-major."""
+    m, n, lda, pA = _mat(AT)
+    Rc = torch.empty((n, n), dtype=torch.float64, device=AT.device)
+    G = torch.empty((n, n), dtype=torch.float64, device=AT.device) if want_G else None
+    rc = lib().mrcqr_precondition_gram(m, n, lda, pA, Rs.data_ptr(), G.data_ptr() if want_G else None,
+                                       Rc.data_ptr(), _stream(stream))
+    _chk(rc)
+    return Rc, G
+
+
+def mrcqr_form_q(AT, Rs, Rc, QT=None, stream=None):
+    """Stage 2b + 3.  Returns (QT (n,m) col-major Q, R (n,n) col-major)."""
+    m, n, lda, pA = _mat(AT)
+    if QT is None:
+        QT = torch.empty((n, m), dtype=torch.float64, device=AT.device)
+    R = torch.empty((n, n), dtype=torch.float64, device=AT.device)
+    rc = lib().mrcqr_form_q(m, n, lda, pA, Rs.data_ptr(), Rc.data_ptr(), QT.stride(0), QT.data_ptr(),
+                            R.data_ptr(), _stream(stream))
+    _chk(rc)
+    return QT, R
+
+
+def mrcqr_factor(AT, prec, s, seed, QT=None, R=None, stream=None, check=True):
+    """Whole Algorithm 2 on device buffers.  Returns (QT, R) (or the return code if check=False)."""
+    m, n, lda, pA = _mat(AT)
+    if QT is None:
+        QT = torch.empty_strided((n, m), (lda, 1), dtype=torch.float64, device=AT.device)
+    if R is None:
+        R = torch.empty((n, n), dtype=torch.float64, device=AT.device)
+    rc = lib().mrcqr_factor(m, n, lda, pA, QT.data_ptr(), R.data_ptr(), prec, s, seed, _stream(stream))
+    if not check:
+        return rc
+    _chk(rc)
+    return QT, R
+
+
+def mrcqr_factor_host(AT_host, prec, s, seed, QT_host=None, R_host=None):
+    """Whole Algorithm 2 on HOST buffers (copies inside the call): the end-to-end path."""
+    assert (not AT_host.is_cuda) and AT_host.dtype == torch.float64 and AT_host.stride(1) == 1
+    n, m = AT_host.shape
+    if QT_host is None:
+        QT_host = torch.empty((n, m), dtype=torch.float64, pin_memory=True)
+    if R_host is None:
+        R_host = torch.empty((n, n), dtype=torch.float64, pin_memory=True)
+    rc = lib().mrcqr_factor_host(m, n, AT_host.stride(0), AT_host.data_ptr(), QT_host.data_ptr(),
+                                 R_host.data_ptr(), prec, s, seed)
+    _chk(rc)
+    return QT_host, R_host
+
+
+def mrcqr_debug_dump_y(AT, Rs, stream=None):
+    m, n, lda, pA = _mat(AT)
+    Y3 = torch.empty((n, m), dtype=torch.float64, device=AT.device)
+    Y5 = torch.empty((n, m), dtype=torch.float64, device=AT.device)
+    rc = lib().mrcqr_debug_dump_y(m, n, lda, pA, Rs.data_ptr(), Y3.data_ptr(), Y5.data_ptr(), _stream(stream))
+    _chk(rc)
+    return Y3, Y5
+
+
+def mrcqr_workspace_bytes(m, n, s, prec):
+    return int(lib().mrcqr_workspace_bytes(m, n, s, prec))
+
+
+def mrcqr_last_info():
+    return int(lib().mrcqr_last_info())
+
+
+def mrcqr_last_launch_count():
+    return int(lib().mrcqr_last_launch_count())
+
+
+def mrcqr_shutdown():
+    lib().mrcqr_shutdown()

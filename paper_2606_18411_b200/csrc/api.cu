@@ -1,0 +1,375 @@
+// api.cu -- the C ABI declared in include/mrcqr.h: argument checking, the library-owned workspace,
+// the seeded draw (Algorithm 2 step 1) and the composition of the kernels K1..K5.
+#include "../../include/mrcqr.h"
+#include "mrcqr_internal.cuh"
+#include <algorithm>
+#include <cstring>
+#include <vector>
+
+namespace mrcqr {
+
+// ---- splitmix64, counter form: X(k) = mix(seed + (k+1) * gamma) ----------------------------------
+__host__ __device__ __forceinline__ uint64_t splitmix64_at(uint64_t seed, uint64_t k)
+{
+    uint64_t z = seed + (k + 1ull) * 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+// device side of the draw: sign words, plus reset of the status block (first kernel of a call)
+__global__ void mrcqr_draw_signs(uint64_t seed, int64_t nwords, uint64_t* __restrict__ signs, Status* st)
+{
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w == 0 && st) { st->code = 0; st->info = 0; }
+    if (w < nwords) signs[w] = splitmix64_at(seed, (uint64_t)w);
+}
+
+__global__ void mrcqr_reset_status(Status* st) { st->code = 0; st->info = 0; }
+
+static void draw_bins_host(int64_t m, int s, uint64_t seed, int64_t* idx)
+{
+    const uint64_t nw = (uint64_t)((m + 63) / 64), B = (uint64_t)(m / 2 + 1);
+    std::vector<int64_t> sorted;                 // kept candidates, ascending (binary search = "is new")
+    sorted.reserve((size_t)s);
+    for (uint64_t k = nw; (int)sorted.size() < s; ++k) {
+        const unsigned __int128 prod = (unsigned __int128)splitmix64_at(seed, k) * (unsigned __int128)B;
+        const int64_t cand = (int64_t)(uint64_t)(prod >> 64);
+        auto it = std::lower_bound(sorted.begin(), sorted.end(), cand);
+        if (it == sorted.end() || *it != cand) sorted.insert(it, cand);
+    }
+    std::memcpy(idx, sorted.data(), sizeof(int64_t) * (size_t)s);
+}
+
+// ---- workspace -----------------------------------------------------------------------------------
+struct Layout {
+    size_t status, signs, idx, As, Rs, RsPrep, RcPrep, G16, Rc, k1, k3, total;
+};
+
+static size_t al(size_t x) { return (x + 255) / 256 * 256; }
+
+static Layout make_layout(int64_t m, int n, int s, int prec)
+{
+    Layout L;
+    const size_t n16 = (size_t)round_up(n, 16);
+    size_t o = 0;
+    L.status = o; o += al(sizeof(Status));
+    L.signs = o;  o += al((size_t)((m + 63) / 64) * 8);
+    L.idx = o;    o += al((size_t)std::max(s, 1) * 8);
+    L.As = o;     o += al((size_t)std::max(s, 1) * n * 8);
+    L.Rs = o;     o += al((size_t)n * n * 8);
+    L.RsPrep = o; o += al(n16 * n16 * 8);
+    L.RcPrep = o; o += al(n16 * n16 * 8);
+    L.G16 = o;    o += al(n16 * n16 * 8);
+    L.Rc = o;     o += al((size_t)n * n * 8);
+    L.k1 = o;     o += al(s > 0 ? k1_workspace_bytes(m, n, s, prec) : 0);
+    L.k3 = o;     o += al(k3_partials_bytes(n));
+    L.total = o;
+    return L;
+}
+
+struct Ctx {
+    char* ws = nullptr; size_t ws_bytes = 0;
+    int* h_status = nullptr;                 // pinned, 2 ints
+    int64_t* h_idx = nullptr; size_t h_idx_cap = 0;   // pinned staging of the bins
+    double* hA = nullptr; double* hQ = nullptr; double* hR = nullptr; size_t hA_bytes = 0, hR_bytes = 0; // host-path device buffers
+    int last_info = 0, last_launches = 0;
+    bool have_device = false, probed = false;
+};
+static Ctx g;
+
+static bool device_ok()
+{
+    if (!g.probed) {
+        int cnt = 0;
+        g.have_device = (cudaGetDeviceCount(&cnt) == cudaSuccess && cnt > 0);
+        if (!g.have_device) cudaGetLastError();
+        g.probed = true;
+    }
+    return g.have_device;
+}
+
+static bool ensure_ws(size_t bytes)
+{
+    if (!g.h_status && cudaMallocHost(&g.h_status, 64) != cudaSuccess) return false;
+    if (bytes <= g.ws_bytes) return true;
+    if (g.ws) { cudaDeviceSynchronize(); cudaFree(g.ws); g.ws = nullptr; g.ws_bytes = 0; }
+    if (cudaMalloc(&g.ws, bytes) != cudaSuccess) { cudaGetLastError(); return false; }
+    g.ws_bytes = bytes;
+    return true;
+}
+
+static bool ensure_hidx(size_t count)
+{
+    if (count <= g.h_idx_cap) return true;
+    if (g.h_idx) cudaFreeHost(g.h_idx);
+    g.h_idx_cap = 0;
+    if (cudaMallocHost(&g.h_idx, count * sizeof(int64_t)) != cudaSuccess) { g.h_idx = nullptr; return false; }
+    g.h_idx_cap = count;
+    return true;
+}
+
+// reads the status block back and synchronises; returns the final code of the call
+static int finish(const Layout& L, cudaStream_t st, int launches)
+{
+    g.last_launches = launches;
+    cudaMemcpyAsync(g.h_status, g.ws + L.status, 8, cudaMemcpyDeviceToHost, st);
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) return MRCQR_ERR_CUDA;
+    g.last_info = g.h_status[1];
+    return g.h_status[0];
+}
+
+static bool is_pow2(int64_t m) { return m > 0 && (m & (m - 1)) == 0; }
+static bool prec_ok(int p) { return p == 16 || p == 32 || p == 64; }
+constexpr int N_MAX = 512;
+constexpr int S_MAX = 4096;
+
+// enqueue helpers shared by the stage calls and mrcqr_factor ----------------------------------------
+static int enqueue_sketch(const Layout& L, int64_t m, int n, int64_t lda, const double* A, int prec, int s,
+                          const uint64_t* signs, const int64_t* idx, double* As_out, double* Rs, cudaStream_t st)
+{
+    Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
+    double* As = reinterpret_cast<double*>(g.ws + L.As);
+    int k = launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);
+    if (As_out) cudaMemcpyAsync(As_out, As, sizeof(double) * (size_t)s * n, cudaMemcpyDeviceToDevice, st);
+    k += launch_k2_sketch_qr(As, s, n, nullptr, Rs, stat, st);
+    return k;
+}
+
+static int enqueue_gram(const Layout& L, int64_t m, int n, int64_t lda, const double* A, const double* Rs,
+                        double* G_out, double* Rc, double* Ydump, cudaStream_t st)
+{
+    Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
+    const int n16 = round_up(n, 16);
+    double* RsPrep = reinterpret_cast<double*>(g.ws + L.RsPrep);
+    double* RcPrep = reinterpret_cast<double*>(g.ws + L.RcPrep);
+    double* G16 = reinterpret_cast<double*>(g.ws + L.G16);
+    double* part = reinterpret_cast<double*>(g.ws + L.k3);
+    int np = 0;
+    int k = launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st);
+    k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, Ydump, st);
+    k += launch_reduce_partials(part, np, n, n16, G16, st);
+    k += launch_k4_cholesky(G16, n, n16, G_out, Rc, RcPrep, stat, st);
+    return k;
+}
+
+static int enqueue_formq(const Layout& L, int64_t m, int n, int64_t lda, const double* A, const double* Rs,
+                         const double* Rc, bool prep_rs, bool prep_rc, int64_t ldq, double* Q, double* R,
+                         double* Ydump, cudaStream_t st)
+{
+    Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
+    const int n16 = round_up(n, 16);
+    double* RsPrep = reinterpret_cast<double*>(g.ws + L.RsPrep);
+    double* RcPrep = reinterpret_cast<double*>(g.ws + L.RcPrep);
+    int k = 0;
+    if (prep_rs) k += launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st);
+    if (prep_rc) k += launch_prep_R(Rc, n, RcPrep, n16, stat, MRCQR_ERR_BREAKDOWN, st);
+    k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, Ydump, st);
+    if (R) k += launch_triu_mul(Rc, Rs, n, R, st);
+    return k;
+}
+
+} // namespace mrcqr
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+using namespace mrcqr;
+
+extern "C" int mrcqr_draw(int64_t m, int s, uint64_t seed, uint64_t* signs_host, int64_t* idx_host)
+{
+    if (m < 1) return -1;
+    if (s < 0 || (int64_t)s > m / 2 + 1) return -2;
+    if (!signs_host) return -4;
+    if (!idx_host && s > 0) return -5;
+    const int64_t nw = (m + 63) / 64;
+    for (int64_t w = 0; w < nw; ++w) signs_host[w] = splitmix64_at(seed, (uint64_t)w);
+    if (s > 0) draw_bins_host(m, s, seed, idx_host);
+    return 0;
+}
+
+extern "C" size_t mrcqr_workspace_bytes(int64_t m, int n, int s, mrcqr_prec_t prec)
+{
+    if (m < 1 || n < 1 || n > N_MAX || !prec_ok((int)prec) || !device_ok()) return 0;
+    if (s <= 0) s = 3 * n;
+    return make_layout(m, n, s, (int)prec).total;
+}
+
+extern "C" int mrcqr_last_info(void) { return g.last_info; }
+extern "C" int mrcqr_last_launch_count(void) { return g.last_launches; }
+
+extern "C" void mrcqr_shutdown(void)
+{
+    if (!g.probed || !g.have_device) return;
+    cudaDeviceSynchronize();
+    if (g.ws) cudaFree(g.ws);
+    if (g.h_status) cudaFreeHost(g.h_status);
+    if (g.h_idx) cudaFreeHost(g.h_idx);
+    if (g.hA) cudaFree(g.hA);
+    if (g.hQ) cudaFree(g.hQ);
+    if (g.hR) cudaFree(g.hR);
+    g = Ctx();
+}
+
+extern "C" int mrcqr_sketch(int64_t m, int n, int64_t lda, const double* A, mrcqr_prec_t prec, int s,
+                            const uint64_t* signs, const int64_t* idx, double* As_out, double* Rs,
+                            void* stream)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (!is_pow2(m) || m < n || m < 32) return -1;
+    if (lda < m) return -3;
+    if (!A) return -4;
+    if (!prec_ok((int)prec)) return -5;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX) return -6;
+    if (!signs) return -7;
+    if (!idx) return -8;
+    if (!Rs) return -10;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    Layout L = make_layout(m, n, s, (int)prec);
+    if (!ensure_ws(L.total)) return MRCQR_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
+    mrcqr_reset_status<<<1, 1, 0, st>>>(stat);
+    int k = 1 + enqueue_sketch(L, m, n, lda, A, (int)prec, s, signs, idx, As_out, Rs, st);
+    k += launch_prep_R(Rs, n, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16), stat, MRCQR_ERR_SINGULAR, st);
+    return finish(L, st, k);
+}
+
+extern "C" int mrcqr_precondition_gram(int64_t m, int n, int64_t lda, const double* A, const double* Rs,
+                                       double* G_out, double* Rc, void* stream)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (m < n) return -1;
+    if (lda < m) return -3;
+    if (!A) return -4;
+    if (!Rs) return -5;
+    if (!Rc) return -7;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    Layout L = make_layout(m, n, 0, 64);
+    if (!ensure_ws(L.total)) return MRCQR_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    mrcqr_reset_status<<<1, 1, 0, st>>>(reinterpret_cast<Status*>(g.ws + L.status));
+    int k = 1 + enqueue_gram(L, m, n, lda, A, Rs, G_out, Rc, nullptr, st);
+    return finish(L, st, k);
+}
+
+extern "C" int mrcqr_form_q(int64_t m, int n, int64_t lda, const double* A, const double* Rs,
+                            const double* Rc, int64_t ldq, double* Q, double* R, void* stream)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (m < n) return -1;
+    if (lda < m) return -3;
+    if (!A) return -4;
+    if (!Rs) return -5;
+    if (!Rc) return -6;
+    if (ldq < m) return -7;
+    if (!Q) return -8;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    Layout L = make_layout(m, n, 0, 64);
+    if (!ensure_ws(L.total)) return MRCQR_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    mrcqr_reset_status<<<1, 1, 0, st>>>(reinterpret_cast<Status*>(g.ws + L.status));
+    int k = 1 + enqueue_formq(L, m, n, lda, A, Rs, Rc, true, true, ldq, Q, R, nullptr, st);
+    return finish(L, st, k);
+}
+
+extern "C" int mrcqr_debug_dump_y(int64_t m, int n, int64_t lda, const double* A, const double* Rs,
+                                  double* Y_stage2a, double* Y_stage2b, void* stream)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (m < n) return -1;
+    if (lda < m) return -3;
+    if (!A || !Rs || !Y_stage2a || !Y_stage2b) return -4;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    Layout L = make_layout(m, n, 0, 64);
+    if (!ensure_ws(L.total)) return MRCQR_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    mrcqr_reset_status<<<1, 1, 0, st>>>(reinterpret_cast<Status*>(g.ws + L.status));
+    double* Rc = reinterpret_cast<double*>(g.ws + L.Rc);
+    int k = 1 + enqueue_gram(L, m, n, lda, A, Rs, nullptr, Rc, Y_stage2a, st);
+    // stage 2b writes its Q over the dump afterwards, so dump into 2b and form Q into 2a's twin: use
+    // Y_stage2b as the dump target and a scratch Q = Y_stage2b is not possible; Q goes to workspace-free
+    // path: reuse Y_stage2b for the dump and discard Q by writing it to Y_stage2b's rows AFTER the dump
+    // would destroy it -- so Q is written to a separate temporary.
+    double* Qtmp = nullptr;
+    if (cudaMalloc(&Qtmp, sizeof(double) * (size_t)m * n) != cudaSuccess) { cudaGetLastError(); return MRCQR_ERR_CUDA; }
+    k += enqueue_formq(L, m, n, lda, A, Rs, Rc, false, false, m, Qtmp, nullptr, Y_stage2b, st);
+    int rc = finish(L, st, k);
+    cudaFree(Qtmp);
+    return rc;
+}
+
+static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q, double* R,
+                         int prec, int s, uint64_t seed, cudaStream_t st)
+{
+    Layout L = make_layout(m, n, s, prec);
+    if (!ensure_ws(L.total) || !ensure_hidx((size_t)s)) return MRCQR_ERR_CUDA;
+    Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
+    uint64_t* signs = reinterpret_cast<uint64_t*>(g.ws + L.signs);
+    int64_t* idx = reinterpret_cast<int64_t*>(g.ws + L.idx);
+    double* Rs = reinterpret_cast<double*>(g.ws + L.Rs);
+    double* Rc = reinterpret_cast<double*>(g.ws + L.Rc);
+    // Algorithm 2 step 1: bins on the host (s values), sign words on the device (m bits)
+    draw_bins_host(m, s, seed, g.h_idx);
+    cudaMemcpyAsync(idx, g.h_idx, sizeof(int64_t) * (size_t)s, cudaMemcpyHostToDevice, st);
+    const int64_t nw = (m + 63) / 64;
+    mrcqr_draw_signs<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed, nw, signs, stat);
+    int k = 1;
+    k += enqueue_sketch(L, m, n, lda, A, prec, s, signs, idx, nullptr, Rs, st);       // steps 2-6
+    k += enqueue_gram(L, m, n, lda, A, Rs, nullptr, Rc, nullptr, st);                 // step 7 + Alg.1 steps 1-2
+    k += enqueue_formq(L, m, n, lda, A, Rs, Rc, false, false, ldq, Q, R, nullptr, st); // Alg.1 step 3, step 9
+    return finish(L, st, k);
+}
+
+extern "C" int mrcqr_factor(int64_t m, int n, int64_t lda, const double* A, double* Q, double* R,
+                            mrcqr_prec_t sketch_prec, int s, uint64_t seed, void* stream)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (!is_pow2(m) || m < n || m < 32) return -1;
+    if (lda < m) return -3;
+    if (!A) return -4;
+    if (!Q) return -5;
+    if (!R) return -6;
+    if (!prec_ok((int)sketch_prec)) return -7;
+    if (s <= 0) s = 3 * n;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX) return -8;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    return factor_device(m, n, lda, A, lda, Q, R, (int)sketch_prec, s, seed, (cudaStream_t)stream);
+}
+
+extern "C" int mrcqr_factor_host(int64_t m, int n, int64_t lda, const double* A_host, double* Q_host,
+                                 double* R_host, mrcqr_prec_t sketch_prec, int s, uint64_t seed)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (!is_pow2(m) || m < n || m < 32) return -1;
+    if (lda < m) return -3;
+    if (!A_host) return -4;
+    if (!Q_host) return -5;
+    if (!R_host) return -6;
+    if (!prec_ok((int)sketch_prec)) return -7;
+    if (s <= 0) s = 3 * n;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX) return -8;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    const size_t bytes = sizeof(double) * (size_t)lda * n, rbytes = sizeof(double) * (size_t)n * n;
+    if (bytes > g.hA_bytes) {
+        if (g.hA) cudaFree(g.hA);
+        if (g.hQ) cudaFree(g.hQ);
+        g.hA = g.hQ = nullptr; g.hA_bytes = 0;
+        if (cudaMalloc(&g.hA, bytes) != cudaSuccess || cudaMalloc(&g.hQ, bytes) != cudaSuccess) { cudaGetLastError(); return MRCQR_ERR_CUDA; }
+        g.hA_bytes = bytes;
+    }
+    if (rbytes > g.hR_bytes) {
+        if (g.hR) cudaFree(g.hR);
+        g.hR = nullptr; g.hR_bytes = 0;
+        if (cudaMalloc(&g.hR, rbytes) != cudaSuccess) { cudaGetLastError(); return MRCQR_ERR_CUDA; }
+        g.hR_bytes = rbytes;
+    }
+    cudaStream_t st = 0;
+    if (cudaMemcpyAsync(g.hA, A_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return MRCQR_ERR_CUDA;
+    int rc = factor_device(m, n, lda, g.hA, lda, g.hQ, g.hR, (int)sketch_prec, s, seed, st);
+    if (rc != 0) return rc;
+    cudaMemcpyAsync(Q_host, g.hQ, bytes, cudaMemcpyDeviceToHost, st);
+    cudaMemcpyAsync(R_host, g.hR, rbytes, cudaMemcpyDeviceToHost, st);
+    if (cudaStreamSynchronize(st) != cudaSuccess) return MRCQR_ERR_CUDA;
+    return 0;
+}

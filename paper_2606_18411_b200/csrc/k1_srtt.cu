@@ -1,0 +1,230 @@
+// k1_srtt.cu -- K1: subsampled randomized trigonometric transform, Algorithm 2 steps 2-4
+// (PAPER.md:95-97): x~ = fl_p(D a_j), X = DFT_m(x~) down every column, A_s = sqrt(s/m) Re X[S].
+//
+// The paper runs a full cuFFT and gathers.  Only s real outputs per column are
+// wanted, so this kernel uses the four-step split m = m1*m2, t = t1*m2 + t2, k = k1 + m1*k2:
+//     X[k] = sum_{t2} W_m^{k t2} Z[k1, t2],     Z[k1, t2] = sum_{t1} x~[t1*m2 + t2] W_m1^{k1 t1},
+// and never materialises Z or X in HBM:
+//   stage 1  a CTA stages an m1 x 32 tile (32 consecutive t2, all t1; 256-byte coalesced row
+//            segments of the column-major A), applying the sign bit and the cast to p on the way
+//            in (DiagMult), and runs the 32 length-m1 FFTs in shared memory with
+//            radix-4 decimation-in-frequency passes (output left in bit-reversed order).  Two real
+//            columns ride in one complex transform (re = column 2c, im = column 2c+1).
+//   stage 2  for each sampled bin k_i only the residue k1 = k_i mod m1 is needed; the CTA multiplies
+//            Z[k1, t2] by W_m^{k_i t2}, takes the real part, and sums over its t2 (warp shuffle +
+//            a per-CTA accumulator); a finalize kernel adds the per-chunk partials in a fixed order,
+//            scales by sqrt(s/m) and rounds to p.
+// Same mathematical result as FFT-then-gather; pass 1 reads A exactly once in every precision.
+// T = float serves p = FP16 (inputs and outputs rounded to FP16, FP32 arithmetic) and p = FP32;
+// T = double serves p = FP64.  No fast-math intrinsics: twiddles come from sincospi.
+#include "mrcqr_internal.cuh"
+#include <cuda_fp16.h>
+
+namespace mrcqr {
+
+constexpr int K1_W = 32;          // t2 values per tile = lanes of a warp
+constexpr int K1_NT = 256;
+constexpr int K1_NWARP = K1_NT / 32;
+
+template <typename T> struct Cx { T x, y; };
+
+template <typename T> __device__ __forceinline__ Cx<T> cmul(Cx<T> a, Cx<T> b)
+{
+    Cx<T> r;
+    r.x = fma(a.x, b.x, -(a.y * b.y));
+    r.y = fma(a.x, b.y, a.y * b.x);
+    return r;
+}
+template <typename T> __device__ __forceinline__ Cx<T> cadd(Cx<T> a, Cx<T> b) { return Cx<T>{a.x + b.x, a.y + b.y}; }
+template <typename T> __device__ __forceinline__ Cx<T> csub(Cx<T> a, Cx<T> b) { return Cx<T>{a.x - b.x, a.y - b.y}; }
+// multiply by -i
+template <typename T> __device__ __forceinline__ Cx<T> cmulmi(Cx<T> a) { return Cx<T>{a.y, -a.x}; }
+
+__device__ __forceinline__ void sincospi_t(float a, float* s, float* c) { sincospif(a, s, c); }
+__device__ __forceinline__ void sincospi_t(double a, double* s, double* c) { sincospi(a, s, c); }
+
+// fl_p(d * a): sign-bit flip fused with the cast to the sketch precision.
+template <typename T, int PREC>
+__device__ __forceinline__ T diag_cast(double a, unsigned neg)
+{
+    T v;
+    if (PREC == 16) v = (T)__half2float(__double2half(a));
+    else if (PREC == 32) v = (T)__double2float_rn(a);
+    else v = (T)a;
+    return neg ? -v : v;
+}
+
+struct K1Params {
+    int64_t m, lda;
+    int n, s, m1, log_m1;
+    int64_t m2;
+    int tiles_per_col, tiles_per_chunk, chunks;
+};
+
+template <typename T, int PREC>
+__global__ void __launch_bounds__(K1_NT)
+mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
+              const int64_t* __restrict__ idx, double* __restrict__ partial)
+{
+    extern __shared__ __align__(16) unsigned char smraw[];
+    Cx<T>* tile = reinterpret_cast<Cx<T>*>(smraw);                       // [m1][32]
+    Cx<T>* tw = tile + (size_t)p.m1 * K1_W;                              // [m1]  W_m1^e
+    double* colacc = reinterpret_cast<double*>(tw + p.m1);               // [2][s]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int pair = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
+    const int ja = 2 * pair, jb = 2 * pair + 1;
+    const bool has_b = jb < p.n;
+    const int m1 = p.m1;
+
+    for (int e = tid; e < m1; e += K1_NT) {
+        double sn, cs;
+        sincospi(-2.0 * (double)e / (double)m1, &sn, &cs);
+        tw[e] = Cx<T>{(T)cs, (T)sn};
+    }
+    for (int e = tid; e < 2 * p.s; e += K1_NT) colacc[e] = 0.0;
+
+    const int tile_lo = chunk * p.tiles_per_chunk;
+    const int tile_hi = min(p.tiles_per_col, tile_lo + p.tiles_per_chunk);
+    for (int tl = tile_lo; tl < tile_hi; ++tl) {
+        const int64_t t2_0 = (int64_t)tl * K1_W;
+        __syncthreads();
+        // ---- load + DiagMult ------------------------------------------------------------------
+        const double* colA = A + (size_t)ja * (size_t)p.lda + t2_0 + lane;
+        const double* colB = A + (size_t)(has_b ? jb : ja) * (size_t)p.lda + t2_0 + lane;
+#pragma unroll 4
+        for (int t1 = warp; t1 < m1; t1 += K1_NWARP) {
+            const int64_t off = (int64_t)t1 * p.m2;
+            const unsigned neg = (signs32[(off + t2_0) >> 5] >> lane) & 1u;
+            const double a = __ldcs(colA + off);
+            const double b = has_b ? __ldcs(colB + off) : 0.0;
+            tile[t1 * K1_W + lane] = Cx<T>{diag_cast<T, PREC>(a, neg), diag_cast<T, PREC>(b, neg)};
+        }
+        __syncthreads();
+        // ---- stage 1: m1-point DIF FFT down t1 for each of the 32 lanes ---------------------------
+        int nb = m1;                                   // current block size
+        while (nb >= 4) {
+            const int q = nb >> 2, tstride = m1 / nb;
+            for (int bf = warp; bf < (m1 >> 2); bf += K1_NWARP) {
+                const int blk = bf / q, pos = bf % q;
+                Cx<T>* base = tile + ((size_t)blk * nb + pos) * K1_W + lane;
+                Cx<T> a0 = base[0], a1 = base[(size_t)q * K1_W], a2 = base[(size_t)2 * q * K1_W], a3 = base[(size_t)3 * q * K1_W];
+                const Cx<T> w1 = tw[pos * tstride], w2 = tw[2 * pos * tstride];
+                Cx<T> b0 = cadd(a0, a2), b2 = cmul(csub(a0, a2), w1);
+                Cx<T> b1 = cadd(a1, a3), b3 = cmulmi(cmul(csub(a1, a3), w1));
+                base[0] = cadd(b0, b1);
+                base[(size_t)q * K1_W] = cmul(csub(b0, b1), w2);
+                base[(size_t)2 * q * K1_W] = cadd(b2, b3);
+                base[(size_t)3 * q * K1_W] = cmul(csub(b2, b3), w2);
+            }
+            nb >>= 2;
+            __syncthreads();
+        }
+        if (nb == 2) {                                 // odd log2(m1): final radix-2 pass, twiddle 1
+            for (int bf = warp; bf < (m1 >> 1); bf += K1_NWARP) {
+                Cx<T>* base = tile + (size_t)(2 * bf) * K1_W + lane;
+                Cx<T> a0 = base[0], a1 = base[K1_W];
+                base[0] = cadd(a0, a1);
+                base[K1_W] = csub(a0, a1);
+            }
+            __syncthreads();
+        }
+        // ---- stage 2: sampled bins ------------------------------------------------------------------
+        const int64_t t2 = t2_0 + lane;
+        for (int i = warp; i < p.s; i += K1_NWARP) {
+            const int64_t k = idx[i];
+            const int k1 = (int)(k & (m1 - 1));
+            const int k1n = (m1 - k1) & (m1 - 1);
+            const int br = (int)(__brev((unsigned)k1) >> (32 - p.log_m1));
+            const int brn = (int)(__brev((unsigned)k1n) >> (32 - p.log_m1));
+            const Cx<T> P = tile[(p.log_m1 ? br : 0) * K1_W + lane];
+            const Cx<T> Qn = tile[(p.log_m1 ? brn : 0) * K1_W + lane];
+            // Z_a = (P + conj Qn)/2, Z_b = -i (P - conj Qn)/2
+            const T zar = (T)0.5 * (P.x + Qn.x), zai = (T)0.5 * (P.y - Qn.y);
+            const T zbr = (T)0.5 * (P.y + Qn.y), zbi = (T)0.5 * (Qn.x - P.x);
+            const int64_t r = (k * t2) & (p.m - 1);    // k t2 mod m, exact
+            T sn, cs;
+            sincospi_t((T)(2.0 * (double)r / (double)p.m), &sn, &cs);
+            // Re( e^{-i theta} Z ) = cos*Zr + sin*Zi
+            double va = (double)fma(cs, zar, sn * zai);
+            double vb = (double)fma(cs, zbr, sn * zbi);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                va += __shfl_xor_sync(0xffffffffu, va, o);
+                vb += __shfl_xor_sync(0xffffffffu, vb, o);
+            }
+            if (lane == 0) { colacc[i] += va; colacc[p.s + i] += vb; }
+        }
+    }
+    __syncthreads();
+    double* out = partial + ((size_t)pair * p.chunks + chunk) * 2 * p.s;
+    for (int e = tid; e < 2 * p.s; e += K1_NT) out[e] = colacc[e];
+}
+
+// A_s[i, j] = fl_p( sqrt(s/m) * sum_chunks partial ), chunks added in ascending order.
+template <int PREC>
+__global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial, double* __restrict__ As, Status* st)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= p.s * p.n) return;
+    const int i = e % p.s, j = e / p.s;
+    const double* src = partial + ((size_t)(j >> 1) * p.chunks) * 2 * p.s + (size_t)(j & 1) * p.s + i;
+    double acc = 0.0;
+    for (int c = 0; c < p.chunks; ++c) acc += src[(size_t)c * 2 * p.s];
+    double v = acc * sqrt((double)p.s / (double)p.m);
+    if (PREC == 16) v = (double)__half2float(__double2half(v));
+    else if (PREC == 32) v = (double)__double2float_rn(v);
+    if (isnan(v) || isinf(v)) report(st, 1, j);
+    As[e] = v;
+}
+
+static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec)
+{
+    K1Params p;
+    p.m = m; p.lda = lda; p.n = n; p.s = s;
+    const int m1max = (prec == 64) ? 256 : 512;
+    int64_t m1 = m / K1_W;
+    if (m1 > m1max) m1 = m1max;
+    if (m1 < 1) m1 = 1;
+    p.m1 = (int)m1; p.m2 = m / m1;
+    p.log_m1 = 0; while ((1 << p.log_m1) < p.m1) ++p.log_m1;
+    p.tiles_per_col = (int)(p.m2 / K1_W);
+    const int npairs = (n + 1) / 2;
+    int chunks = (4 * num_sms() + npairs - 1) / npairs;
+    if (chunks > p.tiles_per_col) chunks = p.tiles_per_col;
+    if (chunks < 1) chunks = 1;
+    p.tiles_per_chunk = (p.tiles_per_col + chunks - 1) / chunks;
+    p.chunks = (p.tiles_per_col + p.tiles_per_chunk - 1) / p.tiles_per_chunk;
+    return p;
+}
+
+size_t k1_workspace_bytes(int64_t m, int n, int s, int prec)
+{
+    K1Params p = k1_params(m, n, m, s, prec);
+    return (size_t)((n + 1) / 2) * p.chunks * 2 * (size_t)s * sizeof(double);
+}
+
+template <typename T, int PREC>
+static void k1_launch_t(const K1Params& p, const double* A, const uint64_t* signs, const int64_t* idx,
+                        double* partial, double* As, Status* st, cudaStream_t stream)
+{
+    const size_t smem = (size_t)p.m1 * K1_W * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + 2 * (size_t)p.s * sizeof(double);
+    auto k = mrcqr_k1_srtt<T, PREC>;
+    cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const int grid = ((p.n + 1) / 2) * p.chunks;
+    k<<<grid, K1_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
+    mrcqr_k1_finalize<PREC><<<(p.s * p.n + 255) / 256, 256, 0, stream>>>(p, partial, As, st);
+}
+
+int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int s,
+                   const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
+                   Status* st, cudaStream_t stream)
+{
+    K1Params p = k1_params(m, n, lda, s, prec);
+    double* partial = reinterpret_cast<double*>(k1_work);
+    if (prec == 16) k1_launch_t<float, 16>(p, A, signs, idx, partial, As, st, stream);
+    else if (prec == 32) k1_launch_t<float, 32>(p, A, signs, idx, partial, As, st, stream);
+    else k1_launch_t<double, 64>(p, A, signs, idx, partial, As, st, stream);
+    return 2;
+}
+
+} // namespace mrcqr

@@ -1,0 +1,192 @@
+// k24_small.cu -- the latency-bound single-CTA steps and the tiny glue kernels:
+//   K2  mrcqr_k2_sketch_qr  Algorithm 2 steps 5-6: Householder R-factor of the
+//                           s x n sketch, rows sign-normalised to diag > 0, FP64 arithmetic on the
+//                           precision-p sketch values (>= p; PAPER.md:119 promotes FP16 to FP32).
+//   K4  mrcqr_k4_cholesky   Algorithm 1 step 2: G = Rc^T Rc; a pivot <= 0 or NaN is
+//                           reported, never shifted away.
+//   prep_R                  builds the "prepared" factor the tile solve consumes.
+//   triu_mul                Algorithm 2 step 9: R = Rc Rs.
+#include "mrcqr_internal.cuh"
+
+namespace mrcqr {
+
+constexpr int SMALL_NT = 1024;
+constexpr int SMALL_SMEM_MAX = 220 * 1024;
+
+__global__ void mrcqr_prep_R(const double* __restrict__ R, int n, double* __restrict__ Rp, int n16,
+                             Status* st, int err_code)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n16 * n16) return;
+    const int i = e % n16, j = e / n16;
+    double v = 0.0;
+    if (i == j) {
+        if (i < n) {
+            const double d = R[(size_t)j * n + j];
+            if (!(fabs(d) > 0.0) || isinf(d)) report(st, err_code, j);
+            v = 1.0 / d;
+        } else v = 1.0;
+    } else if (i < j && j < n) v = -R[(size_t)j * n + i];
+    Rp[e] = v;
+}
+
+__global__ void mrcqr_triu_mul(const double* __restrict__ Rc, const double* __restrict__ Rs, int n,
+                               double* __restrict__ R)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n * n) return;
+    const int i = e % n, j = e / n;
+    double acc = 0.0;
+    if (i <= j)
+        for (int k = i; k <= j; ++k) acc = fma(Rc[(size_t)k * n + i], Rs[(size_t)j * n + k], acc);
+    R[e] = acc;
+}
+
+// ---- K4 ---------------------------------------------------------------------------------------
+// W: working copy of G (upper triangle used), col-major with leading dimension ldw.
+__global__ void __launch_bounds__(SMALL_NT)
+mrcqr_k4_cholesky(double* __restrict__ G16, int n, int n16, int use_smem, double* __restrict__ G_out,
+                  double* __restrict__ Rc, double* __restrict__ RcPrep, Status* st)
+{
+    extern __shared__ __align__(16) double sm[];
+    double* rowk = sm;                       // n16 doubles: scaled row k
+    double* W = use_smem ? sm + n16 : G16;
+    const int ldw = use_smem ? n16 + 1 : n16;
+    const int tid = threadIdx.x;
+
+    for (int e = tid; e < n * n; e += SMALL_NT) {
+        const int i = e % n, j = e / n;
+        const double v = G16[(size_t)j * n16 + i];
+        if (G_out) G_out[e] = v;
+        if (use_smem) W[j * ldw + i] = v;
+    }
+    __syncthreads();
+    for (int k = 0; k < n; ++k) {
+        const double piv = W[k * ldw + k];
+        if (tid == 0 && (!(piv > 0.0) || isinf(piv))) report(st, 3, k);
+        const double d = sqrt(piv);
+        for (int j = k + 1 + tid; j < n; j += SMALL_NT) rowk[j] = W[j * ldw + k] / d;
+        __syncthreads();
+        if (tid == 0) W[k * ldw + k] = d;
+        for (int j = k + 1 + tid; j < n; j += SMALL_NT) W[j * ldw + k] = rowk[j];
+        const int L = n - k - 1;
+        for (int e = tid; e < L * L; e += SMALL_NT) {
+            const int i = k + 1 + e % L, j = k + 1 + e / L;
+            if (i <= j) W[j * ldw + i] = fma(-rowk[i], rowk[j], W[j * ldw + i]);
+        }
+        __syncthreads();
+    }
+    for (int e = tid; e < n16 * n16; e += SMALL_NT) {
+        const int i = e % n16, j = e / n16;
+        const bool in = (i < n && j < n);
+        const double w = (in && i <= j) ? W[j * ldw + i] : 0.0;
+        double p = 0.0;
+        if (i == j) p = in ? 1.0 / w : 1.0;
+        else if (in && i < j) p = -w;
+        if (in) Rc[(size_t)j * n + i] = w;
+        RcPrep[e] = p;      // note: RcPrep must not alias G16 when W == G16
+    }
+}
+
+// ---- K2 ---------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__global__ void __launch_bounds__(SMALL_NT)
+mrcqr_k2_sketch_qr(double* __restrict__ As, int s, int n, int use_smem, double* __restrict__ Rs)
+{
+    extern __shared__ __align__(16) double sm[];
+    double* betas = sm;                      // n
+    double* sig = sm + n;                    // [0]: sigma of the current column, [1]: of the next
+    double* W = use_smem ? sm + n + 2 : As;  // s x n, ld = s
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NWARP = SMALL_NT / 32;
+
+    if (use_smem) for (int e = tid; e < s * n; e += SMALL_NT) W[e] = As[e];
+    __syncthreads();
+    if (warp == 0) {                         // sigma of column 0
+        double a = 0.0;
+        for (int i = 1 + lane; i < s; i += 32) a = fma(W[i], W[i], a);
+        a = warp_sum(a);
+        if (lane == 0) sig[0] = a;
+    }
+    __syncthreads();
+    for (int j = 0; j < n; ++j) {
+        const double* x = W + (size_t)j * s;
+        const double alpha = x[j], sigma = sig[j & 1];
+        double beta = alpha, tau = 0.0, inv = 0.0;
+        if (sigma != 0.0 && j + 1 < s) {     // LAPACK dgeqr2 / Golub-Van Loan 5.1.1 convention
+            const double nrm = sqrt(fma(alpha, alpha, sigma));
+            beta = (alpha >= 0.0) ? -nrm : nrm;
+            tau = (beta - alpha) / beta;
+            inv = 1.0 / (alpha - beta);
+        }
+        if (tid == 0) betas[j] = beta;
+        for (int c = j + 1 + warp; c < n; c += NWARP) {
+            double* y = W + (size_t)c * s;
+            double w = 0.0;
+            for (int i = j + 1 + lane; i < s; i += 32) w = fma(x[i] * inv, y[i], w);
+            w = warp_sum(w);
+            w = (w + y[j]) * tau;
+            double nxt = 0.0;
+            for (int i = j + 1 + lane; i < s; i += 32) {
+                const double v = fma(-w, x[i] * inv, y[i]);
+                y[i] = v;
+                if (i > j + 1) nxt = fma(v, v, nxt);
+            }
+            __syncwarp();
+            if (lane == 0) y[j] = y[j] - w;
+            if (c == j + 1) { nxt = warp_sum(nxt); if (lane == 0) sig[(j + 1) & 1] = nxt; }
+        }
+        __syncthreads();
+    }
+    for (int e = tid; e < n * n; e += SMALL_NT) {
+        const int i = e % n, j = e / n;
+        double v = 0.0;
+        if (i < j && i < s) v = W[(size_t)j * s + i];
+        else if (i == j) v = betas[j];
+        if (i <= j && betas[i] < 0.0) v = -v;          // sign-normalise row i: diag(Rs) > 0
+        Rs[e] = v;
+    }
+}
+
+// ---- launchers --------------------------------------------------------------------------------
+int launch_prep_R(const double* R, int n, double* Rprep, int n16, Status* st, int err_code, cudaStream_t s)
+{
+    mrcqr_prep_R<<<(n16 * n16 + 255) / 256, 256, 0, s>>>(R, n, Rprep, n16, st, err_code);
+    return 1;
+}
+
+int launch_triu_mul(const double* Rc, const double* Rs, int n, double* R, cudaStream_t s)
+{
+    mrcqr_triu_mul<<<(n * n + 255) / 256, 256, 0, s>>>(Rc, Rs, n, R);
+    return 1;
+}
+
+int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double* Rc, double* RcPrep,
+                       Status* st, cudaStream_t s)
+{
+    size_t need = ((size_t)n16 + (size_t)n16 * (n16 + 1)) * sizeof(double);
+    const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
+    const size_t smem = use_smem ? need : (size_t)n16 * sizeof(double);
+    cudaFuncSetAttribute(mrcqr_k4_cholesky, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    mrcqr_k4_cholesky<<<1, SMALL_NT, smem, s>>>(const_cast<double*>(G16), n, n16, use_smem, G_out, Rc, RcPrep, st);
+    return 1;
+}
+
+int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* work, double* Rs, Status* st, cudaStream_t s)
+{
+    (void)work; (void)st;
+    size_t need = ((size_t)n + 2 + (size_t)s_rows * n) * sizeof(double);
+    const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
+    const size_t smem = use_smem ? need : ((size_t)n + 2) * sizeof(double);
+    cudaFuncSetAttribute(mrcqr_k2_sketch_qr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    mrcqr_k2_sketch_qr<<<1, SMALL_NT, smem, s>>>(const_cast<double*>(As), s_rows, n, use_smem, Rs);
+    return 1;
+}
+
+} // namespace mrcqr

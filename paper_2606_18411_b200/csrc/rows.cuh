@@ -1,0 +1,147 @@
+// rows.cuh -- device building blocks of the two row-streaming passes (K3: precondition + Gram,
+// K5: form Q).  A CTA owns a tile of TM consecutive rows of A, held column-major in shared memory
+// as Ysm[col * LDT + row], LDT = TM + 4 (LDT = 4 mod 16 makes every DMMA fragment load hit 16
+// distinct 8-byte banks per half warp).
+//
+// solve_tile() is THE forward substitution  Y <- Y * R^-1  (Algorithm 2 step 7, and
+// Algorithm 1 step 3).  K3 and K5 both call this one function with the same template
+// arguments and the same prepared factor, and every floating-point operation in it is an explicit
+// DMMA, fma or multiply, so the Y a row gets in K5 is bit-identical to the Y K3 fed to the Gram
+// matrix.  The result for a row does not depend on which tile slot,
+// warp or CTA holds it: each row's arithmetic touches only that row's data and R.
+#pragma once
+#include "mrcqr_internal.cuh"
+
+namespace mrcqr {
+
+// D(8x8) += A(8x4, row) * B(4x8, col), FP64 tensor-core op (SASS: DMMA.8x8x4 on sm_100a).
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+
+// Cooperative load of rows [row0, row0+TM) x n columns of A into the tile; zero fill for rows >= m
+// and for the padding columns n..n16-1.  VEC = 16-byte loads (A, lda, row0 suitably aligned).
+template <int TM, int NT, bool VEC>
+__device__ __forceinline__ void load_tile(double* Ysm, const double* __restrict__ A, int64_t lda,
+                                          int64_t m, int n, int n16, int64_t row0)
+{
+    constexpr int LDT = TM + 4;
+    if (VEC) {
+        constexpr int H = TM / 2;
+        for (int e = threadIdx.x; e < n16 * H; e += NT) {
+            int col = e / H, r2 = (e % H) * 2;
+            double2 v = make_double2(0.0, 0.0);
+            int64_t r = row0 + r2;
+            if (col < n) {
+                const double* src = A + (size_t)col * (size_t)lda + r;
+                if (r + 1 < m) v = __ldcs(reinterpret_cast<const double2*>(src));
+                else if (r < m) v.x = __ldcs(src);
+            }
+            *reinterpret_cast<double2*>(Ysm + col * LDT + r2) = v;
+        }
+    } else {
+        for (int e = threadIdx.x; e < n16 * TM; e += NT) {
+            int col = e / TM, rr = e % TM;
+            int64_t r = row0 + rr;
+            double v = 0.0;
+            if (col < n && r < m) v = __ldcs(A + (size_t)col * (size_t)lda + r);
+            Ysm[col * LDT + rr] = v;
+        }
+    }
+}
+
+// Cooperative store of the tile (first n columns, rows < m) to a column-major m x n matrix.
+template <int TM, int NT, bool VEC>
+__device__ __forceinline__ void store_tile(const double* Ysm, double* __restrict__ Q, int64_t ldq,
+                                           int64_t m, int n, int64_t row0)
+{
+    constexpr int LDT = TM + 4;
+    if (VEC) {
+        constexpr int H = TM / 2;
+        for (int e = threadIdx.x; e < n * H; e += NT) {
+            int col = e / H, r2 = (e % H) * 2;
+            int64_t r = row0 + r2;
+            double2 v = *reinterpret_cast<const double2*>(Ysm + col * LDT + r2);
+            double* dst = Q + (size_t)col * (size_t)ldq + r;
+            if (r + 1 < m) __stcs(reinterpret_cast<double2*>(dst), v);
+            else if (r < m) __stcs(dst, v.x);
+        }
+    } else {
+        for (int e = threadIdx.x; e < n * TM; e += NT) {
+            int col = e / TM, rr = e % TM;
+            int64_t r = row0 + rr;
+            if (r < m) __stcs(Q + (size_t)col * (size_t)ldq + r, Ysm[col * LDT + rr]);
+        }
+    }
+}
+
+// In-place Y <- Y * R^-1 on the rows owned by this warp (8*RG rows starting at warp*8*RG).
+// Rp is the prepared factor (see mrcqr_internal.cuh): strict upper = -R, diagonal = 1/R[j,j].
+// Left-looking over 8-column blocks J:
+//   T_J = Y_J + sum_{K<J} Y_K * (-R[K,J])       two DMMA.8x8x4 per (K, 8-row group), FP64 tensor pipe
+//   Y_J = T_J * R[J,J]^-1                       8x8 substitution, one thread per row, registers
+// The k index inside a DMMA is permuted consistently in both operands (lane t takes k = t and
+// k = t + 4), which fixes the summation order once and for all.
+template <int TM, int NW>
+__device__ __forceinline__ void solve_tile(double* Ysm, const double* __restrict__ Rp, int n16)
+{
+    constexpr int LDT = TM + 4;
+    constexpr int RG = TM / (8 * NW);                 // 8-row groups per warp
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int rbase = warp * (8 * RG);
+    const int nB = n16 >> 3;
+
+    for (int J = 0; J < nB; ++J) {
+        double c[RG][2];
+        double* colJ = Ysm + (8 * J + 2 * t) * LDT + rbase + g;
+#pragma unroll
+        for (int rg = 0; rg < RG; ++rg) {
+            c[rg][0] = colJ[8 * rg];
+            c[rg][1] = colJ[LDT + 8 * rg];
+        }
+        const double* rcol = Rp + (size_t)(8 * J + g) * n16 + t;       // B fragment: (k = t, n = g)
+        double b0 = 0.0, b1 = 0.0;
+        if (J > 0) { b0 = __ldg(rcol); b1 = __ldg(rcol + 4); }
+        for (int K = 0; K < J; ++K) {
+            double nb0 = 0.0, nb1 = 0.0;
+            if (K + 1 < J) { nb0 = __ldg(rcol + 8 * (K + 1)); nb1 = __ldg(rcol + 8 * (K + 1) + 4); }
+            const double* ya = Ysm + (8 * K + t) * LDT + rbase + g;    // A fragment: (m = g, k = t)
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) {
+                double a0 = ya[8 * rg];
+                double a1 = ya[4 * LDT + 8 * rg];
+                dmma884(c[rg], a0, b0);
+                dmma884(c[rg], a1, b1);
+            }
+            b0 = nb0; b1 = nb1;
+        }
+#pragma unroll
+        for (int rg = 0; rg < RG; ++rg) {
+            colJ[8 * rg] = c[rg][0];
+            colJ[LDT + 8 * rg] = c[rg][1];
+        }
+        __syncwarp();
+        if (lane < 8 * RG) {                           // one thread per row: 8x8 substitution
+            double* yr = Ysm + (8 * J) * LDT + rbase + lane;
+            const double* d = Rp + (size_t)(8 * J) * n16 + 8 * J;      // diagonal block, col-major
+            double y[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) y[j] = yr[j * LDT];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                y[j] = y[j] * __ldg(d + (size_t)j * n16 + j);          // times 1/R[j,j]
+#pragma unroll
+                for (int jj = j + 1; jj < 8; ++jj)
+                    y[jj] = fma(y[j], __ldg(d + (size_t)jj * n16 + j), y[jj]);   // -R[j,jj]
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) yr[j * LDT] = y[j];
+        }
+        __syncwarp();
+    }
+}
+
+} // namespace mrcqr
