@@ -1,0 +1,288 @@
+#!/usr/bin/env python
+"""bench.py -- MRCQR FP64 thin-QR benchmark (BASELINE.json metric: ms per factorization at m x n,
+achieved HBM GB/s and FP64 TFLOP/s against the B200's measured peaks).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C1|C0|C2|C3]
+
+A "step" is one pass of the whole hot path (mrcqr_factor: draw, K1..K5) over the synthetic
+matrix of BASELINE.json configs[1] (C1: m = 2^20, n = 64, FP16 sketch, s = 128), already resident
+in HBM.  `e2e` is the same factorization through mrcqr_factor_host with pinned HOST buffers
+(H2D of A, D2H of Q and R inside the timed region).  The path does not shard (SURVEY.md 8(e):
+"replicas only"): with N > 1 every rank factors its own replica; the value stays ms per
+factorization of the slowest rank and `factorizations_per_s` aggregates the ranks.
+--impl reference times the CPU oracle (oracle/) on the host cores, rank 0 only.
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "MRCQR FP64 thin-QR ms per factorization"
+FP64_DMMA_PEAK_TFLOPS = 37.2      # measured on this pool's B200 (profiles/r01_peaks.md), DMMA.8x8x4 issue peak
+HBM_FALLBACK_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.idx, self.proc = gpu_index, None
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.tmp.flush()
+        rows = [l.strip().split(",") for l in open(self.tmp.name) if l.strip()]
+        os.unlink(self.tmp.name)
+        sm, reasons = [], set()
+        for r in rows:
+            try:
+                r = [x.strip() for x in r]
+                sm.append(float(r[1])); out["sm_max_mhz"] = float(r[2])
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                pass
+        if sm:
+            sm.sort()
+            out["sm_mhz"] = sm[len(sm) // 2]
+        out["reasons"] = sorted(reasons)
+        out["samples"] = len(sm)
+        return out
+
+
+def workload(name):
+    from paper_2606_18411_b200 import inputs
+    cfg = dict(inputs.CONFIGS[name])
+    cfg["name"] = name
+    return cfg
+
+
+def config_json(cfg, extra=None):
+    c = {"workload": "%s: m=%d n=%d s=%d sketch=fp%d kappa~1e%d, A=G*diag(sigma)*V^T seeds %d/%d/%d" % (
+        cfg["name"], cfg["m"], cfg["n"], cfg["s"], cfg["prec"], cfg["exponent"],
+        cfg["seed_G"], cfg["seed_V"], cfg["seed_draw"]),
+        "m": cfg["m"], "n": cfg["n"], "s": cfg["s"], "sketch_prec": "fp%d" % cfg["prec"],
+        "l2": "inputs larger than L2 (A = %.0f MB read 3x, Q = %.0f MB written per step)" % (
+            8e-6 * cfg["m"] * cfg["n"], 8e-6 * cfg["m"] * cfg["n"]),
+        "parallelism": "replicas only (path does not shard)"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+def oracle_sample(cfg):
+    """The bounded CPU sample: the whole factorization when it is seconds of work (C0, C1, C2), else
+    the first 2^18 rows of the same matrix (the oracle's cost is linear in m, so ms scales by m/2^18)."""
+    full_flops = 4.0 * cfg["m"] * cfg["n"] ** 2
+    if full_flops <= 1.5e11:
+        return cfg["m"], 1.0, "whole factorization (all %d rows)" % cfg["m"]
+    rows = 1 << 18
+    return rows, cfg["m"] / rows, "first 2^18 rows of A, time scaled by m/2^18 = %g" % (cfg["m"] / rows)
+
+
+def time_oracle(cfg, A_np, steps, warmup):
+    import oracle
+    rows, scale, what = oracle_sample(cfg)
+    A = A_np[:rows]
+    s = cfg["s"]
+    signs, idx = oracle.draw(rows, s, cfg["seed_draw"])
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        out = oracle.factor_from_draw(A, signs, idx)
+        dt = time.perf_counter() - t0
+        assert out["rc"] == 0
+        if it >= warmup:
+            times.append(dt * 1e3 * scale)
+    ms = sum(times) / len(times)
+    return ms, {"value": ms, "unit": "ms", "cores": oracle.num_threads(), "kind": "oracle", "sample": what}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, timed on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import torch
+    from paper_2606_18411_b200 import inputs
+    cfg = workload(args.config)
+    AT = inputs.make_config(cfg, "cuda" if torch.cuda.is_available() else "cpu").cpu()
+    A_np = AT.numpy().T
+    steps, warmup = max(1, min(args.steps, 3)), min(args.warmup, 1)
+    ms, cpu = time_oracle(cfg, A_np, steps, warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": args.gpus,
+            "steps": steps, "warmup": warmup, "ms_per_step": ms, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_json(cfg), "cpu_baseline": cpu,
+            "e2e": {"value": ms, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_18411_b200 import binding as B
+    from paper_2606_18411_b200 import inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()
+    cfg = workload(args.config)
+    m, n, s, prec, seed = cfg["m"], cfg["n"], cfg["s"], cfg["prec"], cfg["seed_draw"]
+    AT = inputs.make_config(cfg, "cuda")
+    QT = torch.empty_like(AT)
+    R = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    B.mrcqr_set_timing(True)
+    for _ in range(args.warmup):
+        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
+    sampler = ClockSampler(local)
+    stage_sum = {k: 0.0 for k in B.STAGES}
+    launches = 0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    for _ in range(args.steps):
+        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
+        launches += B.mrcqr_last_launch_count()
+        for k, v in B.mrcqr_last_timing().items():
+            stage_sum[k] += v
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    total_ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms = total_ms / args.steps
+    stages = {k: v / args.steps for k, v in stage_sum.items()}
+
+    # ---- end to end: HOST buffers through mrcqr_factor_host (H2D + D2H inside the timed region) ----
+    B.mrcqr_set_timing(False)
+    A_host = torch.empty((n, m), dtype=torch.float64, pin_memory=True)
+    A_host.copy_(AT)
+    Q_host = torch.empty((n, m), dtype=torch.float64, pin_memory=True)
+    R_host = torch.empty((n, n), dtype=torch.float64, pin_memory=True)
+    e2e_steps = max(1, min(args.steps, 5))
+    B.mrcqr_factor_host(A_host, prec, s, seed, Q_host, R_host)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        B.mrcqr_factor_host(A_host, prec, s, seed, Q_host, R_host)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+
+    if rank == 0:
+        hbm_peak, how = measured_peaks()
+        alg_bytes = 32.0 * m * n                       # 3 reads of A + 1 write of Q (north_star)
+        flops = 4.0 * m * n * n                        # 2 solves in K5, 1 solve + Gram in K3
+        # dominant kernel = the slower of K3 / K5; its algorithmic work
+        dom = "k5_form_q" if stages["k5_form_q"] >= stages["k3_gram"] else "k3_gram"
+        dom_flops = 2.0 * m * n * n
+        dom_bytes = (16.0 if dom == "k5_form_q" else 8.0) * m * n
+        dom_ms = stages[dom]
+        t_hbm, t_f64 = dom_bytes / (hbm_peak * 1e9), dom_flops / (FP64_DMMA_PEAK_TFLOPS * 1e12)
+        if t_f64 >= t_hbm:
+            ach = dom_flops / (dom_ms * 1e-3) / 1e12
+            roof = {"bound": "tensor", "achieved": ach, "peak": FP64_DMMA_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": ach / FP64_DMMA_PEAK_TFLOPS, "traffic": None,
+                    "peak_source": "FP64 DMMA peak measured on this pool (profiles/r01_peaks.md); "
+                                   "MEASURED_PEAKS.json has no FP64 figure"}
+        else:
+            ach = dom_bytes / (dom_ms * 1e-3) / 1e9
+            roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                    "traffic": None, "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % how}
+        roof.update({"kernel": dom, "kernel_ms": dom_ms, "algorithmic_bytes": dom_bytes, "algorithmic_flops": dom_flops,
+                     "hbm_gbs_achieved": dom_bytes / (dom_ms * 1e-3) / 1e9})
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            _, cpu = time_oracle(cfg, AT.cpu().numpy().T, 1, 0)
+        line = {"metric": METRIC, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_json(cfg),
+                "factorizations_per_s": world * 1e3 / ms,
+                "pipeline": {"hbm_gbs": alg_bytes / (ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_peak,
+                             "hbm_frac": alg_bytes / (ms * 1e-3) / 1e9 / hbm_peak,
+                             "fp64_tflops": flops / (ms * 1e-3) / 1e12, "fp64_peak_tflops": FP64_DMMA_PEAK_TFLOPS,
+                             "fp64_frac": flops / (ms * 1e-3) / 1e12 / FP64_DMMA_PEAK_TFLOPS,
+                             "stage_ms": stages},
+                "roofline": roof, "cpu_baseline": cpu,
+                "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": 8 * m * n,
+                        "d2h_bytes_per_step": 8 * m * n + 8 * n * n, "steps": e2e_steps},
+                "gpu_launches": launches, "clocks": clocks}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -119,6 +119,16 @@ int mrcqr_last_info(void);
 int mrcqr_last_launch_count(void);
 
 /*
+ * Per-kernel device timing of mrcqr_factor (CUDA events recorded on the call's stream between the
+ * kernels; off by default).  mrcqr_last_timing fills 7 floats, milliseconds of the last
+ * mrcqr_factor / mrcqr_factor_host call:  [0] K1 sampled transform (Alg.2 steps 2-4),  [1] K2 sketch QR
+ * (steps 5-6),  [2] R_s preparation,  [3] K3 precondition + Gram (step 7, Alg.1 step 1),  [4] partial
+ * reduction + K4 Cholesky (Alg.1 step 2),  [5] K5 form Q (Alg.1 step 3),  [6] R = Rc Rs (step 9).
+ */
+int mrcqr_set_timing(int on);
+int mrcqr_last_timing(float* ms_out_host);
+
+/*
  * Test hook for the "bit-identical Y" requirement: runs the stage-2a and the stage-2b
  * tile solves and dumps the Y = A R_s^-1 each of them computed (m x n, ld = m).  The two dumps
  * must be equal bit for bit.

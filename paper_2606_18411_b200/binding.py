@@ -48,8 +48,11 @@ def lib():
         L.mrcqr_workspace_bytes.argtypes = [i64, ci, ci, ci]
         L.mrcqr_debug_dump_y.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
         L.mrcqr_shutdown.restype = None
+        L.mrcqr_set_timing.argtypes = [ci]
+        L.mrcqr_last_timing.argtypes = [vp]
         for f in ("mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
-                  "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y"):
+                  "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
+                  "mrcqr_set_timing", "mrcqr_last_timing"):
             getattr(L, f).restype = ci
         _lib = L
     return _lib
@@ -57,7 +60,9 @@ def lib():
 
 EXPORTS = ["mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
-           "mrcqr_debug_dump_y", "mrcqr_shutdown"]
+           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing"]
+
+STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "reduce_k4_chol", "k5_form_q", "r_mul"]
 
 
 def _stream(stream):
@@ -173,3 +178,14 @@ def mrcqr_last_launch_count():
 
 def mrcqr_shutdown():
     lib().mrcqr_shutdown()
+
+
+def mrcqr_set_timing(on):
+    lib().mrcqr_set_timing(1 if on else 0)
+
+
+def mrcqr_last_timing():
+    """dict stage name -> ms of the last mrcqr_factor call (needs mrcqr_set_timing(True))."""
+    buf = (C.c_float * 7)()
+    lib().mrcqr_last_timing(buf)
+    return {k: float(buf[i]) for i, k in enumerate(STAGES)}

@@ -74,6 +74,7 @@ struct Ctx {
     int64_t* h_idx = nullptr; size_t h_idx_cap = 0;   // pinned staging of the bins
     double* hA = nullptr; double* hQ = nullptr; double* hR = nullptr; size_t hA_bytes = 0, hR_bytes = 0; // host-path device buffers
     int last_info = 0, last_launches = 0;
+    bool timing = false; cudaEvent_t ev[8] = {}; bool ev_ok = false; float stage_ms[8] = {};
     bool have_device = false, probed = false;
 };
 static Ctx g;
@@ -103,6 +104,7 @@ static bool ensure_hidx(size_t count)
 {
     if (count <= g.h_idx_cap) return true;
     if (g.h_idx) cudaFreeHost(g.h_idx);
+    if (g.ev_ok) for (int i = 0; i < 8; ++i) cudaEventDestroy(g.ev[i]);
     g.h_idx_cap = 0;
     if (cudaMallocHost(&g.h_idx, count * sizeof(int64_t)) != cudaSuccess) { g.h_idx = nullptr; return false; }
     g.h_idx_cap = count;
@@ -205,6 +207,7 @@ extern "C" void mrcqr_shutdown(void)
     if (g.ws) cudaFree(g.ws);
     if (g.h_status) cudaFreeHost(g.h_status);
     if (g.h_idx) cudaFreeHost(g.h_idx);
+    if (g.ev_ok) for (int i = 0; i < 8; ++i) cudaEventDestroy(g.ev[i]);
     if (g.hA) cudaFree(g.hA);
     if (g.hQ) cudaFree(g.hQ);
     if (g.hR) cudaFree(g.hR);
@@ -299,6 +302,24 @@ extern "C" int mrcqr_debug_dump_y(int64_t m, int n, int64_t lda, const double* A
     return rc;
 }
 
+static bool timing_events()
+{
+    if (!g.ev_ok) {
+        for (int i = 0; i < 8; ++i) if (cudaEventCreate(&g.ev[i]) != cudaSuccess) return false;
+        g.ev_ok = true;
+    }
+    return true;
+}
+
+extern "C" int mrcqr_set_timing(int on) { g.timing = (on != 0); return 0; }
+
+extern "C" int mrcqr_last_timing(float* ms_out_host)
+{
+    if (!ms_out_host) return -1;
+    for (int i = 0; i < 7; ++i) ms_out_host[i] = g.stage_ms[i];
+    return 0;
+}
+
 static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q, double* R,
                          int prec, int s, uint64_t seed, cudaStream_t st)
 {
@@ -315,10 +336,35 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
     const int64_t nw = (m + 63) / 64;
     mrcqr_draw_signs<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed, nw, signs, stat);
     int k = 1;
-    k += enqueue_sketch(L, m, n, lda, A, prec, s, signs, idx, nullptr, Rs, st);       // steps 2-6
-    k += enqueue_gram(L, m, n, lda, A, Rs, nullptr, Rc, nullptr, st);                 // step 7 + Alg.1 steps 1-2
-    k += enqueue_formq(L, m, n, lda, A, Rs, Rc, false, false, ldq, Q, R, nullptr, st); // Alg.1 step 3, step 9
-    return finish(L, st, k);
+    const bool tm = g.timing && timing_events();
+    double* As = reinterpret_cast<double*>(g.ws + L.As);
+    if (tm) cudaEventRecord(g.ev[0], st);
+    k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);     // steps 2-4
+    if (tm) cudaEventRecord(g.ev[1], st);
+    k += launch_k2_sketch_qr(As, s, n, nullptr, Rs, stat, st);                             // steps 5-6
+    if (tm) cudaEventRecord(g.ev[2], st);
+    {                                                                                      // step 7 + Alg.1 steps 1-2
+        const int n16 = round_up(n, 16);
+        double* RsPrep = reinterpret_cast<double*>(g.ws + L.RsPrep);
+        double* RcPrep = reinterpret_cast<double*>(g.ws + L.RcPrep);
+        double* G16 = reinterpret_cast<double*>(g.ws + L.G16);
+        double* part = reinterpret_cast<double*>(g.ws + L.k3);
+        int np = 0;
+        k += launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st);
+        if (tm) cudaEventRecord(g.ev[3], st);
+        k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, st);
+        if (tm) cudaEventRecord(g.ev[4], st);
+        k += launch_reduce_partials(part, np, n, n16, G16, st);
+        k += launch_k4_cholesky(G16, n, n16, nullptr, Rc, RcPrep, stat, st);
+        if (tm) cudaEventRecord(g.ev[5], st);
+        k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, st);           // Alg.1 step 3
+        if (tm) cudaEventRecord(g.ev[6], st);
+        k += launch_triu_mul(Rc, Rs, n, R, st);                                            // step 9
+        if (tm) cudaEventRecord(g.ev[7], st);
+    }
+    const int rc = finish(L, st, k);
+    if (tm) for (int i = 0; i < 7; ++i) cudaEventElapsedTime(&g.stage_ms[i], g.ev[i], g.ev[i + 1]);
+    return rc;
 }
 
 extern "C" int mrcqr_factor(int64_t m, int n, int64_t lda, const double* A, double* Q, double* R,

@@ -134,10 +134,10 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
             const int64_t k = idx[i];
             const int k1 = (int)(k & (m1 - 1));
             const int k1n = (m1 - k1) & (m1 - 1);
-            const int br = (int)(__brev((unsigned)k1) >> (32 - p.log_m1));
-            const int brn = (int)(__brev((unsigned)k1n) >> (32 - p.log_m1));
-            const Cx<T> P = tile[(p.log_m1 ? br : 0) * K1_W + lane];
-            const Cx<T> Qn = tile[(p.log_m1 ? brn : 0) * K1_W + lane];
+            const int br = p.log_m1 ? (int)(__brev((unsigned)k1) >> (32 - p.log_m1)) : 0;
+            const int brn = p.log_m1 ? (int)(__brev((unsigned)k1n) >> (32 - p.log_m1)) : 0;
+            const Cx<T> P = tile[br * K1_W + lane];
+            const Cx<T> Qn = tile[brn * K1_W + lane];
             // Z_a = (P + conj Qn)/2, Z_b = -i (P - conj Qn)/2
             const T zar = (T)0.5 * (P.x + Qn.x), zai = (T)0.5 * (P.y - Qn.y);
             const T zbr = (T)0.5 * (P.y + Qn.y), zbi = (T)0.5 * (Qn.x - P.x);
