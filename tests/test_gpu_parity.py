@@ -178,12 +178,16 @@ def test_power_of_two_scaling_is_exact(orc):
 
 def test_breakdown_and_errors_are_reported(orc):
     m, n = 4096, 8
-    A = np.zeros((m, n), order="F")
     rng = np.random.default_rng(0)
+    # rank deficient by an exact zero column.  It is the unpaired last column (n odd) so that no
+    # rounding noise of a neighbouring column leaks into it through the two-columns-per-complex-FFT
+    # packing: its sketch is exactly zero and R_s[6,6] = 0.
+    A7 = np.asfortranarray(rng.standard_normal((m, 7)))
+    A7[:, 6] = 0.0
+    rc = B.mrcqr_factor(colmajor_to_dev(A7), 64, 14, 1, check=False)
+    assert rc == 2 and B.mrcqr_last_info() == 6               # PAPER.md:31 assumes rank n
+    A = np.zeros((m, n), order="F")
     A[:, :] = rng.standard_normal((m, n))
-    A[:, 5] = 0.0                                             # rank deficient: exact zero column
-    rc = B.mrcqr_factor(colmajor_to_dev(A), 64, 16, 1, check=False)
-    assert rc == 2 and B.mrcqr_last_info() == 5               # R_s[5,5] = 0 (PAPER.md:31 assumes rank n)
     A[:, 5] = 2.0 * A[:, 2]                                   # numerically dependent column
     QT = torch.empty((n, m), dtype=torch.float64, device="cuda")
     R = torch.empty((n, n), dtype=torch.float64, device="cuda")
