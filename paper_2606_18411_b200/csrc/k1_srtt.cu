@@ -59,10 +59,11 @@ struct K1Params {
     int n, s, m1, log_m1;
     int64_t m2;
     int tiles_per_col, tiles_per_chunk, chunks;
+    int vec;                      // A and lda allow 16-byte loads
 };
 
 template <typename T, int PREC>
-__global__ void __launch_bounds__(K1_NT)
+__global__ void __launch_bounds__(K1_NT, 3)
 mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
               const int64_t* __restrict__ idx, double* __restrict__ partial)
 {
@@ -88,16 +89,50 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
     for (int tl = tile_lo; tl < tile_hi; ++tl) {
         const int64_t t2_0 = (int64_t)tl * K1_W;
         __syncthreads();
-        // ---- load + DiagMult ------------------------------------------------------------------
-        const double* colA = A + (size_t)ja * (size_t)p.lda + t2_0 + lane;
-        const double* colB = A + (size_t)(has_b ? jb : ja) * (size_t)p.lda + t2_0 + lane;
+        // ---- load + DiagMult: 16-byte loads, a warp covers two 256-byte rows per instruction, eight
+        //      row pairs (16 loads per thread) in flight before the first conversion ------------------
+        if (p.vec) {
+            const int half = lane >> 4, pr = lane & 15;           // row within the pair, double2 index
+            const double2* colA = reinterpret_cast<const double2*>(A + (size_t)ja * (size_t)p.lda + t2_0) + pr;
+            const double2* colB = reinterpret_cast<const double2*>(A + (size_t)(has_b ? jb : ja) * (size_t)p.lda + t2_0) + pr;
+            const int64_t m2h = p.m2 >> 1;                          // row stride in double2
+            for (int t1b = 2 * warp; t1b < m1; t1b += 2 * K1_NWARP * 8) {
+                double2 va[8], vb[8];
+                unsigned sg[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int t1 = t1b + u * 2 * K1_NWARP + half;
+                    va[u] = make_double2(0.0, 0.0); vb[u] = va[u]; sg[u] = 0;
+                    if (t1 < m1) {
+                        const int64_t off = (int64_t)t1 * m2h;
+                        va[u] = __ldcs(colA + off);
+                        if (has_b) vb[u] = __ldcs(colB + off);
+                        sg[u] = signs32[((int64_t)t1 * p.m2 + t2_0) >> 5] >> (2 * pr);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int t1 = t1b + u * 2 * K1_NWARP + half;
+                    if (t1 < m1) {
+                        Cx<T> e0{diag_cast<T, PREC>(va[u].x, sg[u] & 1u), diag_cast<T, PREC>(vb[u].x, sg[u] & 1u)};
+                        Cx<T> e1{diag_cast<T, PREC>(va[u].y, (sg[u] >> 1) & 1u), diag_cast<T, PREC>(vb[u].y, (sg[u] >> 1) & 1u)};
+                        Cx<T>* dst = tile + (size_t)t1 * K1_W + 2 * pr;
+                        dst[0] = e0; dst[1] = e1;
+                    }
+                }
+            }
+        }
+        else {                                                    // unaligned A: 8-byte loads
+            const double* colA = A + (size_t)ja * (size_t)p.lda + t2_0 + lane;
+            const double* colB = A + (size_t)(has_b ? jb : ja) * (size_t)p.lda + t2_0 + lane;
 #pragma unroll 4
-        for (int t1 = warp; t1 < m1; t1 += K1_NWARP) {
-            const int64_t off = (int64_t)t1 * p.m2;
-            const unsigned neg = (signs32[(off + t2_0) >> 5] >> lane) & 1u;
-            const double a = __ldcs(colA + off);
-            const double b = has_b ? __ldcs(colB + off) : 0.0;
-            tile[t1 * K1_W + lane] = Cx<T>{diag_cast<T, PREC>(a, neg), diag_cast<T, PREC>(b, neg)};
+            for (int t1 = warp; t1 < m1; t1 += K1_NWARP) {
+                const int64_t off = (int64_t)t1 * p.m2;
+                const unsigned neg = (signs32[(off + t2_0) >> 5] >> lane) & 1u;
+                const double a = __ldcs(colA + off);
+                const double b = has_b ? __ldcs(colB + off) : 0.0;
+                tile[t1 * K1_W + lane] = Cx<T>{diag_cast<T, PREC>(a, neg), diag_cast<T, PREC>(b, neg)};
+            }
         }
         __syncthreads();
         // ---- stage 1: m1-point DIF FFT down t1 for each of the 32 lanes ---------------------------
@@ -181,7 +216,7 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec)
 {
     K1Params p;
     p.m = m; p.lda = lda; p.n = n; p.s = s;
-    const int m1max = (prec == 64) ? 256 : 512;
+    const int m1max = (prec == 64) ? 128 : 256;      // 64 KB tile: three CTAs per SM
     int64_t m1 = m / K1_W;
     if (m1 > m1max) m1 = m1max;
     if (m1 < 1) m1 = 1;
@@ -189,7 +224,7 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec)
     p.log_m1 = 0; while ((1 << p.log_m1) < p.m1) ++p.log_m1;
     p.tiles_per_col = (int)(p.m2 / K1_W);
     const int npairs = (n + 1) / 2;
-    int chunks = (4 * num_sms() + npairs - 1) / npairs;
+    int chunks = (12 * num_sms() + npairs - 1) / npairs;
     if (chunks > p.tiles_per_col) chunks = p.tiles_per_col;
     if (chunks < 1) chunks = 1;
     p.tiles_per_chunk = (p.tiles_per_col + chunks - 1) / chunks;
@@ -220,6 +255,7 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
                    Status* st, cudaStream_t stream)
 {
     K1Params p = k1_params(m, n, lda, s, prec);
+    p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
     double* partial = reinterpret_cast<double*>(k1_work);
     if (prec == 16) k1_launch_t<float, 16>(p, A, signs, idx, partial, As, st, stream);
     else if (prec == 32) k1_launch_t<float, 32>(p, A, signs, idx, partial, As, st, stream);

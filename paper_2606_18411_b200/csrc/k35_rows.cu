@@ -21,7 +21,7 @@ RowCfg row_config(int n)
     else if (c.n16 <= 128) { c.TM = 128; c.NW = 8; }
     else if (c.n16 <= 256) { c.TM = 64;  c.NW = 8; }
     else                   { c.TM = 32;  c.NW = 4; }
-    c.smem_bytes = c.n16 * (c.TM + 4) * 8;
+    c.smem_bytes = c.n16 * (c.TM + 4) * 8 + 2 * c.n16 * 64;   // tile + diagonal blocks of Rs and Rc
     c.ctas_per_sm = 0;
     return c;
 }
@@ -33,49 +33,139 @@ __device__ __forceinline__ void sb_to_pq(int sb, int& p, int& q)
     q = qq; p = sb - qq * (qq + 1) / 2;
 }
 
+// ---- Gram accumulation, "row pair" scheme (n16 <= 16 * NW) -----------------------------------------
+// Warp w owns the 8x8 blocks (r, r..nB-1) and (r2, r2..nB-1) of the upper triangle, r = w,
+// r2 = nB-1-w: nB+1 blocks for every warp (perfect balance), accumulators stay in registers for the
+// CTA's whole life, one fragment load per block column serves both rows.
+template <int TM, int NBMAX>
+struct GramPair {
+    static constexpr int NH = NBMAX / 2;
+    double acc1[NBMAX][2];      // block (r,  r + cc),      cc = 0 .. nB-1-r
+    double acc2[NH][2];         // block (r2, nB-1 - e),    e  = 0 .. nB-1-r2 (= r)   -- indexed from the end
+    __device__ __forceinline__ void zero()
+    {
+#pragma unroll
+        for (int b = 0; b < NBMAX; ++b) acc1[b][0] = acc1[b][1] = 0.0;
+#pragma unroll
+        for (int b = 0; b < NH; ++b) acc2[b][0] = acc2[b][1] = 0.0;
+    }
+    // r < r2, or r == r2 (odd nB, middle row: acc2 unused); warps with r > r2 own nothing.
+    // Every register array is indexed by unrolled loop counters only (no local memory).
+    __device__ __forceinline__ void accumulate(const double* Ysm, int nB, int r, int r2)
+    {
+        constexpr int LDT = TM + 4;
+        const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+        if (r > r2) return;
+        const int ne = (r2 != r) ? (nB - r2) : 0;
+        const double* y0 = Ysm + g * LDT + t;
+#pragma unroll 2
+        for (int ks = 0; ks < TM / 4; ++ks) {
+            const double* yk = y0 + 4 * ks;
+            double f[NBMAX], fe[NH];
+#pragma unroll
+            for (int cc = 0; cc < NBMAX; ++cc) f[cc] = (r + cc < nB) ? yk[(8 * (r + cc)) * LDT] : 0.0;
+#pragma unroll
+            for (int e = 0; e < NH; ++e) fe[e] = (e < ne) ? yk[(8 * (nB - 1 - e)) * LDT] : 0.0;
+            const double fr2 = yk[(8 * r2) * LDT];
+#pragma unroll
+            for (int cc = 0; cc < NBMAX; ++cc)
+                if (r + cc < nB) dmma884(acc1[cc], f[0], f[cc]);
+#pragma unroll
+            for (int e = 0; e < NH; ++e)
+                if (e < ne) dmma884(acc2[e], fr2, fe[e]);
+        }
+    }
+    __device__ __forceinline__ void flush(double* part, int n16, int nB, int r, int r2, bool first)
+    {
+        const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+        if (r > r2) return;
+        const int ne = (r2 != r) ? (nB - r2) : 0;
+#pragma unroll
+        for (int cc = 0; cc < NBMAX; ++cc) {
+            if (r + cc < nB) {
+                double* dst = part + (size_t)(8 * (r + cc) + 2 * t) * n16 + 8 * r + g;
+                if (first) { dst[0] = acc1[cc][0]; dst[n16] = acc1[cc][1]; }
+                else { dst[0] += acc1[cc][0]; dst[n16] += acc1[cc][1]; }
+                acc1[cc][0] = acc1[cc][1] = 0.0;
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < NH; ++e) {
+            if (e < ne) {
+                double* dst = part + (size_t)(8 * (nB - 1 - e) + 2 * t) * n16 + 8 * r2 + g;
+                if (first) { dst[0] = acc2[e][0]; dst[n16] = acc2[e][1]; }
+                else { dst[0] += acc2[e][0]; dst[n16] += acc2[e][1]; }
+                acc2[e][0] = acc2[e][1] = 0.0;
+            }
+        }
+    }
+};
+
 // G partial of this CTA: n16 x n16 col-major, blocks (I <= J) of the upper triangle only.
 template <int TM, int NW, bool VEC>
-__global__ void __launch_bounds__(NW * 32)
+__global__ void __launch_bounds__(NW * 32, (TM == 128 && NW == 4) ? 3 : 1)
 mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__ A,
               const double* __restrict__ RsPrep, double* __restrict__ partials,
               int64_t ntiles, double* __restrict__ Ydump)
 {
     extern __shared__ __align__(16) double Ysm[];
     constexpr int LDT = TM + 4, NT = NW * 32;
+    constexpr bool PAIR = (TM == 128);                         // n16 <= 16 * NW for both TM = 128 shapes
+    double* Dsm = Ysm + (size_t)n16 * LDT;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane >> 2, t = lane & 3;
-    const int P = n16 >> 4, NS = P * (P + 1) / 2;
-    const int per_warp = (NS - warp + NW - 1) / NW;            // super-blocks of this warp
-    const int sweeps = (per_warp + GRAM_MAXS - 1) / GRAM_MAXS;
-    const bool persist = ((NS + NW - 1) / NW) <= GRAM_MAXS;    // uniform over the CTA
+    const int nB = n16 >> 3;
     double* part = partials + (size_t)blockIdx.x * n16 * n16;
     constexpr int FLUSH_TILES = GRAM_CHAIN * 4 / TM;
+    load_diag_blocks<NT>(Dsm, RsPrep, n16);
 
-    double acc[GRAM_MAXS][4][2];
-#pragma unroll
-    for (int u = 0; u < GRAM_MAXS; ++u)
-#pragma unroll
-        for (int b = 0; b < 4; ++b) acc[u][b][0] = acc[u][b][1] = 0.0;
-    bool first_flush = true;
-    int since_flush = 0;
+    if (PAIR) {
+        GramPair<TM, 2 * NW> gp;
+        gp.zero();
+        const int r = warp, r2 = nB - 1 - warp;
+        bool first = true;
+        int since = 0;
+        for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const int64_t row0 = tile * TM;
+            __syncthreads();
+            load_tile<TM, NT, VEC>(Ysm, A, lda, m, n, n16, row0);
+            __syncthreads();
+            solve_tile<TM, NW>(Ysm, RsPrep, Dsm, n16);
+            __syncthreads();
+            if (Ydump) store_tile<TM, NT, false>(Ysm, Ydump, m, m, n, row0);
+            gp.accumulate(Ysm, nB, r, r2);
+            ++since;
+            if (since >= FLUSH_TILES || tile + gridDim.x >= ntiles) {
+                gp.flush(part, n16, nB, r, r2, first);
+                first = false; since = 0;
+            }
+        }
+        return;
+    }
 
+    // ---- super-block sweeps (n16 > 128): 16x16 super-blocks, flushed to the L2-resident partial every tile
+    const int P = n16 >> 4, NS = P * (P + 1) / 2;
+    const int per_warp = (NS - warp + NW - 1) / NW;
+    const int sweeps = (per_warp + GRAM_MAXS - 1) / GRAM_MAXS;
+    bool first_tile = true;
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int64_t row0 = tile * TM;
-        __syncthreads();                                        // previous tile fully consumed
+        __syncthreads();
         load_tile<TM, NT, VEC>(Ysm, A, lda, m, n, n16, row0);
         __syncthreads();
-        solve_tile<TM, NW>(Ysm, RsPrep, n16);
+        solve_tile<TM, NW>(Ysm, RsPrep, Dsm, n16);
         __syncthreads();
         if (Ydump) store_tile<TM, NT, false>(Ysm, Ydump, m, m, n, row0);
-        const bool last_tile = (tile + gridDim.x >= ntiles);
-        ++since_flush;
         for (int sw = 0; sw < sweeps; ++sw) {
+            double acc[GRAM_MAXS][4][2];
             int pp[GRAM_MAXS], qq[GRAM_MAXS];
             const int cnt = min(GRAM_MAXS, per_warp - sw * GRAM_MAXS);
 #pragma unroll
             for (int u = 0; u < GRAM_MAXS; ++u) {
                 pp[u] = qq[u] = 0;
                 if (u < cnt) sb_to_pq(warp + NW * (sw * GRAM_MAXS + u), pp[u], qq[u]);
+#pragma unroll
+                for (int b = 0; b < 4; ++b) acc[u][b][0] = acc[u][b][1] = 0.0;
             }
             for (int ks = 0; ks < TM / 4; ++ks) {
                 const double* yk = Ysm + g * LDT + 4 * ks + t;          // fragment (i = g, row = t)
@@ -92,44 +182,44 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
                     }
                 }
             }
-            const bool flush = !persist || last_tile || since_flush >= FLUSH_TILES;
-            if (flush) {
 #pragma unroll
-                for (int u = 0; u < GRAM_MAXS; ++u) {
-                    if (u < cnt) {
+            for (int u = 0; u < GRAM_MAXS; ++u) {
+                if (u < cnt) {
 #pragma unroll
-                        for (int b = 0; b < 4; ++b) {
-                            if (b == 2 && pp[u] == qq[u]) continue;
-                            const int I = 2 * pp[u] + (b >> 1), J = 2 * qq[u] + (b & 1);
-                            double* dst = part + (size_t)(8 * J + 2 * t) * n16 + 8 * I + g;
-                            if (first_flush) { dst[0] = acc[u][b][0]; dst[n16] = acc[u][b][1]; }
-                            else { dst[0] += acc[u][b][0]; dst[n16] += acc[u][b][1]; }
-                            acc[u][b][0] = acc[u][b][1] = 0.0;
-                        }
+                    for (int b = 0; b < 4; ++b) {
+                        if (b == 2 && pp[u] == qq[u]) continue;
+                        const int I = 2 * pp[u] + (b >> 1), J = 2 * qq[u] + (b & 1);
+                        double* dst = part + (size_t)(8 * J + 2 * t) * n16 + 8 * I + g;
+                        if (first_tile) { dst[0] = acc[u][b][0]; dst[n16] = acc[u][b][1]; }
+                        else { dst[0] += acc[u][b][0]; dst[n16] += acc[u][b][1]; }
                     }
                 }
             }
         }
-        if (!persist || since_flush >= FLUSH_TILES) { first_flush = false; since_flush = 0; }
+        first_tile = false;
     }
 }
 
 template <int TM, int NW, bool VEC>
-__global__ void __launch_bounds__(NW * 32)
+__global__ void __launch_bounds__(NW * 32, (TM == 128 && NW == 4) ? 3 : 1)
 mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict__ A,
                const double* __restrict__ RsPrep, const double* __restrict__ RcPrep,
                int64_t ldq, double* __restrict__ Q, int64_t ntiles, double* __restrict__ Ydump)
 {
     extern __shared__ __align__(16) double Ysm[];
-    constexpr int NT = NW * 32;
+    constexpr int LDT = TM + 4, NT = NW * 32;
+    double* DsmS = Ysm + (size_t)n16 * LDT;
+    double* DsmC = DsmS + (size_t)n16 * 8;
+    load_diag_blocks<NT>(DsmS, RsPrep, n16);
+    load_diag_blocks<NT>(DsmC, RcPrep, n16);
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int64_t row0 = tile * TM;
         __syncthreads();
         load_tile<TM, NT, VEC>(Ysm, A, lda, m, n, n16, row0);
         __syncthreads();
-        solve_tile<TM, NW>(Ysm, RsPrep, n16);                  // y = a Rs^-1, same code as K3
+        solve_tile<TM, NW>(Ysm, RsPrep, DsmS, n16);            // y = a Rs^-1, same code as K3
         if (Ydump) { __syncthreads(); store_tile<TM, NT, false>(Ysm, Ydump, m, m, n, row0); __syncthreads(); }
-        solve_tile<TM, NW>(Ysm, RcPrep, n16);                  // q = y Rc^-1
+        solve_tile<TM, NW>(Ysm, RcPrep, DsmC, n16);            // q = y Rc^-1
         __syncthreads();
         store_tile<TM, NT, VEC>(Ysm, Q, ldq, m, n, row0);
     }

@@ -17,12 +17,22 @@ namespace mrcqr {
 // D(8x8) += A(8x4, row) * B(4x8, col), FP64 tensor-core op (SASS: DMMA.8x8x4 on sm_100a).
 __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b)
 {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
+// 16-byte asynchronous global -> shared copy (SASS: LDGSTS), src_bytes < 16 zero-fills the rest.
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src, int src_bytes)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gmem_src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 // Cooperative load of rows [row0, row0+TM) x n columns of A into the tile; zero fill for rows >= m
-// and for the padding columns n..n16-1.  VEC = 16-byte loads (A, lda, row0 suitably aligned).
+// and for the padding columns n..n16-1.  VEC (A, lda, row0 16-byte aligned): every thread fires all
+// of its 16-byte cp.async copies back to back, so the whole tile is in flight at once (no register
+// staging, memory-level parallelism = tile size); the caller waits with cp_async_wait_all().
 template <int TM, int NT, bool VEC>
 __device__ __forceinline__ void load_tile(double* Ysm, const double* __restrict__ A, int64_t lda,
                                           int64_t m, int n, int n16, int64_t row0)
@@ -30,17 +40,20 @@ __device__ __forceinline__ void load_tile(double* Ysm, const double* __restrict_
     constexpr int LDT = TM + 4;
     if (VEC) {
         constexpr int H = TM / 2;
-        for (int e = threadIdx.x; e < n16 * H; e += NT) {
-            int col = e / H, r2 = (e % H) * 2;
-            double2 v = make_double2(0.0, 0.0);
-            int64_t r = row0 + r2;
-            if (col < n) {
-                const double* src = A + (size_t)col * (size_t)lda + r;
-                if (r + 1 < m) v = __ldcs(reinterpret_cast<const double2*>(src));
-                else if (r < m) v.x = __ldcs(src);
-            }
-            *reinterpret_cast<double2*>(Ysm + col * LDT + r2) = v;
+        const int64_t left = m - row0;                  // rows available in this tile (may exceed TM)
+#pragma unroll 8
+        for (int e = threadIdx.x; e < n * H; e += NT) {
+            const int col = e / H, r2 = (e % H) * 2;
+            const int64_t avail = left - r2;
+            const int bytes = avail >= 2 ? 16 : (avail == 1 ? 8 : 0);
+            const double* src = A + (size_t)col * (size_t)lda + row0 + (bytes ? r2 : 0);
+            cp_async16(Ysm + col * LDT + r2, src, bytes);
         }
+        for (int e = threadIdx.x; e < (n16 - n) * H; e += NT) {
+            const int col = n + e / H, r2 = (e % H) * 2;
+            *reinterpret_cast<double2*>(Ysm + col * LDT + r2) = make_double2(0.0, 0.0);
+        }
+        cp_async_wait_all();
     } else {
         for (int e = threadIdx.x; e < n16 * TM; e += NT) {
             int col = e / TM, rr = e % TM;
@@ -77,15 +90,29 @@ __device__ __forceinline__ void store_tile(const double* Ysm, double* __restrict
     }
 }
 
+// Copies the 8x8 diagonal blocks of a prepared factor into shared memory: Dsm[J*64 + jj*8 + j] =
+// Rp[8J+j, 8J+jj] (column-major 8x8 per block), so the substitution reads them as broadcast LDS.128.
+template <int NT>
+__device__ __forceinline__ void load_diag_blocks(double* Dsm, const double* __restrict__ Rp, int n16)
+{
+    for (int e = threadIdx.x; e < n16 * 8; e += NT) {
+        const int J = e >> 6, jj = (e >> 3) & 7, j = e & 7;
+        Dsm[e] = __ldg(Rp + (size_t)(8 * J + jj) * n16 + 8 * J + j);
+    }
+}
+
 // In-place Y <- Y * R^-1 on the rows owned by this warp (8*RG rows starting at warp*8*RG).
-// Rp is the prepared factor (see mrcqr_internal.cuh): strict upper = -R, diagonal = 1/R[j,j].
+// Rp is the prepared factor (see mrcqr_internal.cuh): strict upper = -R, diagonal = 1/R[j,j];
+// Dsm its diagonal blocks in shared memory (load_diag_blocks).
 // Left-looking over 8-column blocks J:
-//   T_J = Y_J + sum_{K<J} Y_K * (-R[K,J])       two DMMA.8x8x4 per (K, 8-row group), FP64 tensor pipe
+//   T_J = Y_J + sum_{K<J} Y_K * (-R[K,J])       two DMMA.8x8x4 per (K, 8-row group), FP64 tensor pipe,
+//                                               fragments of step K+1 fetched while step K computes
 //   Y_J = T_J * R[J,J]^-1                       8x8 substitution, one thread per row, registers
 // The k index inside a DMMA is permuted consistently in both operands (lane t takes k = t and
 // k = t + 4), which fixes the summation order once and for all.
 template <int TM, int NW>
-__device__ __forceinline__ void solve_tile(double* Ysm, const double* __restrict__ Rp, int n16)
+__device__ __forceinline__ void solve_tile(double* Ysm, const double* __restrict__ Rp,
+                                           const double* Dsm, int n16)
 {
     constexpr int LDT = TM + 4;
     constexpr int RG = TM / (8 * NW);                 // 8-row groups per warp
@@ -103,20 +130,44 @@ __device__ __forceinline__ void solve_tile(double* Ysm, const double* __restrict
             c[rg][1] = colJ[LDT + 8 * rg];
         }
         const double* rcol = Rp + (size_t)(8 * J + g) * n16 + t;       // B fragment: (k = t, n = g)
-        double b0 = 0.0, b1 = 0.0;
-        if (J > 0) { b0 = __ldg(rcol); b1 = __ldg(rcol + 4); }
-        for (int K = 0; K < J; ++K) {
-            double nb0 = 0.0, nb1 = 0.0;
-            if (K + 1 < J) { nb0 = __ldg(rcol + 8 * (K + 1)); nb1 = __ldg(rcol + 8 * (K + 1) + 4); }
-            const double* ya = Ysm + (8 * K + t) * LDT + rbase + g;    // A fragment: (m = g, k = t)
+        const double* ya = Ysm + t * LDT + rbase + g;                  // A fragment: (m = g, k = t)
+        double b0 = 0.0, b1 = 0.0, a0[RG], a1[RG];
 #pragma unroll
-            for (int rg = 0; rg < RG; ++rg) {
-                double a0 = ya[8 * rg];
-                double a1 = ya[4 * LDT + 8 * rg];
-                dmma884(c[rg], a0, b0);
-                dmma884(c[rg], a1, b1);
+        for (int rg = 0; rg < RG; ++rg) a0[rg] = a1[rg] = 0.0;
+        if (J > 0) {
+            b0 = __ldg(rcol); b1 = __ldg(rcol + 4);
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) { a0[rg] = ya[8 * rg]; a1[rg] = ya[4 * LDT + 8 * rg]; }
+        }
+        for (int K = 0; K < J; ++K) {
+            double nb0 = 0.0, nb1 = 0.0, na0[RG], na1[RG];
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) na0[rg] = na1[rg] = 0.0;
+            if (K + 1 < J) {
+                nb0 = __ldg(rcol + 8 * (K + 1)); nb1 = __ldg(rcol + 8 * (K + 1) + 4);
+                const double* yn = ya + 8 * (K + 1) * LDT;
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) { na0[rg] = yn[8 * rg]; na1[rg] = yn[4 * LDT + 8 * rg]; }
             }
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) dmma884(c[rg], a0[rg], b0);
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) dmma884(c[rg], a1[rg], b1);
             b0 = nb0; b1 = nb1;
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) { a0[rg] = na0[rg]; a1[rg] = na1[rg]; }
+        }
+        // coefficients of the diagonal block (uniform across the warp): d[jj][j], j <= jj
+        double d[8][8];
+        {
+            const double2* dp = reinterpret_cast<const double2*>(Dsm + J * 64);
+#pragma unroll
+            for (int jj = 0; jj < 8; ++jj)
+#pragma unroll
+                for (int h = 0; h <= jj / 2; ++h) {
+                    const double2 v = dp[jj * 4 + h];
+                    d[jj][2 * h] = v.x; d[jj][2 * h + 1] = v.y;
+                }
         }
 #pragma unroll
         for (int rg = 0; rg < RG; ++rg) {
@@ -126,16 +177,14 @@ __device__ __forceinline__ void solve_tile(double* Ysm, const double* __restrict
         __syncwarp();
         if (lane < 8 * RG) {                           // one thread per row: 8x8 substitution
             double* yr = Ysm + (8 * J) * LDT + rbase + lane;
-            const double* d = Rp + (size_t)(8 * J) * n16 + 8 * J;      // diagonal block, col-major
             double y[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) y[j] = yr[j * LDT];
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                y[j] = y[j] * __ldg(d + (size_t)j * n16 + j);          // times 1/R[j,j]
+                y[j] = y[j] * d[j][j];                                 // times 1/R[j,j]
 #pragma unroll
-                for (int jj = j + 1; jj < 8; ++jj)
-                    y[jj] = fma(y[j], __ldg(d + (size_t)jj * n16 + j), y[jj]);   // -R[j,jj]
+                for (int jj = j + 1; jj < 8; ++jj) y[jj] = fma(y[j], d[jj][j], y[jj]);   // -R[j,jj]
             }
 #pragma unroll
             for (int j = 0; j < 8; ++j) yr[j * LDT] = y[j];
