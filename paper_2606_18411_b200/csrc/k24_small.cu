@@ -43,40 +43,85 @@ __global__ void mrcqr_triu_mul(const double* __restrict__ Rc, const double* __re
 }
 
 // ---- K4 ---------------------------------------------------------------------------------------
+// Blocked right-looking Cholesky, 8 columns per outer step (3 barriers per 8 columns instead of 16):
+//   (1) warp 0 factors the 8x8 diagonal block (lane j owns column j in registers, shuffles),
+//   (2) one thread per trailing column solves its 8 rows against the block (the row panel),
+//   (3) rank-8 update of the trailing upper triangle.
 // W: working copy of G (upper triangle used), col-major with leading dimension ldw.
+// Pn: the current row panel, Pn[p * n16 + j] = Rc[k0+p, j].
 __global__ void __launch_bounds__(SMALL_NT)
 mrcqr_k4_cholesky(double* __restrict__ G16, int n, int n16, int use_smem, double* __restrict__ G_out,
                   double* __restrict__ Rc, double* __restrict__ RcPrep, Status* st)
 {
     extern __shared__ __align__(16) double sm[];
-    double* rowk = sm;                       // n16 doubles: scaled row k
-    double* W = use_smem ? sm + n16 : G16;
+    double* Pn = sm;                         // 8 * n16
+    double* W = use_smem ? sm + 8 * n16 : G16;
     const int ldw = use_smem ? n16 + 1 : n16;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, NT = blockDim.x;
 
-    for (int e = tid; e < n * n; e += SMALL_NT) {
+    for (int e = tid; e < n * n; e += NT) {
         const int i = e % n, j = e / n;
         const double v = G16[(size_t)j * n16 + i];
         if (G_out) G_out[e] = v;
         if (use_smem) W[j * ldw + i] = v;
     }
     __syncthreads();
-    for (int k = 0; k < n; ++k) {
-        const double piv = W[k * ldw + k];
-        if (tid == 0 && (!(piv > 0.0) || isinf(piv))) report(st, 3, k);
-        const double d = sqrt(piv);
-        for (int j = k + 1 + tid; j < n; j += SMALL_NT) rowk[j] = W[j * ldw + k] / d;
+    for (int k0 = 0; k0 < n; k0 += 8) {
+        const int kb = min(8, n - k0);
+        if (tid < 32) {                      // (1) diagonal block, lane j < kb owns column k0 + j
+            const int j = tid;
+            double c[8];
+#pragma unroll
+            for (int p = 0; p < 8; ++p) c[p] = (j < kb && p <= j && p < kb) ? W[(k0 + j) * ldw + k0 + p] : 0.0;
+#pragma unroll
+            for (int p = 0; p < 8; ++p) {
+                if (p < kb) {                                        // uniform
+                    const double piv = __shfl_sync(0xffffffffu, c[p], p);
+                    if (j == p && (!(piv > 0.0) || isinf(piv))) report(st, 3, k0 + p);
+                    const double d = sqrt(piv);
+                    const double rp = (j == p) ? d : c[p] / d;       // Rc[k0+p, k0+j] for j >= p
+                    c[p] = rp;
+#pragma unroll
+                    for (int q = p + 1; q < 8; ++q) {                // c[q] -= Rc[p, q] * Rc[p, j]  (q <= j)
+                        const double rq = __shfl_sync(0xffffffffu, rp, q);
+                        if (q <= j) c[q] = fma(-rq, rp, c[q]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int p = 0; p < 8; ++p)
+                if (j < kb && p <= j && p < kb) W[(k0 + j) * ldw + k0 + p] = c[p];
+        }
         __syncthreads();
-        if (tid == 0) W[k * ldw + k] = d;
-        for (int j = k + 1 + tid; j < n; j += SMALL_NT) W[j * ldw + k] = rowk[j];
-        const int L = n - k - 1;
-        for (int e = tid; e < L * L; e += SMALL_NT) {
-            const int i = k + 1 + e % L, j = k + 1 + e / L;
-            if (i <= j) W[j * ldw + i] = fma(-rowk[i], rowk[j], W[j * ldw + i]);
+        for (int j = k0 + kb + tid; j < n; j += NT) {               // (2) row panel: U^T x = w, U the 8x8 block
+            double x[8];
+#pragma unroll
+            for (int p = 0; p < 8; ++p) {
+                if (p < kb) {
+                    double t = W[j * ldw + k0 + p];
+#pragma unroll
+                    for (int q = 0; q < p; ++q) t = fma(-W[(k0 + p) * ldw + k0 + q], x[q], t);
+                    x[p] = t / W[(k0 + p) * ldw + k0 + p];
+                    W[j * ldw + k0 + p] = x[p];
+                    Pn[p * n16 + j] = x[p];
+                } else x[p] = 0.0;
+            }
+        }
+        __syncthreads();
+        const int t0 = k0 + kb, L = n - t0;                          // (3) trailing update
+        for (int e = tid; e < L * L; e += NT) {
+            const int i = t0 + e % L, j = t0 + e / L;
+            if (i <= j) {
+                double acc = W[j * ldw + i];
+#pragma unroll
+                for (int p = 0; p < 8; ++p)
+                    if (p < kb) acc = fma(-Pn[p * n16 + i], Pn[p * n16 + j], acc);
+                W[j * ldw + i] = acc;
+            }
         }
         __syncthreads();
     }
-    for (int e = tid; e < n16 * n16; e += SMALL_NT) {
+    for (int e = tid; e < n16 * n16; e += NT) {
         const int i = e % n16, j = e / n16;
         const bool in = (i < n && j < n);
         const double w = (in && i <= j) ? W[j * ldw + i] : 0.0;
@@ -154,6 +199,99 @@ mrcqr_k2_sketch_qr(double* __restrict__ As, int s, int n, int use_smem, double* 
     }
 }
 
+// ---- K2, register-resident variant (n <= 32*CPW, s <= 32*RPL) -----------------------------------------
+// Column c lives in warp c % 32 (slot c / 32), row i in lane i % 32 (slot i / 32): the whole sketch stays
+// in registers.  Per Householder step: ONE block barrier; the reflector v_j and tau_j travel through a
+// double-buffered shared vector; the warp that owns column j+1 forms v_{j+1} right after updating it.
+template <int CPW, int RPL>
+__global__ void __launch_bounds__(SMALL_NT)
+mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __restrict__ Rs)
+{
+    __shared__ double vbuf[2][RPL * 32];
+    __shared__ double taub[2];
+    __shared__ double betas[32 * CPW];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double a[CPW][RPL];
+#pragma unroll
+    for (int k = 0; k < CPW; ++k)
+#pragma unroll
+        for (int r = 0; r < RPL; ++r) {
+            const int c = warp + 32 * k, i = lane + 32 * r;
+            a[k][r] = (c < n && i < s) ? As[(size_t)c * s + i] : 0.0;
+        }
+    // forms the reflector of column j (held in slot k of this warp) and publishes it in buffer j & 1
+    auto make_v = [&](int k, int j) {
+        double alpha_l = 0.0, sig_l = 0.0;
+#pragma unroll
+        for (int r = 0; r < RPL; ++r) {
+            const int i = lane + 32 * r;
+            if (i == j) alpha_l = a[k][r];
+            if (i > j) sig_l = fma(a[k][r], a[k][r], sig_l);
+        }
+        const double alpha = __shfl_sync(0xffffffffu, alpha_l, j & 31);
+        const double sigma = warp_sum(sig_l);
+        double beta = alpha, tau = 0.0, inv = 0.0;
+        if (sigma != 0.0) {
+            const double nrm = sqrt(fma(alpha, alpha, sigma));
+            beta = (alpha >= 0.0) ? -nrm : nrm;
+            tau = (beta - alpha) / beta;
+            inv = 1.0 / (alpha - beta);
+        }
+#pragma unroll
+        for (int r = 0; r < RPL; ++r) {
+            const int i = lane + 32 * r;
+            const double v = (i > j) ? a[k][r] * inv : (i == j ? 1.0 : 0.0);
+            vbuf[j & 1][i] = v;
+            if (i == j) a[k][r] = beta;                      // R[j,j]
+            if (i > j) a[k][r] = 0.0;
+        }
+        if (lane == 0) { taub[j & 1] = tau; betas[j] = beta; }
+    };
+    if (warp == 0) make_v(0, 0);
+    for (int j = 0; j < n; ++j) {
+        __syncthreads();
+        double v[RPL];
+#pragma unroll
+        for (int r = 0; r < RPL; ++r) v[r] = vbuf[j & 1][lane + 32 * r];
+        const double tau = taub[j & 1];
+        double w[CPW];
+#pragma unroll
+        for (int k = 0; k < CPW; ++k) {
+            w[k] = 0.0;
+#pragma unroll
+            for (int r = 0; r < RPL; ++r) w[k] = fma(v[r], a[k][r], w[k]);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+            for (int k = 0; k < CPW; ++k) w[k] += __shfl_xor_sync(0xffffffffu, w[k], o);
+#pragma unroll
+        for (int k = 0; k < CPW; ++k) {
+            const int c = warp + 32 * k;
+            if (c > j && c < n) {
+                const double wt = w[k] * tau;
+#pragma unroll
+                for (int r = 0; r < RPL; ++r) a[k][r] = fma(-wt, v[r], a[k][r]);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < CPW; ++k)
+            if (warp + 32 * k == j + 1 && j + 1 < n) make_v(k, j + 1);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < CPW; ++k)
+#pragma unroll
+        for (int r = 0; r < RPL; ++r) {
+            const int c = warp + 32 * k, i = lane + 32 * r;
+            if (c < n && i < n) {
+                double val = (i <= c) ? a[k][r] : 0.0;
+                if (i <= c && betas[i] < 0.0) val = -val;    // sign-normalise row i: diag(Rs) > 0
+                Rs[(size_t)c * n + i] = val;
+            }
+        }
+}
+
 // ---- launchers --------------------------------------------------------------------------------
 int launch_prep_R(const double* R, int n, double* Rprep, int n16, Status* st, int err_code, cudaStream_t s)
 {
@@ -170,17 +308,23 @@ int launch_triu_mul(const double* Rc, const double* Rs, int n, double* R, cudaSt
 int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double* Rc, double* RcPrep,
                        Status* st, cudaStream_t s)
 {
-    size_t need = ((size_t)n16 + (size_t)n16 * (n16 + 1)) * sizeof(double);
+    size_t need = ((size_t)8 * n16 + (size_t)n16 * (n16 + 1)) * sizeof(double);
     const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
-    const size_t smem = use_smem ? need : (size_t)n16 * sizeof(double);
+    const size_t smem = use_smem ? need : (size_t)8 * n16 * sizeof(double);
+    const int threads = n16 <= 64 ? 256 : (n16 <= 128 ? 512 : SMALL_NT);
     cudaFuncSetAttribute(mrcqr_k4_cholesky, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mrcqr_k4_cholesky<<<1, SMALL_NT, smem, s>>>(const_cast<double*>(G16), n, n16, use_smem, G_out, Rc, RcPrep, st);
+    mrcqr_k4_cholesky<<<1, threads, smem, s>>>(const_cast<double*>(G16), n, n16, use_smem, G_out, Rc, RcPrep, st);
     return 1;
 }
 
 int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* work, double* Rs, Status* st, cudaStream_t s)
 {
     (void)work; (void)st;
+    if (n <= 64 && s_rows <= 256) {
+        if (n <= 32 && s_rows <= 128) mrcqr_k2_sketch_qr_reg<1, 4><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs);
+        else mrcqr_k2_sketch_qr_reg<2, 8><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs);
+        return 1;
+    }
     size_t need = ((size_t)n + 2 + (size_t)s_rows * n) * sizeof(double);
     const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
     const size_t smem = use_smem ? need : ((size_t)n + 2) * sizeof(double);
