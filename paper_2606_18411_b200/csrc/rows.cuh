@@ -101,15 +101,49 @@ __device__ __forceinline__ void load_diag_blocks(double* Dsm, const double* __re
     }
 }
 
+// 8x8 substitution of block J for the rows of this warp, one thread per row:
+//   y_j = t_j / R[j,j],  t_jj -= y_j R[j,jj]  (jj > j), coefficients from the shared diagonal blocks.
+template <int TM, int RG>
+__device__ __forceinline__ void diag_block(double* Ysm, const double* Dsm, int J, int rbase, int lane)
+{
+    constexpr int LDT = TM + 4;
+    double d[8][8];
+    const double2* dp = reinterpret_cast<const double2*>(Dsm + J * 64);
+#pragma unroll
+    for (int jj = 0; jj < 8; ++jj)
+#pragma unroll
+        for (int h = 0; h <= jj / 2; ++h) {
+            const double2 v = dp[jj * 4 + h];
+            d[jj][2 * h] = v.x; d[jj][2 * h + 1] = v.y;
+        }
+    if (lane < 8 * RG) {
+        double* yr = Ysm + (8 * J) * LDT + rbase + lane;
+        double y[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) y[j] = yr[j * LDT];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            y[j] = y[j] * d[j][j];                                     // times 1/R[j,j]
+#pragma unroll
+            for (int jj = j + 1; jj < 8; ++jj) y[jj] = fma(y[j], d[jj][j], y[jj]);   // -R[j,jj]
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) yr[j * LDT] = y[j];
+    }
+}
+
 // In-place Y <- Y * R^-1 on the rows owned by this warp (8*RG rows starting at warp*8*RG).
 // Rp is the prepared factor (see mrcqr_internal.cuh): strict upper = -R, diagonal = 1/R[j,j];
 // Dsm its diagonal blocks in shared memory (load_diag_blocks).
-// Left-looking over 8-column blocks J:
-//   T_J = Y_J + sum_{K<J} Y_K * (-R[K,J])       two DMMA.8x8x4 per (K, 8-row group), FP64 tensor pipe,
-//                                               fragments of step K+1 fetched while step K computes
-//   Y_J = T_J * R[J,J]^-1                       8x8 substitution, one thread per row, registers
-// The k index inside a DMMA is permuted consistently in both operands (lane t takes k = t and
-// k = t + 4), which fixes the summation order once and for all.
+// Left-looking over PAIRS of 8-column blocks (J0, J1 = J0 + 1), so every A fragment read from shared
+// memory feeds two DMMAs (shared-memory bandwidth, not the FP64 pipe, was the first limit):
+//   T_J0, T_J1 += Y_K * (-R[K,J0]), Y_K * (-R[K,J1])   K < J0      DMMA.8x8x4, fragments prefetched
+//   Y_J0 = T_J0 * R[J0,J0]^-1                                      8x8 substitution, thread per row
+//   T_J1 += Y_J0 * (-R[J0,J1]);  Y_J1 = T_J1 * R[J1,J1]^-1
+// Fragment conventions (fixed, so the summation order is fixed): in a DMMA lane (g, t) supplies
+// k = t and k = t + 4; accumulator column 2t+e of the hardware layout carries matrix column t + 4e
+// of the block (B fragment lane g loads column (g>>1) + 4(g&1)), which makes the accumulator's
+// shared-memory loads and stores bank-conflict free with LDT = 4 mod 16.
 template <int TM, int NW>
 __device__ __forceinline__ void solve_tile(double* Ysm, const double* __restrict__ Rp,
                                            const double* Dsm, int n16)
@@ -120,75 +154,69 @@ __device__ __forceinline__ void solve_tile(double* Ysm, const double* __restrict
     const int g = lane >> 2, t = lane & 3;
     const int rbase = warp * (8 * RG);
     const int nB = n16 >> 3;
+    const int csel = (g >> 1) + 4 * (g & 1);           // matrix column carried by hardware column g
+    const double* ya = Ysm + t * LDT + rbase + g;      // A fragment base: (m = g, k = t)
 
-    for (int J = 0; J < nB; ++J) {
-        double c[RG][2];
-        double* colJ = Ysm + (8 * J + 2 * t) * LDT + rbase + g;
+    for (int J0 = 0; J0 < nB; J0 += 2) {
+        const int J1 = J0 + 1;
+        double cA[RG][2], cB[RG][2];
+        double* colA = Ysm + (8 * J0 + t) * LDT + rbase + g;           // accumulator element e: + 4e*LDT
+        double* colB = colA + 8 * LDT;
 #pragma unroll
         for (int rg = 0; rg < RG; ++rg) {
-            c[rg][0] = colJ[8 * rg];
-            c[rg][1] = colJ[LDT + 8 * rg];
+            cA[rg][0] = colA[8 * rg]; cA[rg][1] = colA[4 * LDT + 8 * rg];
+            cB[rg][0] = colB[8 * rg]; cB[rg][1] = colB[4 * LDT + 8 * rg];
         }
-        const double* rcol = Rp + (size_t)(8 * J + g) * n16 + t;       // B fragment: (k = t, n = g)
-        const double* ya = Ysm + t * LDT + rbase + g;                  // A fragment: (m = g, k = t)
-        double b0 = 0.0, b1 = 0.0, a0[RG], a1[RG];
-#pragma unroll
-        for (int rg = 0; rg < RG; ++rg) a0[rg] = a1[rg] = 0.0;
-        if (J > 0) {
-            b0 = __ldg(rcol); b1 = __ldg(rcol + 4);
+        const double* rA = Rp + (size_t)(8 * J0 + csel) * n16 + t;     // B fragments: (k = t, n = g)
+        const double* rB = rA + (size_t)8 * n16;
+        if (J0 > 0) {
+            double a0[RG], a1[RG];
+            double bA0 = __ldg(rA), bA1 = __ldg(rA + 4), bB0 = __ldg(rB), bB1 = __ldg(rB + 4);
 #pragma unroll
             for (int rg = 0; rg < RG; ++rg) { a0[rg] = ya[8 * rg]; a1[rg] = ya[4 * LDT + 8 * rg]; }
-        }
-        for (int K = 0; K < J; ++K) {
-            double nb0 = 0.0, nb1 = 0.0, na0[RG], na1[RG];
+            for (int K = 0; K < J0; ++K) {
+                const int Kn = (K + 1 < J0) ? K + 1 : K;               // prefetch (re-reads the last one)
+                const double nA0 = __ldg(rA + 8 * Kn), nA1 = __ldg(rA + 8 * Kn + 4);
+                const double nB0 = __ldg(rB + 8 * Kn), nB1 = __ldg(rB + 8 * Kn + 4);
+                const double* yn = ya + 8 * Kn * LDT;
+                double n0[RG], n1[RG];
 #pragma unroll
-            for (int rg = 0; rg < RG; ++rg) na0[rg] = na1[rg] = 0.0;
-            if (K + 1 < J) {
-                nb0 = __ldg(rcol + 8 * (K + 1)); nb1 = __ldg(rcol + 8 * (K + 1) + 4);
-                const double* yn = ya + 8 * (K + 1) * LDT;
+                for (int rg = 0; rg < RG; ++rg) { n0[rg] = yn[8 * rg]; n1[rg] = yn[4 * LDT + 8 * rg]; }
 #pragma unroll
-                for (int rg = 0; rg < RG; ++rg) { na0[rg] = yn[8 * rg]; na1[rg] = yn[4 * LDT + 8 * rg]; }
+                for (int rg = 0; rg < RG; ++rg) dmma884(cA[rg], a0[rg], bA0);
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) dmma884(cB[rg], a0[rg], bB0);
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) dmma884(cA[rg], a1[rg], bA1);
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) dmma884(cB[rg], a1[rg], bB1);
+                bA0 = nA0; bA1 = nA1; bB0 = nB0; bB1 = nB1;
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) { a0[rg] = n0[rg]; a1[rg] = n1[rg]; }
             }
-#pragma unroll
-            for (int rg = 0; rg < RG; ++rg) dmma884(c[rg], a0[rg], b0);
-#pragma unroll
-            for (int rg = 0; rg < RG; ++rg) dmma884(c[rg], a1[rg], b1);
-            b0 = nb0; b1 = nb1;
-#pragma unroll
-            for (int rg = 0; rg < RG; ++rg) { a0[rg] = na0[rg]; a1[rg] = na1[rg]; }
         }
-        // coefficients of the diagonal block (uniform across the warp): d[jj][j], j <= jj
-        double d[8][8];
-        {
-            const double2* dp = reinterpret_cast<const double2*>(Dsm + J * 64);
+        // ---- block J0
+        const double xB0 = __ldg(rB + 8 * J0), xB1 = __ldg(rB + 8 * J0 + 4);    // -R[J0, J1] fragments
 #pragma unroll
-            for (int jj = 0; jj < 8; ++jj)
-#pragma unroll
-                for (int h = 0; h <= jj / 2; ++h) {
-                    const double2 v = dp[jj * 4 + h];
-                    d[jj][2 * h] = v.x; d[jj][2 * h + 1] = v.y;
-                }
-        }
-#pragma unroll
-        for (int rg = 0; rg < RG; ++rg) {
-            colJ[8 * rg] = c[rg][0];
-            colJ[LDT + 8 * rg] = c[rg][1];
-        }
+        for (int rg = 0; rg < RG; ++rg) { colA[8 * rg] = cA[rg][0]; colA[4 * LDT + 8 * rg] = cA[rg][1]; }
         __syncwarp();
-        if (lane < 8 * RG) {                           // one thread per row: 8x8 substitution
-            double* yr = Ysm + (8 * J) * LDT + rbase + lane;
-            double y[8];
+        diag_block<TM, RG>(Ysm, Dsm, J0, rbase, lane);
+        __syncwarp();
+        // ---- cross term and block J1
+        {
+            const double* yj = ya + 8 * J0 * LDT;
+            double a0[RG], a1[RG];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) y[j] = yr[j * LDT];
+            for (int rg = 0; rg < RG; ++rg) { a0[rg] = yj[8 * rg]; a1[rg] = yj[4 * LDT + 8 * rg]; }
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                y[j] = y[j] * d[j][j];                                 // times 1/R[j,j]
+            for (int rg = 0; rg < RG; ++rg) dmma884(cB[rg], a0[rg], xB0);
 #pragma unroll
-                for (int jj = j + 1; jj < 8; ++jj) y[jj] = fma(y[j], d[jj][j], y[jj]);   // -R[j,jj]
-            }
-#pragma unroll
-            for (int j = 0; j < 8; ++j) yr[j * LDT] = y[j];
+            for (int rg = 0; rg < RG; ++rg) dmma884(cB[rg], a1[rg], xB1);
         }
+#pragma unroll
+        for (int rg = 0; rg < RG; ++rg) { colB[8 * rg] = cB[rg][0]; colB[4 * LDT + 8 * rg] = cB[rg][1]; }
+        __syncwarp();
+        diag_block<TM, RG>(Ysm, Dsm, J1, rbase, lane);
         __syncwarp();
     }
 }
