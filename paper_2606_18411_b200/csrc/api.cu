@@ -104,7 +104,6 @@ static bool ensure_hidx(size_t count)
 {
     if (count <= g.h_idx_cap) return true;
     if (g.h_idx) cudaFreeHost(g.h_idx);
-    if (g.ev_ok) for (int i = 0; i < 8; ++i) cudaEventDestroy(g.ev[i]);
     g.h_idx_cap = 0;
     if (cudaMallocHost(&g.h_idx, count * sizeof(int64_t)) != cudaSuccess) { g.h_idx = nullptr; return false; }
     g.h_idx_cap = count;
@@ -149,9 +148,11 @@ static int enqueue_gram(const Layout& L, int64_t m, int n, int64_t lda, const do
     double* part = reinterpret_cast<double*>(g.ws + L.k3);
     int np = 0;
     int k = launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st);
+    k += upload_diag(RsPrep, n16, 0, st);
     k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, Ydump, st);
     k += launch_reduce_partials(part, np, n, n16, G16, st);
     k += launch_k4_cholesky(G16, n, n16, G_out, Rc, RcPrep, stat, st);
+    k += upload_diag(RcPrep, n16, 1, st);
     return k;
 }
 
@@ -164,8 +165,8 @@ static int enqueue_formq(const Layout& L, int64_t m, int n, int64_t lda, const d
     double* RsPrep = reinterpret_cast<double*>(g.ws + L.RsPrep);
     double* RcPrep = reinterpret_cast<double*>(g.ws + L.RcPrep);
     int k = 0;
-    if (prep_rs) k += launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st);
-    if (prep_rc) k += launch_prep_R(Rc, n, RcPrep, n16, stat, MRCQR_ERR_BREAKDOWN, st);
+    if (prep_rs) { k += launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st); k += upload_diag(RsPrep, n16, 0, st); }
+    if (prep_rc) { k += launch_prep_R(Rc, n, RcPrep, n16, stat, MRCQR_ERR_BREAKDOWN, st); k += upload_diag(RcPrep, n16, 1, st); }
     k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, Ydump, st);
     if (R) k += launch_triu_mul(Rc, Rs, n, R, st);
     return k;
@@ -351,11 +352,13 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
         double* part = reinterpret_cast<double*>(g.ws + L.k3);
         int np = 0;
         k += launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st);
+        k += upload_diag(RsPrep, n16, 0, st);
         if (tm) cudaEventRecord(g.ev[3], st);
         k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, st);
         if (tm) cudaEventRecord(g.ev[4], st);
         k += launch_reduce_partials(part, np, n, n16, G16, st);
         k += launch_k4_cholesky(G16, n, n16, nullptr, Rc, RcPrep, stat, st);
+        k += upload_diag(RcPrep, n16, 1, st);
         if (tm) cudaEventRecord(g.ev[5], st);
         k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, st);           // Alg.1 step 3
         if (tm) cudaEventRecord(g.ev[6], st);

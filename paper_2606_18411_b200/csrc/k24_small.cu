@@ -16,18 +16,13 @@ constexpr int SMALL_SMEM_MAX = 220 * 1024;
 __global__ void mrcqr_prep_R(const double* __restrict__ R, int n, double* __restrict__ Rp, int n16,
                              Status* st, int err_code)
 {
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n16 * n16) return;
-    const int i = e % n16, j = e / n16;
-    double v = 0.0;
-    if (i == j) {
-        if (i < n) {
-            const double d = R[(size_t)j * n + j];
-            if (!(fabs(d) > 0.0) || isinf(d)) report(st, err_code, j);
-            v = 1.0 / d;
-        } else v = 1.0;
-    } else if (i < j && j < n) v = -R[(size_t)j * n + i];
-    Rp[e] = v;
+    const int nB = n16 >> 3;
+    const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
+    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= total) return;
+    int bad = -1;
+    Rp[o] = prep_value(R, n, n, nB, o, &bad);
+    if (bad >= 0) report(st, err_code, bad);
 }
 
 __global__ void mrcqr_triu_mul(const double* __restrict__ Rc, const double* __restrict__ Rs, int n,
@@ -121,15 +116,17 @@ mrcqr_k4_cholesky(double* __restrict__ G16, int n, int n16, int use_smem, double
         }
         __syncthreads();
     }
-    for (int e = tid; e < n16 * n16; e += NT) {
-        const int i = e % n16, j = e / n16;
-        const bool in = (i < n && j < n);
-        const double w = (in && i <= j) ? W[j * ldw + i] : 0.0;
-        double p = 0.0;
-        if (i == j) p = in ? 1.0 / w : 1.0;
-        else if (in && i < j) p = -w;
-        if (in) Rc[(size_t)j * n + i] = w;
-        RcPrep[e] = p;      // note: RcPrep must not alias G16 when W == G16
+    for (int e = tid; e < n * n; e += NT) {
+        const int i = e % n, j = e / n;
+        const double w = (i <= j) ? W[j * ldw + i] : 0.0;
+        Rc[e] = w;
+    }
+    __syncthreads();
+    {                                        // prepared R_c (fragment order + diagonal blocks), from W
+        const int nB = n16 >> 3;
+        const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
+        int bad = -1;
+        for (size_t o = tid; o < total; o += NT) RcPrep[o] = prep_value(W, ldw, n, nB, o, &bad);
     }
 }
 
@@ -295,7 +292,9 @@ mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __re
 // ---- launchers --------------------------------------------------------------------------------
 int launch_prep_R(const double* R, int n, double* Rprep, int n16, Status* st, int err_code, cudaStream_t s)
 {
-    mrcqr_prep_R<<<(n16 * n16 + 255) / 256, 256, 0, s>>>(R, n, Rprep, n16, st, err_code);
+    const int nB = n16 >> 3;
+    const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
+    mrcqr_prep_R<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(R, n, Rprep, n16, st, err_code);
     return 1;
 }
 

@@ -1,30 +1,145 @@
 // k35_rows.cu -- the two passes over A that dominate MRCQR ("TRSM x2" is 56-74 %
 // of the paper's runtime):
 //   K3  mrcqr_k3_gram   Algorithm 2 step 7 fused with Algorithm 1 step 1:
-//                       per row y = a Rs^-1 (solve_tile), G += y^T y on DMMA; Y never leaves the SM.
+//                       per row y = a Rs^-1 (solve_slab), G += y^T y on DMMA; Y never leaves the SM.
 //   K5  mrcqr_k5_formq  Algorithm 1 step 3: y recomputed bit-identically,
-//                       q = y Rc^-1, Q streamed out.
-// Persistent CTAs, static tile -> CTA map (tile i belongs to CTA i mod grid, visited in ascending
-// order), so every sum has a fixed order: results are deterministic run to run.
+//                       q = y Rc^-1, Q streamed out.  Warps are fully independent (no CTA barrier).
+// Persistent CTAs, static slab -> warp map, so every sum has a fixed order: results are
+// deterministic run to run.
 #include "rows.cuh"
+#include <type_traits>
 
 namespace mrcqr {
 
 constexpr int GRAM_MAXS = 6;          // 16x16 super-blocks of G a warp accumulates per sweep (48 doubles)
 constexpr int GRAM_CHAIN = 256;       // max DMMA k-steps chained into one accumulator before a flush
+constexpr int SMEM_CAP = 227 * 1024;
 
 RowCfg row_config(int n)
 {
     RowCfg c;
     c.n16 = round_up(n, 16);
-    if (c.n16 <= 64)       { c.TM = 128; c.NW = 4; }
-    else if (c.n16 <= 128) { c.TM = 128; c.NW = 8; }
-    else if (c.n16 <= 256) { c.TM = 64;  c.NW = 8; }
-    else                   { c.TM = 32;  c.NW = 4; }
-    c.smem_bytes = c.n16 * (c.TM + 4) * 8 + 2 * c.n16 * 64;   // tile + diagonal blocks of Rs and Rc
-    c.ctas_per_sm = 0;
+    if (c.n16 <= 64)       { c.RG = 4; c.NW = 4; }
+    else if (c.n16 <= 128) { c.RG = 2; c.NW = 8; }
+    else if (c.n16 <= 256) { c.RG = 1; c.NW = 8; }
+    else                   { c.RG = 1; c.NW = 4; }
+    c.smem_bytes = c.NW * c.n16 * (8 * c.RG + 4) * 8;
     return c;
 }
+
+// ---- Gram accumulation with compile-time block ownership (n16 <= 128) --------------------------------
+// The upper triangle of G in 8x8 blocks (I <= J) is split over the NWG warps of a CTA so that a warp's
+// blocks form rectangles / triangles: a warp that owns a set of blocks loads one fragment per distinct
+// block row / column it touches and reuses it across its blocks (2-D register blocking; shared-memory
+// traffic, not the FP64 pipe, was the limit of a row-wise split).
+template <int NB, int NWG>
+__host__ __device__ constexpr int gram_owner(int I, int J)
+{
+    if (NB == 8 && NWG == 4) {                       // 9 blocks per warp
+        if (J < 4) return (I == 0 && J == 3) ? 2 : 0;
+        if (I >= 4) return (I == 4 && J == 7) ? 3 : 1;
+        return I < 2 ? 2 : 3;
+    }
+    if (NB == 16 && NWG == 8) {                      // 18,18,18,18,16,16,16,16 blocks
+        const int a = I >> 2, b = J >> 2;
+        if (a == b) return a;
+        if (a == 0 && b == 1) return (I & 3) < 2 ? 0 : 1;
+        if (a == 2 && b == 3) return (I & 3) < 2 ? 2 : 3;
+        if (a == 0 && b == 2) return 4;
+        if (a == 0 && b == 3) return 5;
+        if (a == 1 && b == 2) return 6;
+        return 7;
+    }
+    return (I < NB - 1 - I ? I : NB - 1 - I) % NWG;  // block rows r and NB-1-r: NB+1 blocks per warp
+}
+template <int NB, int NWG>
+__host__ __device__ constexpr int gram_slot(int role, int I, int J)   // index of (I,J) among role's blocks
+{
+    int cnt = 0;
+    for (int i = 0; i < NB; ++i)
+        for (int j = i; j < NB; ++j) {
+            if (i == I && j == J) return cnt;
+            if (gram_owner<NB, NWG>(i, j) == role) ++cnt;
+        }
+    return cnt;
+}
+template <int NB, int NWG>
+__host__ __device__ constexpr bool gram_needs(int role, int c)
+{
+    for (int i = 0; i < NB; ++i)
+        for (int j = i; j < NB; ++j)
+            if (gram_owner<NB, NWG>(i, j) == role && (i == c || j == c)) return true;
+    return false;
+}
+template <int NB, int NWG>
+__host__ __device__ constexpr int gram_maxown()
+{
+    int mx = 0;
+    for (int r = 0; r < NWG; ++r) { const int c = gram_slot<NB, NWG>(r, NB, NB); if (c > mx) mx = c; }
+    return mx;
+}
+
+// compile-time loop: f(std::integral_constant<int, B>) ... f(std::integral_constant<int, E-1>)
+template <int B, int E, typename F>
+__device__ __forceinline__ void static_for(F&& f)
+{
+    if constexpr (B < E) { f(std::integral_constant<int, B>{}); static_for<B + 1, E>(f); }
+}
+
+template <int NB, int NWG, int ROLE, int SR, int NSLAB, int MAXOWN>
+__device__ __forceinline__ void gram_accumulate(double (&acc)[MAXOWN][2], const double* tile, int slab_stride, int lane)
+{
+    constexpr int LDS_ = SR + 4;
+    const int g = lane >> 2, t = lane & 3;
+    for (int w = 0; w < NSLAB; ++w) {
+        const double* y0 = tile + (size_t)w * slab_stride + g * LDS_ + t;
+#pragma unroll 2
+        for (int ks = 0; ks < SR / 4; ++ks) {
+            const double* yk = y0 + 4 * ks;
+            double f[NB];
+            static_for<0, NB>([&](auto Cc) {
+                constexpr int c = decltype(Cc)::value;
+                if constexpr (gram_needs<NB, NWG>(ROLE, c)) f[c] = yk[(8 * c) * LDS_];
+            });
+            static_for<0, NB>([&](auto Ic) {
+                constexpr int I = decltype(Ic)::value;
+                static_for<I, NB>([&](auto Jc) {
+                    constexpr int J = decltype(Jc)::value;
+                    if constexpr (gram_owner<NB, NWG>(I, J) == ROLE) {
+                        constexpr int slot = gram_slot<NB, NWG>(ROLE, I, J);
+                        dmma884(acc[slot], f[I], f[J]);
+                    }
+                });
+            });
+        }
+    }
+}
+
+template <int NB, int NWG, int ROLE, int MAXOWN>
+__device__ __forceinline__ void gram_flush(double (&acc)[MAXOWN][2], double* part, int n16, bool first, int lane)
+{
+    const int g = lane >> 2, t = lane & 3;
+    static_for<0, NB>([&](auto Ic) {
+        constexpr int I = decltype(Ic)::value;
+        static_for<I, NB>([&](auto Jc) {
+            constexpr int J = decltype(Jc)::value;
+            if constexpr (gram_owner<NB, NWG>(I, J) == ROLE) {
+                constexpr int slot = gram_slot<NB, NWG>(ROLE, I, J);
+                double* dst = part + (size_t)(8 * J + 2 * t) * n16 + 8 * I + g;
+                if (first) { dst[0] = acc[slot][0]; dst[n16] = acc[slot][1]; }
+                else { dst[0] += acc[slot][0]; dst[n16] += acc[slot][1]; }
+                acc[slot][0] = acc[slot][1] = 0.0;
+            }
+        });
+    });
+}
+
+#define MRCQR_ROLE_SWITCH(CALL)                                                                  \
+    switch (warp) {                                                                              \
+        case 0: CALL(0) break; case 1: CALL(1) break; case 2: CALL(2) break; case 3: CALL(3) break; \
+        case 4: if (NW > 4) { CALL(4) } break; case 5: if (NW > 4) { CALL(5) } break;            \
+        case 6: if (NW > 4) { CALL(6) } break; default: if (NW > 4) { CALL(7) } break;           \
+    }
 
 __device__ __forceinline__ void sb_to_pq(int sb, int& p, int& q)
 {
@@ -33,129 +148,70 @@ __device__ __forceinline__ void sb_to_pq(int sb, int& p, int& q)
     q = qq; p = sb - qq * (qq + 1) / 2;
 }
 
-// ---- Gram accumulation, "row pair" scheme (n16 <= 16 * NW) -----------------------------------------
-// Warp w owns the 8x8 blocks (r, r..nB-1) and (r2, r2..nB-1) of the upper triangle, r = w,
-// r2 = nB-1-w: nB+1 blocks for every warp (perfect balance), accumulators stay in registers for the
-// CTA's whole life, one fragment load per block column serves both rows.
-template <int TM, int NBMAX>
-struct GramPair {
-    static constexpr int NH = NBMAX / 2;
-    double acc1[NBMAX][2];      // block (r,  r + cc),      cc = 0 .. nB-1-r
-    double acc2[NH][2];         // block (r2, nB-1 - e),    e  = 0 .. nB-1-r2 (= r)   -- indexed from the end
-    __device__ __forceinline__ void zero()
-    {
-#pragma unroll
-        for (int b = 0; b < NBMAX; ++b) acc1[b][0] = acc1[b][1] = 0.0;
-#pragma unroll
-        for (int b = 0; b < NH; ++b) acc2[b][0] = acc2[b][1] = 0.0;
-    }
-    // r < r2, or r == r2 (odd nB, middle row: acc2 unused); warps with r > r2 own nothing.
-    // Every register array is indexed by unrolled loop counters only (no local memory).
-    __device__ __forceinline__ void accumulate(const double* Ysm, int nB, int r, int r2)
-    {
-        constexpr int LDT = TM + 4;
-        const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-        if (r > r2) return;
-        const int ne = (r2 != r) ? (nB - r2) : 0;
-        const double* y0 = Ysm + g * LDT + t;
-#pragma unroll 2
-        for (int ks = 0; ks < TM / 4; ++ks) {
-            const double* yk = y0 + 4 * ks;
-            double f[NBMAX], fe[NH];
-#pragma unroll
-            for (int cc = 0; cc < NBMAX; ++cc) f[cc] = (r + cc < nB) ? yk[(8 * (r + cc)) * LDT] : 0.0;
-#pragma unroll
-            for (int e = 0; e < NH; ++e) fe[e] = (e < ne) ? yk[(8 * (nB - 1 - e)) * LDT] : 0.0;
-            const double fr2 = yk[(8 * r2) * LDT];
-#pragma unroll
-            for (int cc = 0; cc < NBMAX; ++cc)
-                if (r + cc < nB) dmma884(acc1[cc], f[0], f[cc]);
-#pragma unroll
-            for (int e = 0; e < NH; ++e)
-                if (e < ne) dmma884(acc2[e], fr2, fe[e]);
-        }
-    }
-    __device__ __forceinline__ void flush(double* part, int n16, int nB, int r, int r2, bool first)
-    {
-        const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-        if (r > r2) return;
-        const int ne = (r2 != r) ? (nB - r2) : 0;
-#pragma unroll
-        for (int cc = 0; cc < NBMAX; ++cc) {
-            if (r + cc < nB) {
-                double* dst = part + (size_t)(8 * (r + cc) + 2 * t) * n16 + 8 * r + g;
-                if (first) { dst[0] = acc1[cc][0]; dst[n16] = acc1[cc][1]; }
-                else { dst[0] += acc1[cc][0]; dst[n16] += acc1[cc][1]; }
-                acc1[cc][0] = acc1[cc][1] = 0.0;
-            }
-        }
-#pragma unroll
-        for (int e = 0; e < NH; ++e) {
-            if (e < ne) {
-                double* dst = part + (size_t)(8 * (nB - 1 - e) + 2 * t) * n16 + 8 * r2 + g;
-                if (first) { dst[0] = acc2[e][0]; dst[n16] = acc2[e][1]; }
-                else { dst[0] += acc2[e][0]; dst[n16] += acc2[e][1]; }
-                acc2[e][0] = acc2[e][1] = 0.0;
-            }
-        }
-    }
-};
-
 // G partial of this CTA: n16 x n16 col-major, blocks (I <= J) of the upper triangle only.
-template <int TM, int NW, bool VEC>
-__global__ void __launch_bounds__(NW * 32, (TM == 128 && NW == 4) ? 3 : 1)
+// NB > 0: n16 = 8*NB <= 128, compile-time Gram ownership, accumulators live in registers across tiles.
+// NB = 0: n16 > 128, 16x16 super-blocks in sweeps, flushed to the L2-resident partial every tile.
+template <int RG, int NW, int NB, bool VEC>
+__global__ void __launch_bounds__(NW * 32, (RG == 4 && NW == 4) ? 3 : 1)
 mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__ A,
-              const double* __restrict__ RsPrep, double* __restrict__ partials,
+              const double2* __restrict__ fragS, double* __restrict__ partials,
               int64_t ntiles, double* __restrict__ Ydump)
 {
     extern __shared__ __align__(16) double Ysm[];
-    constexpr int LDT = TM + 4, NT = NW * 32;
-    constexpr bool PAIR = (TM == 128);                         // n16 <= 16 * NW for both TM = 128 shapes
-    double* Dsm = Ysm + (size_t)n16 * LDT;
+    constexpr int SR = 8 * RG, LDS_ = SR + 4, TM = SR * NW;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane >> 2, t = lane & 3;
     const int nB = n16 >> 3;
+    const int slab_stride = n16 * LDS_;
+    double* slab = Ysm + (size_t)warp * slab_stride;
     double* part = partials + (size_t)blockIdx.x * n16 * n16;
-    constexpr int FLUSH_TILES = GRAM_CHAIN * 4 / TM;
-    load_diag_blocks<NT>(Dsm, RsPrep, n16);
+    zero_pad_columns<SR>(slab, n, n16, lane);
 
-    if (PAIR) {
-        GramPair<TM, 2 * NW> gp;
-        gp.zero();
-        const int r = warp, r2 = nB - 1 - warp;
+    if (NB > 0) {
+        constexpr int NBc = NB > 0 ? NB : 2;
+        constexpr int MAXOWN = gram_maxown<NBc, NW>();
+        constexpr int FLUSH_TILES = GRAM_CHAIN * 4 / TM;
+        double acc[MAXOWN][2];
+#pragma unroll
+        for (int b = 0; b < MAXOWN; ++b) acc[b][0] = acc[b][1] = 0.0;
         bool first = true;
         int since = 0;
         for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            const int64_t row0 = tile * TM;
+            const int64_t row0 = tile * TM + warp * SR;
+            load_slab<SR, VEC>(slab, A, lda, m, n, row0, lane);
+            if (VEC) cp_async_wait_all();
+            __syncwarp();
+            solve_slab<RG, 0, NBc>(slab, fragS, nB, lane);
+            if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); }
             __syncthreads();
-            load_tile<TM, NT, VEC>(Ysm, A, lda, m, n, n16, row0);
-            __syncthreads();
-            solve_tile<TM, NW>(Ysm, RsPrep, Dsm, n16);
-            __syncthreads();
-            if (Ydump) store_tile<TM, NT, false>(Ysm, Ydump, m, m, n, row0);
-            gp.accumulate(Ysm, nB, r, r2);
+#define GRAM_ACC(R_) gram_accumulate<NBc, NW, R_, SR, NW, MAXOWN>(acc, Ysm, slab_stride, lane);
+            MRCQR_ROLE_SWITCH(GRAM_ACC)
+#undef GRAM_ACC
             ++since;
             if (since >= FLUSH_TILES || tile + gridDim.x >= ntiles) {
-                gp.flush(part, n16, nB, r, r2, first);
+#define GRAM_FLUSH(R_) gram_flush<NBc, NW, R_, MAXOWN>(acc, part, n16, first, lane);
+                MRCQR_ROLE_SWITCH(GRAM_FLUSH)
+#undef GRAM_FLUSH
                 first = false; since = 0;
             }
+            __syncthreads();
         }
         return;
     }
 
-    // ---- super-block sweeps (n16 > 128): 16x16 super-blocks, flushed to the L2-resident partial every tile
+    // ---- super-block sweeps (n16 > 128)
     const int P = n16 >> 4, NS = P * (P + 1) / 2;
     const int per_warp = (NS - warp + NW - 1) / NW;
     const int sweeps = (per_warp + GRAM_MAXS - 1) / GRAM_MAXS;
     bool first_tile = true;
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int64_t row0 = tile * TM;
+        const int64_t row0 = tile * TM + warp * SR;
+        load_slab<SR, VEC>(slab, A, lda, m, n, row0, lane);
+        if (VEC) cp_async_wait_all();
+        __syncwarp();
+        solve_slab<RG, 0>(slab, fragS, nB, lane);
+        if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); }
         __syncthreads();
-        load_tile<TM, NT, VEC>(Ysm, A, lda, m, n, n16, row0);
-        __syncthreads();
-        solve_tile<TM, NW>(Ysm, RsPrep, Dsm, n16);
-        __syncthreads();
-        if (Ydump) store_tile<TM, NT, false>(Ysm, Ydump, m, m, n, row0);
         for (int sw = 0; sw < sweeps; ++sw) {
             double acc[GRAM_MAXS][4][2];
             int pp[GRAM_MAXS], qq[GRAM_MAXS];
@@ -167,21 +223,22 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
 #pragma unroll
                 for (int b = 0; b < 4; ++b) acc[u][b][0] = acc[u][b][1] = 0.0;
             }
-            for (int ks = 0; ks < TM / 4; ++ks) {
-                const double* yk = Ysm + g * LDT + 4 * ks + t;          // fragment (i = g, row = t)
+            for (int w = 0; w < NW; ++w)
+                for (int ks = 0; ks < SR / 4; ++ks) {
+                    const double* yk = Ysm + (size_t)w * slab_stride + g * LDS_ + 4 * ks + t;   // fragment (i = g, row = t)
 #pragma unroll
-                for (int u = 0; u < GRAM_MAXS; ++u) {
-                    if (u < cnt) {
-                        const double fa0 = yk[(16 * pp[u]) * LDT], fa1 = yk[(16 * pp[u] + 8) * LDT];
-                        double fb0 = fa0, fb1 = fa1;
-                        if (pp[u] != qq[u]) { fb0 = yk[(16 * qq[u]) * LDT]; fb1 = yk[(16 * qq[u] + 8) * LDT]; }
-                        dmma884(acc[u][0], fa0, fb0);
-                        dmma884(acc[u][1], fa0, fb1);
-                        if (pp[u] != qq[u]) dmma884(acc[u][2], fa1, fb0);
-                        dmma884(acc[u][3], fa1, fb1);
+                    for (int u = 0; u < GRAM_MAXS; ++u) {
+                        if (u < cnt) {
+                            const double fa0 = yk[(16 * pp[u]) * LDS_], fa1 = yk[(16 * pp[u] + 8) * LDS_];
+                            double fb0 = fa0, fb1 = fa1;
+                            if (pp[u] != qq[u]) { fb0 = yk[(16 * qq[u]) * LDS_]; fb1 = yk[(16 * qq[u] + 8) * LDS_]; }
+                            dmma884(acc[u][0], fa0, fb0);
+                            dmma884(acc[u][1], fa0, fb1);
+                            if (pp[u] != qq[u]) dmma884(acc[u][2], fa1, fb0);
+                            dmma884(acc[u][3], fa1, fb1);
+                        }
                     }
                 }
-            }
 #pragma unroll
             for (int u = 0; u < GRAM_MAXS; ++u) {
                 if (u < cnt) {
@@ -197,31 +254,35 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
             }
         }
         first_tile = false;
+        __syncthreads();
     }
 }
 
-template <int TM, int NW, bool VEC>
-__global__ void __launch_bounds__(NW * 32, (TM == 128 && NW == 4) ? 3 : 1)
+// K5: every warp streams its own slabs (slab i belongs to global warp i mod (grid * NW)); no CTA barrier.
+template <int RG, int NBT, bool VEC>
+__global__ void __launch_bounds__(384, 1)
 mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict__ A,
-               const double* __restrict__ RsPrep, const double* __restrict__ RcPrep,
-               int64_t ldq, double* __restrict__ Q, int64_t ntiles, double* __restrict__ Ydump)
+               const double2* __restrict__ fragS, const double2* __restrict__ fragC,
+               int64_t ldq, double* __restrict__ Q, int64_t nslabs, double* __restrict__ Ydump)
 {
     extern __shared__ __align__(16) double Ysm[];
-    constexpr int LDT = TM + 4, NT = NW * 32;
-    double* DsmS = Ysm + (size_t)n16 * LDT;
-    double* DsmC = DsmS + (size_t)n16 * 8;
-    load_diag_blocks<NT>(DsmS, RsPrep, n16);
-    load_diag_blocks<NT>(DsmC, RcPrep, n16);
-    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int64_t row0 = tile * TM;
-        __syncthreads();
-        load_tile<TM, NT, VEC>(Ysm, A, lda, m, n, n16, row0);
-        __syncthreads();
-        solve_tile<TM, NW>(Ysm, RsPrep, DsmS, n16);            // y = a Rs^-1, same code as K3
-        if (Ydump) { __syncthreads(); store_tile<TM, NT, false>(Ysm, Ydump, m, m, n, row0); __syncthreads(); }
-        solve_tile<TM, NW>(Ysm, RcPrep, DsmC, n16);            // q = y Rc^-1
-        __syncthreads();
-        store_tile<TM, NT, VEC>(Ysm, Q, ldq, m, n, row0);
+    constexpr int SR = 8 * RG, LDS_ = SR + 4;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int nB = n16 >> 3;
+    double* slab = Ysm + (size_t)warp * n16 * LDS_;
+    zero_pad_columns<SR>(slab, n, n16, lane);
+    const int64_t stride = (int64_t)gridDim.x * nw;
+    for (int64_t i = (int64_t)blockIdx.x * nw + warp; i < nslabs; i += stride) {
+        const int64_t row0 = i * SR;
+        __syncwarp();
+        load_slab<SR, VEC>(slab, A, lda, m, n, row0, lane);
+        if (VEC) cp_async_wait_all();
+        __syncwarp();
+        solve_slab<RG, 0, NBT>(slab, fragS, nB, lane);        // y = a Rs^-1, same code as K3
+        if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); __syncwarp(); }
+        solve_slab<RG, 1, NBT>(slab, fragC, nB, lane);        // q = y Rc^-1
+        __syncwarp();
+        store_slab<SR, VEC>(slab, Q, ldq, m, n, row0, lane);
     }
 }
 
@@ -273,6 +334,14 @@ size_t k3_partials_bytes(int n)
     return (size_t)num_sms() * 4 * (size_t)c.n16 * c.n16 * sizeof(double);
 }
 
+int upload_diag(const double* prep, int n16, int fac, cudaStream_t s)
+{
+    const int nB = n16 >> 3;
+    cudaMemcpyToSymbolAsync(c_diag, prep + prep_diag_offset(nB), sizeof(double) * PREP_DIAG * nB,
+                            sizeof(double) * (size_t)fac * PREP_MAX_NB * PREP_DIAG, cudaMemcpyDeviceToDevice, s);
+    return 1;
+}
+
 template <typename K>
 static int grid_for(K kernel, int threads, int smem, int64_t ntiles)
 {
@@ -287,24 +356,29 @@ static int grid_for(K kernel, int threads, int smem, int64_t ntiles)
 
 static bool vec_ok(const void* p, int64_t ld) { return ((uintptr_t)p % 16 == 0) && (ld % 2 == 0); }
 
-#define MRCQR_ROW_DISPATCH(CALL)                                                     \
-    if (c.TM == 128 && c.NW == 4) { if (vec) { CALL(128, 4, true) } else { CALL(128, 4, false) } }      \
-    else if (c.TM == 128 && c.NW == 8) { if (vec) { CALL(128, 8, true) } else { CALL(128, 8, false) } } \
-    else if (c.TM == 64) { if (vec) { CALL(64, 8, true) } else { CALL(64, 8, false) } }                 \
-    else { if (vec) { CALL(32, 4, true) } else { CALL(32, 4, false) } }
-
 int launch_k3_gram(int64_t m, int n, int64_t lda, const double* A, const double* RsPrep,
                    double* partials, int* n_partials_out, double* Ydump, cudaStream_t s)
 {
     RowCfg c = row_config(n);
-    const int64_t ntiles = (m + c.TM - 1) / c.TM;
+    const int TM = 8 * c.RG * c.NW;
+    const int64_t ntiles = (m + TM - 1) / TM;
     const bool vec = vec_ok(A, lda);
-#define K3_CALL(TM_, NW_, V_)                                                                       \
-    { auto k = mrcqr_k3_gram<TM_, NW_, V_>;                                                         \
+    const double2* frag = reinterpret_cast<const double2*>(RsPrep);
+#define K3_GO(RG_, NW_, NB_, V_)                                                                    \
+    { auto k = mrcqr_k3_gram<RG_, NW_, NB_, V_>;                                                    \
       int grid = grid_for(k, NW_ * 32, c.smem_bytes, ntiles); *n_partials_out = grid;               \
-      k<<<grid, NW_ * 32, c.smem_bytes, s>>>(m, n, c.n16, lda, A, RsPrep, partials, ntiles, Ydump); }
-    MRCQR_ROW_DISPATCH(K3_CALL)
+      k<<<grid, NW_ * 32, c.smem_bytes, s>>>(m, n, c.n16, lda, A, frag, partials, ntiles, Ydump); }
+#define K3_CALL(RG_, NW_, NB_) { if (vec) K3_GO(RG_, NW_, NB_, true) else K3_GO(RG_, NW_, NB_, false) }
+    switch (c.n16) {
+        case 16:  K3_CALL(4, 4, 2) break;   case 32:  K3_CALL(4, 4, 4) break;
+        case 48:  K3_CALL(4, 4, 6) break;   case 64:  K3_CALL(4, 4, 8) break;
+        case 80:  K3_CALL(2, 8, 10) break;  case 96:  K3_CALL(2, 8, 12) break;
+        case 112: K3_CALL(2, 8, 14) break;  case 128: K3_CALL(2, 8, 16) break;
+        default:
+            if (c.n16 <= 256) K3_CALL(1, 8, 0) else K3_CALL(1, 4, 0)
+    }
 #undef K3_CALL
+#undef K3_GO
     return 1;
 }
 
@@ -312,14 +386,32 @@ int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double
                     const double* RcPrep, int64_t ldq, double* Q, double* Ydump, cudaStream_t s)
 {
     RowCfg c = row_config(n);
-    const int64_t ntiles = (m + c.TM - 1) / c.TM;
+    const int SR = 8 * c.RG;
+    const int slab_bytes = c.n16 * (SR + 4) * 8;
+    int nw = SMEM_CAP / slab_bytes;
+    if (nw > 12) nw = 12;
+    if (nw < 1) nw = 1;
+    const int smem = nw * slab_bytes;
+    const int64_t nslabs = (m + SR - 1) / SR;
+    int64_t grid = (nslabs + nw - 1) / nw;
+    if (grid > num_sms()) grid = num_sms();
     const bool vec = vec_ok(A, lda) && vec_ok(Q, ldq);
-#define K5_CALL(TM_, NW_, V_)                                                                       \
-    { auto k = mrcqr_k5_formq<TM_, NW_, V_>;                                                        \
-      int grid = grid_for(k, NW_ * 32, c.smem_bytes, ntiles);                                       \
-      k<<<grid, NW_ * 32, c.smem_bytes, s>>>(m, n, c.n16, lda, A, RsPrep, RcPrep, ldq, Q, ntiles, Ydump); }
-    MRCQR_ROW_DISPATCH(K5_CALL)
+    const double2* fS = reinterpret_cast<const double2*>(RsPrep);
+    const double2* fC = reinterpret_cast<const double2*>(RcPrep);
+#define K5_GO(RG_, NB_, V_)                                                                         \
+    { auto k = mrcqr_k5_formq<RG_, NB_, V_>;                                                           \
+      cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);                   \
+      k<<<(int)grid, nw * 32, smem, s>>>(m, n, c.n16, lda, A, fS, fC, ldq, Q, nslabs, Ydump); }
+#define K5_CALL(RG_, NB_) { if (vec) K5_GO(RG_, NB_, true) else K5_GO(RG_, NB_, false) }
+    switch (c.n16) {
+        case 16:  K5_CALL(4, 2) break;   case 32:  K5_CALL(4, 4) break;
+        case 48:  K5_CALL(4, 6) break;   case 64:  K5_CALL(4, 8) break;
+        case 80:  K5_CALL(2, 10) break;  case 96:  K5_CALL(2, 12) break;
+        case 112: K5_CALL(2, 14) break;  case 128: K5_CALL(2, 16) break;
+        default:  K5_CALL(1, 0)
+    }
 #undef K5_CALL
+#undef K5_GO
     return 1;
 }
 

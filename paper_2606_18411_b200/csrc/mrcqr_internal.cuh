@@ -16,17 +16,53 @@ __device__ __forceinline__ void report(Status* st, int code, int info)
 
 inline int round_up(int x, int q) { return (x + q - 1) / q * q; }
 
-// ---- tile geometry of the row-streaming kernels (K3 / K5), chosen from n only -----------------
-// n16 = n padded to a multiple of 16 (8-wide DMMA blocks, 16-wide Gram super-blocks).
-struct RowCfg { int n16; int TM; int NW; int smem_bytes; int ctas_per_sm; };
+// ---- slab geometry of the row-streaming kernels (K3 / K5), chosen from n only -----------------
+// n16 = n padded to a multiple of 16 (8-wide DMMA blocks in pairs).  A warp owns a slab of 8*RG rows,
+// a CTA NW slabs; slab = n16 x (8*RG + 4) doubles of shared memory.
+struct RowCfg { int n16; int RG; int NW; int smem_bytes; };
 RowCfg row_config(int n);
 
-// "prepared" upper-triangular factor consumed by the tile solve: n16 x n16 col-major, ld = n16,
-//   strictly upper part = -R[k,j], diagonal = 1/R[j,j], padding = identity, strictly lower = 0.
-// Built once per factor by prep_R; both K3 and K5 read the same buffer (bit-identical Y).
+// "prepared" upper-triangular factor consumed by the slab solve (n16 x n16 doubles reserved), nB = n16/8:
+//   [0, 64 * nB(nB-1)/2)   off-diagonal 8x8 blocks (K < J) in DMMA B-fragment order, pair index
+//                          J(J-1)/2 + K, 32 lanes x (k = t, k = t + 4) of -R   (see rows.cuh)
+//   [.., + 36 * nB)        diagonal blocks: 8 reciprocals 1/R[j,j], then 28 values -R[j,jj], j < jj
+// padding rows / columns (>= n) are the identity.  Built once per factor by prep_R (R_s) and by the
+// Cholesky kernel (R_c); K3 and K5 read the same buffer (bit-identical Y).  The diagonal part is also
+// copied to constant memory (upload_diag) before the row kernels run.
+constexpr int PREP_DIAG = 36;
+constexpr int PREP_MAX_NB = 64;
+__host__ __device__ inline size_t prep_diag_offset(int nB) { return (size_t)32 * nB * (nB - 1); }
+// value of prepared element o (0 <= o < prep_diag_offset + 36 nB) from R (n x n, element (i,j) = R[j*ldr+i]);
+// *zero_diag is set when a diagonal entry is 0 / non-finite
+__device__ __forceinline__ double prep_value(const double* R, int ldr, int n, int nB, size_t o, int* bad_col)
+{
+    const size_t doff = prep_diag_offset(nB);
+    if (o < doff) {
+        const int pair = (int)(o >> 6), w = (int)(o & 63), lane = w >> 1, h = w & 1;
+        int J = 1;
+        while ((J + 1) * J / 2 <= pair) ++J;
+        const int K = pair - J * (J - 1) / 2;
+        const int g = lane >> 2, t = lane & 3;
+        const int row = 8 * K + t + 4 * h, col = 8 * J + (g >> 1) + 4 * (g & 1);
+        return (row < n && col < n) ? -R[(size_t)col * ldr + row] : 0.0;
+    }
+    const int e = (int)(o - doff), J = e / PREP_DIAG, i = e % PREP_DIAG;
+    if (i < 8) {
+        const int j = 8 * J + i;
+        if (j >= n) return 1.0;
+        const double d = R[(size_t)j * ldr + j];
+        if (!(fabs(d) > 0.0) || isinf(d)) *bad_col = j;
+        return 1.0 / d;
+    }
+    int j = 0, rem = i - 8;
+    while (rem >= 7 - j) { rem -= 7 - j; ++j; }
+    const int row = 8 * J + j, col = 8 * J + j + 1 + rem;
+    return (row < n && col < n) ? -R[(size_t)col * ldr + row] : 0.0;
+}
 
 // launchers (each returns the number of kernel launches it enqueued)
 int launch_prep_R(const double* R, int n, double* Rprep, int n16, Status* st, int err_code, cudaStream_t s);
+int upload_diag(const double* prep, int n16, int fac, cudaStream_t s);      // prepared diagonal blocks -> constant memory
 int launch_k3_gram(int64_t m, int n, int64_t lda, const double* A, const double* RsPrep,
                    double* partials, int* n_partials_out, double* Ydump, cudaStream_t s);
 int launch_reduce_partials(const double* partials, int n_partials, int n, int n16, double* G16, cudaStream_t s);
