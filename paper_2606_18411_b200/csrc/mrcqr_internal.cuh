@@ -25,7 +25,7 @@ RowCfg row_config(int n);
 // "prepared" upper-triangular factor consumed by the slab solve (n16 x n16 doubles reserved), nB = n16/8:
 //   [0, 64 * nB(nB-1)/2)   off-diagonal 8x8 blocks (K < J) in DMMA B-fragment order, pair index
 //                          J(J-1)/2 + K, 32 lanes x (k = t, k = t + 4) of -R   (see rows.cuh)
-//   [.., + 36 * nB)        diagonal blocks: 8 reciprocals 1/R[j,j], then 28 values -R[j,jj], j < jj
+//   [.., + 36 * nB)        diagonal blocks: 8 reciprocals 1/R[j,j], then 28 values -R[j,jj]/R[jj,jj], j < jj
 // padding rows / columns (>= n) are the identity.  Built once per factor by prep_R (R_s) and by the
 // Cholesky kernel (R_c); K3 and K5 read the same buffer (bit-identical Y).  The diagonal part is also
 // copied to constant memory (upload_diag) before the row kernels run.
@@ -57,7 +57,7 @@ __device__ __forceinline__ double prep_value(const double* R, int ldr, int n, in
     int j = 0, rem = i - 8;
     while (rem >= 7 - j) { rem -= 7 - j; ++j; }
     const int row = 8 * J + j, col = 8 * J + j + 1 + rem;
-    return (row < n && col < n) ? -R[(size_t)col * ldr + row] : 0.0;
+    return (row < n && col < n) ? -R[(size_t)col * ldr + row] / R[(size_t)col * ldr + col] : 0.0;
 }
 
 // launchers (each returns the number of kernel launches it enqueued)

@@ -107,27 +107,19 @@ __device__ __forceinline__ void store_slab(const double* slab, double* __restric
     }
 }
 
-// 8x8 substitution of global block Kg for the rows of this warp, one thread per row, in place in
-// the slab:  y_j = t_j * (1/R[j,j]),  t_jj += y_j * (-R[j,jj])  (jj > j).
-template <int SR, int FAC>
-__device__ __forceinline__ void diag_rows(double* slab, int Kg, int lane)
+// 8x8 substitution of one diagonal block for one row, in registers:
+//   y_jj = t_jj / R[jj,jj] + sum_{j<jj} y_j * (-R[j,jj] / R[jj,jj]),
+// i.e. the columns are scaled first (8 independent multiplies) and the substitution is unit upper
+// triangular: the dependent chain is 7 fma deep instead of 16 operations.  c: the block's 36 prepared
+// coefficients (constant memory, warp-uniform).
+__device__ __forceinline__ void diag_substitute(double (&y)[8], const double* c)
 {
-    constexpr int LDS_ = SR + 4;
-    if (SR >= 32 || lane < SR) {
-        double* yr = slab + (8 * Kg) * LDS_ + lane;
-        const double* c = &c_diag[FAC][Kg * PREP_DIAG];
-        double y[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) y[j] = yr[j * LDS_];
+    for (int j = 0; j < 8; ++j) y[j] = y[j] * c[j];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            y[j] = y[j] * c[j];
+    for (int j = 0; j < 8; ++j)
 #pragma unroll
-            for (int jj = j + 1; jj < 8; ++jj) y[jj] = fma(y[j], c[diag_off(j, jj)], y[jj]);
-        }
-#pragma unroll
-        for (int j = 0; j < 8; ++j) yr[j * LDS_] = y[j];
-    }
+        for (int jj = j + 1; jj < 8; ++jj) y[jj] = fma(y[j], c[diag_off(j, jj)], y[jj]);
 }
 
 // Fragment conventions (fixed, so the summation order is fixed).  DMMA.8x8x4: lane (g, t) = (lane/4,
@@ -141,7 +133,79 @@ __device__ __forceinline__ const double2* fragpair(const double2* __restrict__ f
     return frag + ((size_t)(Jg * (Jg - 1) / 2 + Kg) * 32 + lane);
 }
 
-// One panel of PB column blocks starting at global block P0, for the RG row groups of this warp.
+// ---- where a block goes between its DMMA (accumulator) form and its one-thread-per-row form -------
+// SlabXpose: through the block's own columns of the slab (leading dimension SR + 4); the solved block
+// stays there (in-place solve).
+template <int RG>
+struct SlabXpose {
+    static constexpr int SR = 8 * RG, LDS_ = SR + 4;
+    static constexpr bool REUSE = false;      // every block has its own columns: no barrier before the next step
+    double* slab; int lane, g, t;
+    __device__ __forceinline__ SlabXpose(double* s, int l) : slab(s), lane(l), g(l >> 2), t(l & 3) {}
+    __device__ __forceinline__ double* accp(int Kg, int rg, int e) const { return slab + (8 * Kg + t + 4 * e) * LDS_ + 8 * rg + g; }
+    __device__ __forceinline__ double* rowp(int Kg, int j) const { return slab + (8 * Kg + j) * LDS_ + lane; }
+    __device__ __forceinline__ bool row_active() const { return SR >= 32 || lane < SR; }
+};
+struct NoSink { __device__ __forceinline__ void operator()(int, const double (&)[8]) const {} };
+
+// The right-looking sweep inside a panel of PB column blocks starting at global block P0, on the
+// accumulator registers acc[rg][J][e] (matrix column 8(P0+J) + t + 4e of row 8 rg + g).
+// Step K: block K is final; it goes through X to one thread per row for its 8x8 substitution and
+// comes back as A fragments.  The updates of the
+// blocks J > K+1 by block K are DELAYED into step K+1, where they are independent of (and overlap
+// with) the dependent fma chain of that step's substitution; only J = K+1 is updated at once.
+// sink(Kg, y) sees every solved block in row form (lane = row of the slab).
+// This is the ONLY place the solve's arithmetic lives: K3 and K5 both run it.
+template <int RG, int FAC, int PB, typename X, typename SINK>
+__device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp, const double2* __restrict__ frag,
+                                           int P0, int lane, const SINK& sink)
+{
+    double ap0[RG], ap1[RG];                                  // A fragments of block K-1
+#pragma unroll
+    for (int K = 0; K < PB; ++K) {
+#pragma unroll
+        for (int rg = 0; rg < RG; ++rg) { *xp.accp(P0 + K, rg, 0) = acc[rg][K][0]; *xp.accp(P0 + K, rg, 1) = acc[rg][K][1]; }
+        __syncwarp();
+        double y[8];
+        if (xp.row_active()) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) y[j] = *xp.rowp(P0 + K, j);
+        }
+        if (K > 0) {
+#pragma unroll
+            for (int J = K + 1; J < PB; ++J) {
+                const double2 b = __ldg(fragpair(frag, P0 + K - 1, P0 + J, lane));
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], ap0[rg], b.x);
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], ap1[rg], b.y);
+            }
+        }
+        if (xp.row_active()) {
+            diag_substitute(y, &c_diag[FAC][(P0 + K) * PREP_DIAG]);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) *xp.rowp(P0 + K, j) = y[j];
+            sink(P0 + K, y);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int rg = 0; rg < RG; ++rg) { ap0[rg] = *xp.accp(P0 + K, rg, 0); ap1[rg] = *xp.accp(P0 + K, rg, 1); }
+        if (X::REUSE) {
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) { acc[rg][K][0] = ap0[rg]; acc[rg][K][1] = ap1[rg]; }
+        }
+        if (K + 1 < PB) {
+            const double2 b = __ldg(fragpair(frag, P0 + K, P0 + K + 1, lane));
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][K + 1], ap0[rg], b.x);
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][K + 1], ap1[rg], b.y);
+        }
+        if (X::REUSE) __syncwarp();
+    }
+}
+
+// One panel of PB column blocks starting at global block P0 of an in-place slab solve.
 template <int RG, int FAC, int PB>
 __device__ __forceinline__ void solve_panel(double* slab, const double2* __restrict__ frag, int P0, int lane)
 {
@@ -173,33 +237,7 @@ __device__ __forceinline__ void solve_panel(double* slab, const double2* __restr
             for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a1[rg], b.y);
         }
     }
-    // ---- inside the panel: right-looking
-#pragma unroll
-    for (int K = 0; K < PB; ++K) {
-#pragma unroll
-        for (int rg = 0; rg < RG; ++rg) {
-            yw[(8 * (P0 + K)) * LDS_ + 8 * rg] = acc[rg][K][0];
-            yw[(8 * (P0 + K) + 4) * LDS_ + 8 * rg] = acc[rg][K][1];
-        }
-        __syncwarp();
-        diag_rows<SR, FAC>(slab, P0 + K, lane);
-        __syncwarp();
-        if (K + 1 < PB) {
-#pragma unroll
-            for (int rg = 0; rg < RG; ++rg) {                // solved block K, back in A-fragment form
-                acc[rg][K][0] = yw[(8 * (P0 + K)) * LDS_ + 8 * rg];
-                acc[rg][K][1] = yw[(8 * (P0 + K) + 4) * LDS_ + 8 * rg];
-            }
-#pragma unroll
-            for (int J = K + 1; J < PB; ++J) {
-                const double2 b = __ldg(fragpair(frag, P0 + K, P0 + J, lane));
-#pragma unroll
-                for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], acc[rg][K][0], b.x);
-#pragma unroll
-                for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], acc[rg][K][1], b.y);
-            }
-        }
-    }
+    panel_core<RG, FAC, PB>(acc, SlabXpose<RG>(slab, lane), frag, P0, lane, NoSink());
 }
 
 // In-place Y <- Y * R^-1 on this warp's slab (8*RG rows x 8*nB columns).  frag: prepared factor in
