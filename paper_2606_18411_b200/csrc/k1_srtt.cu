@@ -235,7 +235,9 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec)
 size_t k1_workspace_bytes(int64_t m, int n, int s, int prec)
 {
     K1Params p = k1_params(m, n, m, s, prec);
-    return (size_t)((n + 1) / 2) * p.chunks * 2 * (size_t)s * sizeof(double);
+    const size_t fft = (size_t)((n + 1) / 2) * p.chunks * 2 * (size_t)s * sizeof(double);
+    const size_t tc = k1_tc_workspace_bytes();
+    return fft > tc ? fft : tc;
 }
 
 template <typename T, int PREC>
@@ -254,6 +256,8 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
                    Status* st, cudaStream_t stream)
 {
+    if (k1_tc_usable(m, n, lda, A, prec, s))
+        return launch_k1_tc(m, n, lda, A, s, signs, idx, k1_work, As, st, stream);
     K1Params p = k1_params(m, n, lda, s, prec);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
     double* partial = reinterpret_cast<double*>(k1_work);

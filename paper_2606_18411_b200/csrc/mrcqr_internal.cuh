@@ -79,6 +79,12 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
                    Status* st, cudaStream_t stream);
 
+// K1, tensor-core form for the FP16 sketch with s <= 128 (k1_tc.cu)
+bool k1_tc_usable(int64_t m, int n, int64_t lda, const double* A, int prec, int s);
+size_t k1_tc_workspace_bytes();
+int launch_k1_tc(int64_t m, int n, int64_t lda, const double* A, int s, const uint64_t* signs,
+                 const int64_t* idx, void* work, double* As, Status* st, cudaStream_t stream);
+
 size_t k3_partials_bytes(int n);
 int num_sms();
 
