@@ -133,7 +133,7 @@ static int enqueue_sketch(const Layout& L, int64_t m, int n, int64_t lda, const 
     double* As = reinterpret_cast<double*>(g.ws + L.As);
     int k = launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);
     if (As_out) cudaMemcpyAsync(As_out, As, sizeof(double) * (size_t)s * n, cudaMemcpyDeviceToDevice, st);
-    k += launch_k2_sketch_qr(As, s, n, nullptr, Rs, stat, st);
+    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16), stat, st);
     return k;
 }
 
@@ -151,7 +151,7 @@ static int enqueue_gram(const Layout& L, int64_t m, int n, int64_t lda, const do
     k += upload_diag(RsPrep, n16, 0, st);
     k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, Ydump, st);
     k += launch_reduce_partials(part, np, n, n16, G16, st);
-    k += launch_k4_cholesky(G16, n, n16, G_out, Rc, RcPrep, stat, st);
+    k += launch_k4_cholesky(G16, n, n16, G_out, Rc, RcPrep, nullptr, nullptr, stat, st);
     k += upload_diag(RcPrep, n16, 1, st);
     return k;
 }
@@ -235,7 +235,6 @@ extern "C" int mrcqr_sketch(int64_t m, int n, int64_t lda, const double* A, mrcq
     Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
     mrcqr_reset_status<<<1, 1, 0, st>>>(stat);
     int k = 1 + enqueue_sketch(L, m, n, lda, A, (int)prec, s, signs, idx, As_out, Rs, st);
-    k += launch_prep_R(Rs, n, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16), stat, MRCQR_ERR_SINGULAR, st);
     return finish(L, st, k);
 }
 
@@ -342,7 +341,7 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
     if (tm) cudaEventRecord(g.ev[0], st);
     k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);     // steps 2-4
     if (tm) cudaEventRecord(g.ev[1], st);
-    k += launch_k2_sketch_qr(As, s, n, nullptr, Rs, stat, st);                             // steps 5-6
+    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16), stat, st); // steps 5-6
     if (tm) cudaEventRecord(g.ev[2], st);
     {                                                                                      // step 7 + Alg.1 steps 1-2
         const int n16 = round_up(n, 16);
@@ -351,19 +350,16 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
         double* G16 = reinterpret_cast<double*>(g.ws + L.G16);
         double* part = reinterpret_cast<double*>(g.ws + L.k3);
         int np = 0;
-        k += launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st);
         k += upload_diag(RsPrep, n16, 0, st);
         if (tm) cudaEventRecord(g.ev[3], st);
         k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, st);
         if (tm) cudaEventRecord(g.ev[4], st);
         k += launch_reduce_partials(part, np, n, n16, G16, st);
-        k += launch_k4_cholesky(G16, n, n16, nullptr, Rc, RcPrep, stat, st);
+        k += launch_k4_cholesky(G16, n, n16, nullptr, Rc, RcPrep, Rs, R, stat, st);     // + step 9: R = Rc Rs
         k += upload_diag(RcPrep, n16, 1, st);
         if (tm) cudaEventRecord(g.ev[5], st);
         k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, st);           // Alg.1 step 3
-        if (tm) cudaEventRecord(g.ev[6], st);
-        k += launch_triu_mul(Rc, Rs, n, R, st);                                            // step 9
-        if (tm) cudaEventRecord(g.ev[7], st);
+        if (tm) { cudaEventRecord(g.ev[6], st); cudaEventRecord(g.ev[7], st); }
     }
     const int rc = finish(L, st, k);
     if (tm) for (int i = 0; i < 7; ++i) cudaEventElapsedTime(&g.stage_ms[i], g.ev[i], g.ev[i + 1]);

@@ -237,7 +237,10 @@ __global__ void mrcqr_k1_tc_finalize(K1TcParams p, int NG, const float* __restri
     const int i = e % p.s, j = e / p.s;
     const int64_t tpc = p.tiles_per_col, c_lo = j * tpc, c_hi = c_lo + tpc;
     double acc = 0.0;
-    for (int c = 0; c < p.grid; ++c) {
+    int c0 = (int)((c_lo * p.grid) / p.total_tiles) - 1, c1 = (int)((c_hi * p.grid) / p.total_tiles) + 1;
+    if (c0 < 0) c0 = 0;
+    if (c1 > p.grid - 1) c1 = p.grid - 1;
+    for (int c = c0; c <= c1; ++c) {
         const int64_t lo = tc_range_lo(c, p.grid, p.total_tiles), hi = tc_range_lo(c + 1, p.grid, p.total_tiles);
         if (lo >= hi || lo >= c_hi || hi <= c_lo) continue;
         const int seg = j - (int)(lo / tpc);

@@ -39,18 +39,23 @@ __global__ void mrcqr_triu_mul(const double* __restrict__ Rc, const double* __re
 
 // ---- K4 ---------------------------------------------------------------------------------------
 // Blocked right-looking Cholesky, 8 columns per outer step (3 barriers per 8 columns instead of 16):
-//   (1) warp 0 factors the 8x8 diagonal block (lane j owns column j in registers, shuffles),
-//   (2) one thread per trailing column solves its 8 rows against the block (the row panel),
+//   (1) warp 0 factors the 8x8 diagonal block (lane j owns column j in registers, shuffles); a pivot
+//       costs one rsqrt: Rc[p,p] = piv * rsqrt(piv), and rows are scaled by rsqrt(piv),
+//   (2) one thread per trailing column solves its 8 rows against the block (the row panel) with the
+//       stored reciprocals of the diagonal,
 //   (3) rank-8 update of the trailing upper triangle.
 // W: working copy of G (upper triangle used), col-major with leading dimension ldw.
-// Pn: the current row panel, Pn[p * n16 + j] = Rc[k0+p, j].
+// Pn: the current row panel, Pn[p * n16 + j] = Rc[k0+p, j].  dinv[j] = 1 / Rc[j,j].
+// Epilogue: Rc, the prepared Rc (fragment order) and, if Rs is given, R = Rc Rs (Algorithm 2 step 9).
 __global__ void __launch_bounds__(SMALL_NT)
 mrcqr_k4_cholesky(double* __restrict__ G16, int n, int n16, int use_smem, double* __restrict__ G_out,
-                  double* __restrict__ Rc, double* __restrict__ RcPrep, Status* st)
+                  double* __restrict__ Rc, double* __restrict__ RcPrep, const double* __restrict__ Rs,
+                  double* __restrict__ R, Status* st)
 {
     extern __shared__ __align__(16) double sm[];
     double* Pn = sm;                         // 8 * n16
-    double* W = use_smem ? sm + 8 * n16 : G16;
+    double* dinv = sm + 8 * n16;             // n16
+    double* W = use_smem ? sm + 9 * n16 : G16;
     const int ldw = use_smem ? n16 + 1 : n16;
     const int tid = threadIdx.x, NT = blockDim.x;
 
@@ -73,9 +78,10 @@ mrcqr_k4_cholesky(double* __restrict__ G16, int n, int n16, int use_smem, double
                 if (p < kb) {                                        // uniform
                     const double piv = __shfl_sync(0xffffffffu, c[p], p);
                     if (j == p && (!(piv > 0.0) || isinf(piv))) report(st, 3, k0 + p);
-                    const double d = sqrt(piv);
-                    const double rp = (j == p) ? d : c[p] / d;       // Rc[k0+p, k0+j] for j >= p
+                    const double ri = rsqrt(piv);
+                    const double rp = (j == p) ? piv * ri : c[p] * ri;   // Rc[k0+p, k0+j] for j >= p
                     c[p] = rp;
+                    if (j == p) dinv[k0 + p] = ri;
 #pragma unroll
                     for (int q = p + 1; q < 8; ++q) {                // c[q] -= Rc[p, q] * Rc[p, j]  (q <= j)
                         const double rq = __shfl_sync(0xffffffffu, rp, q);
@@ -96,7 +102,7 @@ mrcqr_k4_cholesky(double* __restrict__ G16, int n, int n16, int use_smem, double
                     double t = W[j * ldw + k0 + p];
 #pragma unroll
                     for (int q = 0; q < p; ++q) t = fma(-W[(k0 + p) * ldw + k0 + q], x[q], t);
-                    x[p] = t / W[(k0 + p) * ldw + k0 + p];
+                    x[p] = t * dinv[k0 + p];
                     W[j * ldw + k0 + p] = x[p];
                     Pn[p * n16 + j] = x[p];
                 } else x[p] = 0.0;
@@ -118,11 +124,15 @@ mrcqr_k4_cholesky(double* __restrict__ G16, int n, int n16, int use_smem, double
     }
     for (int e = tid; e < n * n; e += NT) {
         const int i = e % n, j = e / n;
-        const double w = (i <= j) ? W[j * ldw + i] : 0.0;
+        double w = 0.0, r = 0.0;
+        if (i <= j) {
+            w = W[j * ldw + i];
+            if (R) for (int k = i; k <= j; ++k) r = fma(W[k * ldw + i], Rs[(size_t)j * n + k], r);
+        }
         Rc[e] = w;
+        if (R) R[e] = r;
     }
-    __syncthreads();
-    {                                        // prepared R_c (fragment order + diagonal blocks), from W
+    {                                        // prepared Rc (fragment order + diagonal blocks), from W
         const int nB = n16 >> 3;
         const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
         int bad = -1;
@@ -138,8 +148,21 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
+// epilogue shared by both K2 variants: Rs (just written by this CTA) -> prepared Rs, singular check
+__device__ __forceinline__ void k2_prepare(const double* Rs, int n, double* RsPrep, int n16, Status* st)
+{
+    if (!RsPrep) return;
+    __syncthreads();
+    const int nB = n16 >> 3;
+    const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
+    int bad = -1;
+    for (size_t o = threadIdx.x; o < total; o += blockDim.x) RsPrep[o] = prep_value(Rs, n, n, nB, o, &bad);
+    if (bad >= 0) report(st, 2, bad);
+}
+
 __global__ void __launch_bounds__(SMALL_NT)
-mrcqr_k2_sketch_qr(double* __restrict__ As, int s, int n, int use_smem, double* __restrict__ Rs)
+mrcqr_k2_sketch_qr(double* __restrict__ As, int s, int n, int use_smem, double* __restrict__ Rs,
+                   double* __restrict__ RsPrep, int n16, Status* st)
 {
     extern __shared__ __align__(16) double sm[];
     double* betas = sm;                      // n
@@ -194,18 +217,22 @@ mrcqr_k2_sketch_qr(double* __restrict__ As, int s, int n, int use_smem, double* 
         if (i <= j && betas[i] < 0.0) v = -v;          // sign-normalise row i: diag(Rs) > 0
         Rs[e] = v;
     }
+    k2_prepare(Rs, n, RsPrep, n16, st);
 }
 
 // ---- K2, register-resident variant (n <= 32*CPW, s <= 32*RPL) -----------------------------------------
 // Column c lives in warp c % 32 (slot c / 32), row i in lane i % 32 (slot i / 32): the whole sketch stays
-// in registers.  Per Householder step: ONE block barrier; the reflector v_j and tau_j travel through a
-// double-buffered shared vector; the warp that owns column j+1 forms v_{j+1} right after updating it.
+// in registers.  Per Householder step: ONE block barrier; the reflector travels through a double-buffered
+// shared vector; the warp that owns column j+1 forms v_{j+1} right after updating it.
+// Reflector, unnormalised: v = x - beta e_j (v_j = alpha - beta), H = I - c v v^T, c = 1 / (beta (beta - alpha))
+// (= tau / v_j^2 of the LAPACK form): one square root and one reciprocal per column.
 template <int CPW, int RPL>
 __global__ void __launch_bounds__(SMALL_NT)
-mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __restrict__ Rs)
+mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __restrict__ Rs,
+                       double* __restrict__ RsPrep, int n16, Status* st)
 {
     __shared__ double vbuf[2][RPL * 32];
-    __shared__ double taub[2];
+    __shared__ double cbuf[2];
     __shared__ double betas[32 * CPW];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     double a[CPW][RPL];
@@ -227,22 +254,21 @@ mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __re
         }
         const double alpha = __shfl_sync(0xffffffffu, alpha_l, j & 31);
         const double sigma = warp_sum(sig_l);
-        double beta = alpha, tau = 0.0, inv = 0.0;
+        double beta = alpha, cf = 0.0;
         if (sigma != 0.0) {
             const double nrm = sqrt(fma(alpha, alpha, sigma));
             beta = (alpha >= 0.0) ? -nrm : nrm;
-            tau = (beta - alpha) / beta;
-            inv = 1.0 / (alpha - beta);
+            cf = 1.0 / (beta * (beta - alpha));
         }
 #pragma unroll
         for (int r = 0; r < RPL; ++r) {
             const int i = lane + 32 * r;
-            const double v = (i > j) ? a[k][r] * inv : (i == j ? 1.0 : 0.0);
+            const double v = (i > j) ? a[k][r] : (i == j ? alpha - beta : 0.0);
             vbuf[j & 1][i] = v;
             if (i == j) a[k][r] = beta;                      // R[j,j]
             if (i > j) a[k][r] = 0.0;
         }
-        if (lane == 0) { taub[j & 1] = tau; betas[j] = beta; }
+        if (lane == 0) { cbuf[j & 1] = cf; betas[j] = beta; }
     };
     if (warp == 0) make_v(0, 0);
     for (int j = 0; j < n; ++j) {
@@ -250,7 +276,7 @@ mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __re
         double v[RPL];
 #pragma unroll
         for (int r = 0; r < RPL; ++r) v[r] = vbuf[j & 1][lane + 32 * r];
-        const double tau = taub[j & 1];
+        const double cf = cbuf[j & 1];
         double w[CPW];
 #pragma unroll
         for (int k = 0; k < CPW; ++k) {
@@ -266,7 +292,7 @@ mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __re
         for (int k = 0; k < CPW; ++k) {
             const int c = warp + 32 * k;
             if (c > j && c < n) {
-                const double wt = w[k] * tau;
+                const double wt = w[k] * cf;
 #pragma unroll
                 for (int r = 0; r < RPL; ++r) a[k][r] = fma(-wt, v[r], a[k][r]);
             }
@@ -287,6 +313,7 @@ mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __re
                 Rs[(size_t)c * n + i] = val;
             }
         }
+    k2_prepare(Rs, n, RsPrep, n16, st);
 }
 
 // ---- launchers --------------------------------------------------------------------------------
@@ -305,30 +332,31 @@ int launch_triu_mul(const double* Rc, const double* Rs, int n, double* R, cudaSt
 }
 
 int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double* Rc, double* RcPrep,
-                       Status* st, cudaStream_t s)
+                       const double* Rs, double* R, Status* st, cudaStream_t s)
 {
-    size_t need = ((size_t)8 * n16 + (size_t)n16 * (n16 + 1)) * sizeof(double);
+    size_t need = ((size_t)9 * n16 + (size_t)n16 * (n16 + 1)) * sizeof(double);
     const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
-    const size_t smem = use_smem ? need : (size_t)8 * n16 * sizeof(double);
+    const size_t smem = use_smem ? need : (size_t)9 * n16 * sizeof(double);
     const int threads = n16 <= 64 ? 256 : (n16 <= 128 ? 512 : SMALL_NT);
     cudaFuncSetAttribute(mrcqr_k4_cholesky, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mrcqr_k4_cholesky<<<1, threads, smem, s>>>(const_cast<double*>(G16), n, n16, use_smem, G_out, Rc, RcPrep, st);
+    mrcqr_k4_cholesky<<<1, threads, smem, s>>>(const_cast<double*>(G16), n, n16, use_smem, G_out, Rc, RcPrep, Rs, R, st);
     return 1;
 }
 
-int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* work, double* Rs, Status* st, cudaStream_t s)
+int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* Rs, double* RsPrep, int n16,
+                        Status* st, cudaStream_t s)
 {
-    (void)work; (void)st;
     if (n <= 64 && s_rows <= 256) {
-        if (n <= 32 && s_rows <= 128) mrcqr_k2_sketch_qr_reg<1, 4><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs);
-        else mrcqr_k2_sketch_qr_reg<2, 8><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs);
+        if (n <= 32 && s_rows <= 128) mrcqr_k2_sketch_qr_reg<1, 4><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
+        else if (s_rows <= 128) mrcqr_k2_sketch_qr_reg<2, 4><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
+        else mrcqr_k2_sketch_qr_reg<2, 8><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
         return 1;
     }
     size_t need = ((size_t)n + 2 + (size_t)s_rows * n) * sizeof(double);
     const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
     const size_t smem = use_smem ? need : ((size_t)n + 2) * sizeof(double);
     cudaFuncSetAttribute(mrcqr_k2_sketch_qr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mrcqr_k2_sketch_qr<<<1, SMALL_NT, smem, s>>>(const_cast<double*>(As), s_rows, n, use_smem, Rs);
+    mrcqr_k2_sketch_qr<<<1, SMALL_NT, smem, s>>>(const_cast<double*>(As), s_rows, n, use_smem, Rs, RsPrep, n16, st);
     return 1;
 }
 

@@ -287,31 +287,30 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
 }
 
 // G16[i,j] (i <= j) = sum over the CTA partials in a FIXED order (deterministic split-m reduction):
-// partials are taken in groups of 16 consecutive CTAs summed in order; thread q of an element adds the
-// groups q, q+8, q+16, ... in order; the 8 per-thread sums are combined by a fixed binary tree.
-// 32 elements x 8 group lanes per CTA; mirrored to the lower triangle.
-__global__ void __launch_bounds__(256)
+// thread (element, q) adds the partials q, q+32, q+64, ... in ascending order; the 32 per-thread sums of
+// an element are combined by a fixed binary tree in shared memory.  32 elements x 32 lanes per CTA;
+// mirrored to the lower triangle.
+__global__ void __launch_bounds__(1024)
 mrcqr_reduce_partials(const double* __restrict__ partials, int np, int n16, double* __restrict__ G16)
 {
-    __shared__ double sm[8][33];
+    __shared__ double sm[32][33];
     const int el = threadIdx.x & 31, q = threadIdx.x >> 5;
     const int e = blockIdx.x * 32 + el;
     const size_t stride = (size_t)n16 * n16;
     const int i = e % n16, j = e / n16;
     const bool live = (e < n16 * n16) && (i <= j);
     double total = 0.0;
-    if (live) {
-        for (int c0 = 16 * q; c0 < np; c0 += 16 * 8) {
-            double sub = 0.0;
-            const int c1 = min(np, c0 + 16);
-            for (int c = c0; c < c1; ++c) sub += partials[(size_t)c * stride + e];
-            total += sub;
-        }
-    }
+    if (live)
+        for (int c = q; c < np; c += 32) total += partials[(size_t)c * stride + e];
     sm[q][el] = total;
     __syncthreads();
+#pragma unroll
+    for (int h = 16; h > 0; h >>= 1) {
+        if (q < h) sm[q][el] += sm[q + h][el];
+        __syncthreads();
+    }
     if (q == 0 && live) {
-        const double t = ((sm[0][el] + sm[1][el]) + (sm[2][el] + sm[3][el])) + ((sm[4][el] + sm[5][el]) + (sm[6][el] + sm[7][el]));
+        const double t = sm[0][el];
         G16[e] = t;
         G16[(size_t)i * n16 + j] = t;
     }
@@ -419,7 +418,7 @@ int launch_reduce_partials(const double* partials, int n_partials, int n, int n1
 {
     (void)n;
     const int total = n16 * n16;
-    mrcqr_reduce_partials<<<(total + 31) / 32, 256, 0, s>>>(partials, n_partials, n16, G16);
+    mrcqr_reduce_partials<<<(total + 31) / 32, 1024, 0, s>>>(partials, n_partials, n16, G16);
     return 1;
 }
 

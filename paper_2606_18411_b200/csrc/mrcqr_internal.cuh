@@ -67,11 +67,13 @@ int launch_k3_gram(int64_t m, int n, int64_t lda, const double* A, const double*
                    double* partials, int* n_partials_out, double* Ydump, cudaStream_t s);
 int launch_reduce_partials(const double* partials, int n_partials, int n, int n16, double* G16, cudaStream_t s);
 int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double* Rc, double* RcPrep,
-                       Status* st, cudaStream_t s);
+                       const double* Rs, double* R, Status* st, cudaStream_t s);   // Rs, R nullable: R = Rc Rs
 int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double* RsPrep,
                     const double* RcPrep, int64_t ldq, double* Q, double* Ydump, cudaStream_t s);
 int launch_triu_mul(const double* Rc, const double* Rs, int n, double* R, cudaStream_t s);
-int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* work, double* Rs, Status* st, cudaStream_t s);
+// RsPrep nullable: when given, the kernel also writes the prepared Rs and reports a singular diagonal
+int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* Rs, double* RsPrep, int n16,
+                        Status* st, cudaStream_t s);
 
 // K1: sampled transform.  Returns launches.  As (s x n, ld = s) receives precision-p values in FP64.
 size_t k1_workspace_bytes(int64_t m, int n, int s, int prec);
