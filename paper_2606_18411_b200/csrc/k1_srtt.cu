@@ -256,8 +256,10 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
                    Status* st, cudaStream_t stream)
 {
-    if (k1_tc_usable(m, n, lda, A, prec, s))
-        return launch_k1_tc(m, n, lda, A, s, signs, idx, k1_work, As, st, stream);
+    if (k1_tc_usable(m, n, lda, A, prec, s)) {
+        const int k = launch_k1_tc(m, n, lda, A, s, signs, idx, k1_work, As, st, stream);
+        if (k > 0) return k;                          // < 0: the tensor map could not be encoded -> FFT form
+    }
     K1Params p = k1_params(m, n, lda, s, prec);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
     double* partial = reinterpret_cast<double*>(k1_work);

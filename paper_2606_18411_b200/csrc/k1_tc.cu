@@ -18,10 +18,12 @@
 // computes every butterfly in half.)
 //
 // A CTA (8 warps) keeps its rows of F as A fragments in registers for its whole life and streams
-// tiles of 256 (t1) x 32 (t2) elements of one column: LDG.128 of the next tile are in flight while
-// the current tile is multiplied; the converted / folded FP16 tile is double buffered in shared memory.
+// tiles of 256 (t1) x 32 (t2) elements of one column: the raw FP64 rows of the next two tiles arrive by
+// bulk asynchronous copies (cp.async.bulk, one 256-byte row per thread, completion on an mbarrier)
+// while the current tile is multiplied; the converted / folded FP16 tile is double buffered.
 #include "mrcqr_internal.cuh"
 #include <cuda_fp16.h>
+#include <cuda.h>
 
 namespace mrcqr {
 
@@ -67,6 +69,34 @@ __device__ __forceinline__ float diag_half(double a, unsigned neg)
     return neg ? -v : v;
 }
 
+// ---- mbarrier + bulk asynchronous copy (global -> shared, completion counted in bytes on the mbarrier) ----
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "MBAR_WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra MBAR_DONE_%=;\n\t"
+        "bra MBAR_WAIT_%=;\n\t"
+        "MBAR_DONE_%=:\n\t}"
+        ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+// TMA: one 3-D box (TC_NT t2 x 256 t1 x 1 column) of FP64 -> shared memory, completion in bytes on the mbarrier
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, int x, int y, int z, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(tm), "r"(x), "r"(y), "r"(z),
+                   "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+
 // lo / hi tile of CTA c out of G over T tiles: contiguous, balanced ranges of the column-major tile list
 __host__ __device__ __forceinline__ int64_t tc_range_lo(int c, int G, int64_t T) { return ((int64_t)c * T) / G; }
 
@@ -74,7 +104,7 @@ __host__ __device__ __forceinline__ int64_t tc_range_lo(int c, int G, int64_t T)
 // (2 NTW) m-tiles of 16 bins x (4 / NTW) column groups.
 template <int NTW>
 __global__ void __launch_bounds__(TC_THREADS, 1)
-mrcqr_k1_tc(K1TcParams p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
+mrcqr_k1_tc(K1TcParams p, const __grid_constant__ CUtensorMap tmapA, const uint32_t* __restrict__ signs32,
             const int64_t* __restrict__ idx, float* __restrict__ partial)
 {
     __shared__ __align__(16) __half Xe[2][128 * TC_LDX];
@@ -121,32 +151,43 @@ mrcqr_k1_tc(K1TcParams p, const double* __restrict__ A, const uint32_t* __restri
     const int64_t lo = tc_range_lo(blockIdx.x, p.grid, p.total_tiles);
     const int64_t hi = tc_range_lo(blockIdx.x + 1, p.grid, p.total_tiles);
     const int tpc = p.tiles_per_col;
-    double2 v[16];
-    unsigned sg = 0;
-    auto load_tile = [&](int64_t id) {
+    // raw FP64 tiles: 2 stages x 256 rows x 256 bytes, each filled by ONE TMA box load (thread 0 issues it)
+    extern __shared__ __align__(128) unsigned char raw_sm[];
+    __shared__ __align__(8) uint64_t mbar[2];
+    if (tid == 0) { mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+    unsigned sgs[2] = {0u, 0u};                       // this thread's sign bits of the tile in each stage
+    auto issue_tile = [&](int64_t id, int stg) {      // tile id -> raw stage stg; sign words -> registers
         const int j = (int)(id / tpc), tl = (int)(id % tpc);
-        const double* base = A + (size_t)j * (size_t)p.lda + (int64_t)tl * TC_NT + 2 * c16;
-        sg = 0;
+        if (tid == 0) {
+            mbar_arrive_expect_tx(&mbar[stg], TC_M1 * TC_NT * 8);
+            tma_load_3d(raw_sm + (size_t)stg * (TC_M1 * TC_NT * 8), &tmapA, tl * TC_NT, 0, j, &mbar[stg]);
+        }
+        unsigned sg = 0;
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             const int t1 = rgp + 16 * u, t1m = (t1 == 0) ? 128 : TC_M1 - t1;
-            v[2 * u] = __ldcs(reinterpret_cast<const double2*>(base + (int64_t)t1 * p.m2));
-            v[2 * u + 1] = __ldcs(reinterpret_cast<const double2*>(base + (int64_t)t1m * p.m2));
             const unsigned w0 = (signs32[((int64_t)t1 * p.m2 + (int64_t)tl * TC_NT) >> 5] >> (2 * c16)) & 3u;
             const unsigned w1 = (signs32[((int64_t)t1m * p.m2 + (int64_t)tl * TC_NT) >> 5] >> (2 * c16)) & 3u;
             sg |= (w0 | (w1 << 2)) << (4 * u);
         }
+        sgs[stg] = sg;
     };
-    auto convert_tile = [&](int b) {                 // DiagMult + fold + round to FP16
+    auto convert_tile = [&](int b) {                 // DiagMult + fold + round to FP16: raw[b] -> X[b]
+        const double2* raw = reinterpret_cast<const double2*>(raw_sm + (size_t)b * (TC_M1 * TC_NT * 8)) + c16;
+        const unsigned sg = b ? sgs[1] : sgs[0];
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const int t1 = rgp + 16 * u;
+            const int t1 = rgp + 16 * u, t1m = (t1 == 0) ? 128 : TC_M1 - t1;
+            const double2 va = raw[t1 * (TC_NT / 2)], vb = raw[t1m * (TC_NT / 2)];
             const unsigned bits = sg >> (4 * u);
-            const float f0 = diag_half(v[2 * u].x, bits & 1u), f1 = diag_half(v[2 * u].y, bits & 2u);
-            const float g0 = diag_half(v[2 * u + 1].x, bits & 4u), g1 = diag_half(v[2 * u + 1].y, bits & 8u);
-            uint32_t e, o;
-            if (t1 != 0) { e = pack_half2(f0 + g0, f1 + g1); o = pack_half2(f0 - g0, f1 - g1); }
-            else { e = pack_half2(f0, f1); o = 0u; x128[b][2 * c16] = g0; x128[b][2 * c16 + 1] = g1; }
+            const float f0 = diag_half(va.x, bits & 1u), f1 = diag_half(va.y, bits & 2u);
+            const float g0 = diag_half(vb.x, bits & 4u), g1 = diag_half(vb.y, bits & 8u);
+            const bool fold = (t1 != 0);              // t1 = 0: x~[0] alone; its "mirror" slot carries row 128
+            const uint32_t e = pack_half2(fold ? f0 + g0 : f0, fold ? f1 + g1 : f1);
+            const uint32_t o = fold ? pack_half2(f0 - g0, f1 - g1) : 0u;
+            if (!fold) { x128[b][2 * c16] = g0; x128[b][2 * c16 + 1] = g1; }
             *reinterpret_cast<uint32_t*>(&Xe[b][t1 * TC_LDX + 2 * c16]) = e;
             *reinterpret_cast<uint32_t*>(&Xo[b][t1 * TC_LDX + 2 * c16]) = o;
         }
@@ -165,11 +206,14 @@ mrcqr_k1_tc(K1TcParams p, const double* __restrict__ A, const uint32_t* __restri
             accb[h] = 0.0f;
         }
     };
-    if (lo < hi) { load_tile(lo); convert_tile(0); }
-    __syncthreads();
+    if (lo < hi) issue_tile(lo, 0);
+    if (lo + 1 < hi) issue_tile(lo + 1, 1);
     for (int64_t id = lo; id < hi; ++id) {
         const int b = (int)(id - lo) & 1;
-        if (id + 1 < hi) load_tile(id + 1);
+        mbar_wait(&mbar[b], (unsigned)((id - lo) >> 1) & 1u);
+        convert_tile(b);
+        __syncthreads();                              // X[b] complete; raw[b] and X[b^1] free
+        if (id + 2 < hi) { if (b == 0) issue_tile(id + 2, 0); else issue_tile(id + 2, 1); }
         // ---- first stage on the tensor cores: (Cc, Cs) = F * X~ for this warp's 16 bins x 8 NTW columns
         float accC[NTW][4], accS[NTW][4];
 #pragma unroll
@@ -221,8 +265,6 @@ mrcqr_k1_tc(K1TcParams p, const double* __restrict__ A, const uint32_t* __restri
             sincospif(2.0f * (float)r / (float)p.m, &st, &ct);
             accb[h] += ct * S1 - st * S2;
         }
-        if (id + 1 < hi) convert_tile(b ^ 1);
-        __syncthreads();
     }
     if (lo < hi) flush();
 }
@@ -253,9 +295,28 @@ __global__ void mrcqr_k1_tc_finalize(K1TcParams p, int NG, const float* __restri
     As[e] = v;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*tc_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static tc_encode_fn tc_encode()
+{
+    static tc_encode_fn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* ptr = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess) fn = reinterpret_cast<tc_encode_fn>(ptr);
+        else cudaGetLastError();
+    }
+    return fn;
+}
+
 bool k1_tc_usable(int64_t m, int n, int64_t lda, const double* A, int prec, int s)
 {
-    return prec == 16 && s <= 128 && m >= (int64_t)TC_M1 * TC_NT && n <= num_sms() &&
+    return tc_encode() != nullptr && prec == 16 && s <= 128 && m >= (int64_t)TC_M1 * TC_NT && n <= num_sms() &&
            ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
 }
 
@@ -272,9 +333,20 @@ int launch_k1_tc(int64_t m, int n, int64_t lda, const double* A, int s, const ui
     p.grid = (int)(p.total_tiles < num_sms() ? p.total_tiles : num_sms());
     float* partial = reinterpret_cast<float*>(work);
     const uint32_t* s32 = reinterpret_cast<const uint32_t*>(signs);
-    if (p.sp == 32) mrcqr_k1_tc<1><<<p.grid, TC_THREADS, 0, stream>>>(p, A, s32, idx, partial);
-    else if (p.sp == 64) mrcqr_k1_tc<2><<<p.grid, TC_THREADS, 0, stream>>>(p, A, s32, idx, partial);
-    else mrcqr_k1_tc<4><<<p.grid, TC_THREADS, 0, stream>>>(p, A, s32, idx, partial);
+    constexpr int raw_bytes = 2 * TC_M1 * TC_NT * 8;
+    CUtensorMap tm;
+    {   // A viewed as (t2: m2) x (t1: 256) x (column: n), strides 8, 8 m2, 8 lda bytes; box = 32 x 256 x 1
+        const cuuint64_t gdim[3] = {(cuuint64_t)p.m2, (cuuint64_t)TC_M1, (cuuint64_t)n};
+        const cuuint64_t gstr[2] = {(cuuint64_t)p.m2 * 8, (cuuint64_t)lda * 8};
+        const cuuint32_t box[3] = {TC_NT, TC_M1, 1}, estr[3] = {1, 1, 1};
+        if (tc_encode()(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(A), gdim, gstr, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return -1;
+    }
+#define K1TC_GO(NTW_) { cudaFuncSetAttribute(mrcqr_k1_tc<NTW_>, cudaFuncAttributeMaxDynamicSharedMemorySize, raw_bytes); \
+                        mrcqr_k1_tc<NTW_><<<p.grid, TC_THREADS, raw_bytes, stream>>>(p, tm, s32, idx, partial); }
+    if (p.sp == 32) K1TC_GO(1) else if (p.sp == 64) K1TC_GO(2) else K1TC_GO(4)
+#undef K1TC_GO
     mrcqr_k1_tc_finalize<<<(s * n + 255) / 256, 256, 0, stream>>>(p, 128 / p.sp, partial, As, st);
     return 2;
 }

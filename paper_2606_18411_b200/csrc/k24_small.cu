@@ -140,6 +140,114 @@ mrcqr_k4_cholesky(double* __restrict__ G16, int n, int n16, int use_smem, double
     }
 }
 
+// 1/sqrt(x) for a positive finite double: hardware seed + two Newton steps (a few ulp; the pivot's own
+// rounding error is of the same size).  Short dependent chain: it sits on the critical path of every pivot.
+__device__ __forceinline__ double rsqrt_fast(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double h = 0.5 * x;
+    y = y * fma(-h * y, y, 1.5);
+    y = y * fma(-h * y, y, 1.5);
+    return y;
+}
+
+// ---- K4, shared-memory form (n16 <= 160): unblocked right-looking, ONE barrier per pivot -----------
+// Step k: every thread updates its elements (i, j), k < i <= j, with the UNSCALED row k and the
+// reciprocal square root of pivot k:  W[i,j] -= (W[k,i] ri_k) (W[k,j] ri_k); the thread that owns
+// (k+1, k+1) then publishes ri_{k+1} = rsqrt(pivot), so the next step needs no second barrier.
+// Rows are scaled at the end: Rc[k,j] = W[k,j] ri_k, Rc[k,k] = pivot ri_k.
+template <int JM>                            // JM = ceil(n / 32): elements per thread = JM x JM, in registers per step
+__global__ void __launch_bounds__(SMALL_NT)
+mrcqr_k4_cholesky_sm(const double* __restrict__ G16, int n, int n16, double* __restrict__ G_out,
+                     double* __restrict__ Rc, double* __restrict__ RcPrep, const double* __restrict__ Rs,
+                     double* __restrict__ R, Status* st)
+{
+    extern __shared__ __align__(16) double sm[];
+    double* dinv = sm;                       // n16 (+ pad): ri_k
+    double* W = sm + n16 + 2;
+    const int ldw = n16 + 1;
+    const int tid = threadIdx.x, NT = blockDim.x;
+    for (int e = tid; e < n * n; e += NT) {
+        const int i = e % n, j = e / n;
+        const double v = G16[(size_t)j * n16 + i];
+        if (G_out) G_out[e] = v;
+        W[j * ldw + i] = v;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        const double piv = W[0];
+        if (!(piv > 0.0) || isinf(piv)) report(st, 3, 0);
+        dinv[0] = rsqrt(piv);
+    }
+    const int ti = tid & 31, tj = tid >> 5, NJ = 32;                 // 2-D thread layout: no index division
+    for (int k = 0; k < n - 1; ++k) {
+        __syncthreads();
+        if (tj + 32 * (JM - 1) <= k) continue;                       // warp-uniform: no column j > k in this warp
+        const double ri = dinv[k];
+        double a[JM], b[JM], w[JM][JM];
+#pragma unroll
+        for (int u = 0; u < JM; ++u) {                               // all loads first: nothing aliases column k
+            const int x = ti + 32 * u, y = tj + 32 * u;
+            a[u] = (x > k && x < n) ? W[x * ldw + k] : 0.0;
+            b[u] = (y > k && y < n) ? W[y * ldw + k] : 0.0;
+        }
+#pragma unroll
+        for (int v = 0; v < JM; ++v)
+#pragma unroll
+            for (int u = 0; u < JM; ++u) {
+                const int i = ti + 32 * u, j = tj + 32 * v;
+                w[v][u] = (i > k && i <= j && j < n) ? W[j * ldw + i] : 0.0;
+            }
+#pragma unroll
+        for (int v = 0; v < JM; ++v)
+#pragma unroll
+            for (int u = 0; u < JM; ++u) {
+                const int i = ti + 32 * u, j = tj + 32 * v;
+                if (i > k && i <= j && j < n) {
+                    const double r = fma(-(a[u] * ri), b[v] * ri, w[v][u]);
+                    W[j * ldw + i] = r;
+                    if (i == k + 1 && j == k + 1) {
+                        if (!(r > 0.0) || isinf(r)) report(st, 3, k + 1);
+                        dinv[k + 1] = rsqrt_fast(r);
+                    }
+                }
+            }
+    }
+    __syncthreads();
+    // scale the rows (W upper <- Rc); stage Rs in the free strictly-lower triangle, transposed:
+    // Rs[k,j] (k < j) at W[k*ldw + j], diag(Rs) in rsd
+    double* rsd = dinv + n16 + 2 + n16 * ldw;                        // n16 doubles after W
+    for (int j = tj; j < n; j += NJ)
+        for (int i = ti; i <= j; i += 32) {
+            W[j * ldw + i] *= dinv[i];
+            if (R) {
+                const double v = Rs[(size_t)j * n + i];
+                if (i < j) W[i * ldw + j] = v; else rsd[j] = v;
+            }
+        }
+    __syncthreads();
+    for (int j = tj; j < n; j += NJ)
+        for (int i = ti; i < n; i += 32) {
+            double w = 0.0, r = 0.0;
+            if (i <= j) {
+                w = W[j * ldw + i];
+                if (R) {
+                    for (int k = i; k < j; ++k) r = fma(W[k * ldw + i], W[k * ldw + j], r);
+                    r = fma(w, rsd[j], r);
+                }
+            }
+            Rc[(size_t)j * n + i] = w;
+            if (R) R[(size_t)j * n + i] = r;
+        }
+    {
+        const int nB = n16 >> 3;
+        const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
+        int bad = -1;
+        for (size_t o = tid; o < total; o += NT) RcPrep[o] = prep_value(W, ldw, n, nB, o, &bad);
+    }
+}
+
 // ---- K2 ---------------------------------------------------------------------------------------
 __device__ __forceinline__ double warp_sum(double v)
 {
@@ -334,9 +442,17 @@ int launch_triu_mul(const double* Rc, const double* Rs, int n, double* R, cudaSt
 int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double* Rc, double* RcPrep,
                        const double* Rs, double* R, Status* st, cudaStream_t s)
 {
-    size_t need = ((size_t)9 * n16 + (size_t)n16 * (n16 + 1)) * sizeof(double);
+    size_t need = ((size_t)9 * n16 + 2 + (size_t)n16 * (n16 + 1)) * sizeof(double);
     const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
     const size_t smem = use_smem ? need : (size_t)9 * n16 * sizeof(double);
+    if (use_smem) {
+        const size_t sm2 = ((size_t)2 * n16 + 2 + (size_t)n16 * (n16 + 1)) * sizeof(double);
+#define K4_GO(JM_) { cudaFuncSetAttribute(mrcqr_k4_cholesky_sm<JM_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2); \
+                     mrcqr_k4_cholesky_sm<JM_><<<1, SMALL_NT, sm2, s>>>(G16, n, n16, G_out, Rc, RcPrep, Rs, R, st); }
+        if (n <= 32) K4_GO(1) else if (n <= 64) K4_GO(2) else if (n <= 96) K4_GO(3) else if (n <= 128) K4_GO(4) else K4_GO(5)
+#undef K4_GO
+        return 1;
+    }
     const int threads = n16 <= 64 ? 256 : (n16 <= 128 ? 512 : SMALL_NT);
     cudaFuncSetAttribute(mrcqr_k4_cholesky, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     mrcqr_k4_cholesky<<<1, threads, smem, s>>>(const_cast<double*>(G16), n, n16, use_smem, G_out, Rc, RcPrep, Rs, R, st);
