@@ -26,6 +26,9 @@ sys.path.insert(0, ROOT)
 
 METRIC = "MRCQR FP64 thin-QR ms per factorization"
 FP64_DMMA_PEAK_TFLOPS = 37.2      # measured on this pool's B200 (profiles/r01_peaks.md), DMMA.8x8x4 issue peak
+# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the ncu --set full capture of
+# config C1 summarised in profiles/r01_ncu_full_v7.md; only valid for that workload
+NCU_TRAFFIC_C1 = {"k5_form_q": 536.97e6 + 486.98e6, "k3_gram": 554.86e6 + 22.85e6}
 HBM_FALLBACK_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
 
 
@@ -245,6 +248,8 @@ def run_ours(args):
             ach = dom_bytes / (dom_ms * 1e-3) / 1e9
             roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
                     "traffic": None, "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % how}
+        if cfg["name"] == "C1":
+            roof["traffic"] = NCU_TRAFFIC_C1.get(dom)
         roof.update({"kernel": dom, "kernel_ms": dom_ms, "algorithmic_bytes": dom_bytes, "algorithmic_flops": dom_flops,
                      "hbm_gbs_achieved": dom_bytes / (dom_ms * 1e-3) / 1e9})
         cpu = None
