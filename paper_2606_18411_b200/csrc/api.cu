@@ -63,7 +63,7 @@ static Layout make_layout(int64_t m, int n, int s, int prec)
     L.G16 = o;    o += al(n16 * n16 * 8);
     L.Rc = o;     o += al((size_t)n * n * 8);
     L.k1 = o;     o += al(s > 0 ? k1_workspace_bytes(m, n, s, prec) : 0);
-    L.k3 = o;     o += al(k3_partials_bytes(n));
+    L.k3 = o;     o += al(std::max(k3_partials_bytes(n), syrk_partials_bytes(n)));
     L.total = o;
     return L;
 }
@@ -167,7 +167,7 @@ static int enqueue_formq(const Layout& L, int64_t m, int n, int64_t lda, const d
     int k = 0;
     if (prep_rs) { k += launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st); k += upload_diag(RsPrep, n16, 0, st); }
     if (prep_rc) { k += launch_prep_R(Rc, n, RcPrep, n16, stat, MRCQR_ERR_BREAKDOWN, st); k += upload_diag(RcPrep, n16, 1, st); }
-    k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, Ydump, st);
+    k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, Ydump, 3, st);
     if (R) k += launch_triu_mul(Rc, Rs, n, R, st);
     return k;
 }
@@ -352,13 +352,21 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
         int np = 0;
         k += upload_diag(RsPrep, n16, 0, st);
         if (tm) cudaEventRecord(g.ev[3], st);
-        k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, st);
-        if (tm) cudaEventRecord(g.ev[4], st);
-        k += launch_reduce_partials(part, np, n, n16, G16, st);
+        const bool store_y = n16 > 128;          // Gram of a stored Y (k3_syrk.cu): Y = A Rs^-1 lives in the Q buffer
+        if (store_y) {
+            k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 1, st);
+            if (tm) cudaEventRecord(g.ev[4], st);
+            k += launch_syrk(m, n, ldq, Q, part, n16, G16, st);
+        } else {
+            k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, st);
+            if (tm) cudaEventRecord(g.ev[4], st);
+            k += launch_reduce_partials(part, np, n, n16, G16, st);
+        }
         k += launch_k4_cholesky(G16, n, n16, nullptr, Rc, RcPrep, Rs, R, stat, st);     // + step 9: R = Rc Rs
         k += upload_diag(RcPrep, n16, 1, st);
         if (tm) cudaEventRecord(g.ev[5], st);
-        k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, st);           // Alg.1 step 3
+        if (store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);   // q = y Rc^-1 in place
+        else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 3, st);        // Alg.1 step 3
         if (tm) { cudaEventRecord(g.ev[6], st); cudaEventRecord(g.ev[7], st); }
     }
     const int rc = finish(L, st, k);

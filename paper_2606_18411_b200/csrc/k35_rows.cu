@@ -259,11 +259,13 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
 }
 
 // K5: every warp streams its own slabs (slab i belongs to global warp i mod (grid * NW)); no CTA barrier.
+// mode 3: both solves (y = a Rs^-1, q = y Rc^-1); mode 1: only the first (store-Y form of stage 2a for
+// n16 > 128, Y goes to the Q buffer); mode 2: only the second, in place on the stored Y.
 template <int RG, int NBT, bool VEC>
 __global__ void __launch_bounds__(384, 1)
 mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict__ A,
                const double2* __restrict__ fragS, const double2* __restrict__ fragC,
-               int64_t ldq, double* __restrict__ Q, int64_t nslabs, double* __restrict__ Ydump)
+               int64_t ldq, double* __restrict__ Q, int64_t nslabs, double* __restrict__ Ydump, int mode)
 {
     extern __shared__ __align__(16) double Ysm[];
     constexpr int SR = 8 * RG, LDS_ = SR + 4;
@@ -278,9 +280,9 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
         load_slab<SR, VEC>(slab, A, lda, m, n, row0, lane);
         if (VEC) cp_async_wait_all();
         __syncwarp();
-        solve_slab<RG, 0, NBT>(slab, fragS, nB, lane);        // y = a Rs^-1, same code as K3
+        if (mode & 1) solve_slab<RG, 0, NBT>(slab, fragS, nB, lane);        // y = a Rs^-1, same code as K3
         if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); __syncwarp(); }
-        solve_slab<RG, 1, NBT>(slab, fragC, nB, lane);        // q = y Rc^-1
+        if (mode & 2) solve_slab<RG, 1, NBT>(slab, fragC, nB, lane);        // q = y Rc^-1
         __syncwarp();
         store_slab<SR, VEC>(slab, Q, ldq, m, n, row0, lane);
     }
@@ -382,7 +384,7 @@ int launch_k3_gram(int64_t m, int n, int64_t lda, const double* A, const double*
 }
 
 int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double* RsPrep,
-                    const double* RcPrep, int64_t ldq, double* Q, double* Ydump, cudaStream_t s)
+                    const double* RcPrep, int64_t ldq, double* Q, double* Ydump, int mode, cudaStream_t s)
 {
     RowCfg c = row_config(n);
     const int SR = 8 * c.RG;
@@ -400,7 +402,7 @@ int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double
 #define K5_GO(RG_, NB_, V_)                                                                         \
     { auto k = mrcqr_k5_formq<RG_, NB_, V_>;                                                           \
       cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);                   \
-      k<<<(int)grid, nw * 32, smem, s>>>(m, n, c.n16, lda, A, fS, fC, ldq, Q, nslabs, Ydump); }
+      k<<<(int)grid, nw * 32, smem, s>>>(m, n, c.n16, lda, A, fS, fC, ldq, Q, nslabs, Ydump, mode); }
 #define K5_CALL(RG_, NB_) { if (vec) K5_GO(RG_, NB_, true) else K5_GO(RG_, NB_, false) }
     switch (c.n16) {
         case 16:  K5_CALL(4, 2) break;   case 32:  K5_CALL(4, 4) break;

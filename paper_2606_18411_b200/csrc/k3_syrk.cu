@@ -1,0 +1,213 @@
+// k3_syrk.cu -- Gram matrix of a STORED Y (Algorithm 1 step 1) for n16 > 128.
+//
+// For n <= 128 the Gram matrix is accumulated inside K3 while Y is still in shared memory.  Beyond
+// that the upper triangle of G (131 k doubles at n = 512) no longer fits the register file of one SM,
+// so stage 2a runs in the paper's own order (TrsmPre writes A_1 = A Rs^-1, here into
+// the Q buffer), this kernel forms G = Y^T Y from it, and stage 2b solves in place (SURVEY.md 8(f)
+// "store-Y": 3 m n^2 flops instead of 4 m n^2; Y costs one write and 1 + reads of 8 m n bytes).
+//
+// G is cut into 128 x 128 blocks (I <= J); a CTA owns one block and one contiguous range of rows
+// (deterministic split of m), streams 32-row chunks of the two 128-column panels of Y through a
+// double-buffered shared-memory tile (cp.async) and accumulates on DMMA: 8 warps as 4 x 2, each
+// 32 x 64 of the block (4 x 8 accumulators, 12 fragment loads per 32 DMMA).  Accumulator chains are
+// flushed to the CTA's partial every 1024 rows (reading R7); a reduction kernel adds the
+// partials of a block in a fixed order.  No atomics: bit-reproducible.
+#include "mrcqr_internal.cuh"
+
+namespace mrcqr {
+
+constexpr int SY_B = 128;             // block edge (columns)
+constexpr int SY_KC = 32;             // rows per chunk
+constexpr int SY_LD = SY_KC + 4;      // 36: conflict-free DMMA fragment loads
+constexpr int SY_THREADS = 256;
+constexpr int SY_FLUSH = 32;          // chunks per accumulator chain (1024 rows = 256 DMMA k-steps)
+
+__device__ __forceinline__ void sy_dmma(double (&c)[2], double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void sy_cp16(void* dst, const void* src, int bytes)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src), "r"(bytes) : "memory");
+}
+
+struct SyrkParams {
+    int64_t m, ldy;
+    int n, n16, P, pairs, ksplit;
+    int64_t rows_per_split;           // multiple of SY_KC
+    int vec;
+};
+
+__device__ __forceinline__ void sy_pair(int p, int& I, int& J)      // p -> (I <= J), column-major over the upper triangle
+{
+    int j = 0;
+    while ((j + 1) * (j + 2) / 2 <= p) ++j;
+    J = j; I = p - j * (j + 1) / 2;
+}
+
+// loads rows [r0, r0+32) of the 128-column panel `pan` of Y into dst[col][SY_LD]; zero fill outside m x n
+__device__ __forceinline__ void sy_load_panel(double* dst, const SyrkParams& p, const double* __restrict__ Y,
+                                              int pan, int64_t r0, int tid)
+{
+    const int64_t left = p.m - r0;
+    if (p.vec) {
+        for (int e = tid; e < SY_B * (SY_KC / 2); e += SY_THREADS) {
+            const int col = e / (SY_KC / 2), r2 = (e % (SY_KC / 2)) * 2;
+            const int gc = pan * SY_B + col;
+            const int64_t avail = (gc < p.n) ? left - r2 : 0;
+            const int bytes = avail >= 2 ? 16 : (avail == 1 ? 8 : 0);
+            const double* src = Y + (bytes ? (size_t)gc * (size_t)p.ldy + r0 + r2 : 0);
+            sy_cp16(dst + col * SY_LD + r2, src, bytes);
+        }
+    } else {
+        for (int e = tid; e < SY_B * SY_KC; e += SY_THREADS) {
+            const int col = e / SY_KC, rr = e % SY_KC;
+            const int gc = pan * SY_B + col;
+            dst[col * SY_LD + rr] = (gc < p.n && rr < left) ? Y[(size_t)gc * (size_t)p.ldy + r0 + rr] : 0.0;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(SY_THREADS, 1)
+mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ partials)
+{
+    extern __shared__ __align__(16) double sy_sm[];        // [2 stages][2 panels][128 * SY_LD]
+    constexpr int PAN = SY_B * SY_LD;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+    const int pair = blockIdx.x / p.ksplit, ks_id = blockIdx.x % p.ksplit;
+    int I, J;
+    sy_pair(pair, I, J);
+    const bool diag = (I == J);
+    const int wi = warp & 3, wj = warp >> 2;
+    const bool skip = diag && (32 * wi >= 64 * wj + 64);    // sub-block strictly below the diagonal
+    const int64_t mpad = (p.m + SY_KC - 1) / SY_KC * SY_KC;
+    const int64_t k0 = (int64_t)ks_id * p.rows_per_split;
+    int64_t k1 = k0 + p.rows_per_split;
+    if (k1 > mpad) k1 = mpad;
+    const int nchunks = k1 > k0 ? (int)((k1 - k0) / SY_KC) : 0;
+    double* part = partials + (size_t)blockIdx.x * SY_B * SY_B;
+
+    double acc[4][8][2];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 8; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+    bool first = true;
+    auto issue = [&](int c) {
+        double* st = sy_sm + (size_t)(c & 1) * 2 * PAN;
+        sy_load_panel(st, p, Y, I, k0 + (int64_t)c * SY_KC, tid);
+        if (!diag) sy_load_panel(st + PAN, p, Y, J, k0 + (int64_t)c * SY_KC, tid);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    auto flush = [&]() {
+        if (!skip) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int b = 0; b < 8; ++b) {
+                    double* dst = part + (size_t)(64 * wj + 8 * b + 2 * t) * SY_B + 32 * wi + 8 * a + g;
+                    if (first) { dst[0] = acc[a][b][0]; dst[SY_B] = acc[a][b][1]; }
+                    else { dst[0] += acc[a][b][0]; dst[SY_B] += acc[a][b][1]; }
+                    acc[a][b][0] = acc[a][b][1] = 0.0;
+                }
+        }
+        first = false;
+    };
+    if (nchunks > 0) issue(0);
+    for (int c = 0; c < nchunks; ++c) {
+        if (c + 1 < nchunks) { issue(c + 1); asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+        else asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+        if (!skip) {
+            const double* pI = sy_sm + (size_t)(c & 1) * 2 * PAN;
+            const double* pJ = diag ? pI : pI + PAN;
+            const double* fi = pI + (32 * wi + g) * SY_LD + t;
+            const double* fj = pJ + (64 * wj + g) * SY_LD + t;
+#pragma unroll 2
+            for (int ks = 0; ks < SY_KC / 4; ++ks) {
+                double fI[4], fJ[8];
+#pragma unroll
+                for (int a = 0; a < 4; ++a) fI[a] = fi[(8 * a) * SY_LD + 4 * ks];
+#pragma unroll
+                for (int b = 0; b < 8; ++b) fJ[b] = fj[(8 * b) * SY_LD + 4 * ks];
+#pragma unroll
+                for (int a = 0; a < 4; ++a)
+#pragma unroll
+                    for (int b = 0; b < 8; ++b) sy_dmma(acc[a][b], fI[a], fJ[b]);
+            }
+        }
+        __syncthreads();
+        if ((c + 1) % SY_FLUSH == 0 || c + 1 == nchunks) flush();
+    }
+    if (nchunks == 0) flush();                               // an empty range still owns a (zero) partial
+}
+
+// G16[i,j] (i <= j) = sum over the row ranges of block (I,J), fixed order (32 lanes of ranges + binary tree)
+__global__ void __launch_bounds__(1024)
+mrcqr_syrk_reduce(SyrkParams p, const double* __restrict__ partials, double* __restrict__ G16)
+{
+    __shared__ double sm[32][33];
+    const int el = threadIdx.x & 31, q = threadIdx.x >> 5;
+    constexpr int CH = SY_B * SY_B / 32;
+    const int pair = blockIdx.x / CH, e = (blockIdx.x % CH) * 32 + el;
+    int I, J;
+    sy_pair(pair, I, J);
+    const int i = e % SY_B, j = e / SY_B;
+    const int gi = SY_B * I + i, gj = SY_B * J + j;
+    const bool live = gi <= gj && gj < p.n16;
+    double total = 0.0;
+    if (live)
+        for (int c = q; c < p.ksplit; c += 32) total += partials[((size_t)pair * p.ksplit + c) * SY_B * SY_B + e];
+    sm[q][el] = total;
+    __syncthreads();
+#pragma unroll
+    for (int h = 16; h > 0; h >>= 1) {
+        if (q < h) sm[q][el] += sm[q + h][el];
+        __syncthreads();
+    }
+    if (q == 0 && live) {
+        const double v = sm[0][el];
+        G16[(size_t)gj * p.n16 + gi] = v;
+        G16[(size_t)gi * p.n16 + gj] = v;
+    }
+}
+
+static SyrkParams syrk_params(int64_t m, int n, int n16)
+{
+    SyrkParams p;
+    p.m = m; p.n = n; p.n16 = n16;
+    p.P = (n16 + SY_B - 1) / SY_B;
+    p.pairs = p.P * (p.P + 1) / 2;
+    int ks = num_sms() / p.pairs;
+    if (ks < 1) ks = 1;
+    const int64_t chunks = (m + SY_KC - 1) / SY_KC;
+    if (ks > chunks) ks = (int)chunks;
+    p.ksplit = ks;
+    p.rows_per_split = (chunks + ks - 1) / ks * SY_KC;
+    return p;
+}
+
+size_t syrk_partials_bytes(int n)
+{
+    const int n16 = round_up(n, 16);
+    if (n16 <= 128) return 0;
+    const int P = (n16 + SY_B - 1) / SY_B, pairs = P * (P + 1) / 2;
+    int ks = num_sms() / pairs;
+    if (ks < 1) ks = 1;
+    return (size_t)pairs * ks * SY_B * SY_B * sizeof(double);
+}
+
+int launch_syrk(int64_t m, int n, int64_t ldy, const double* Y, double* partials, int n16, double* G16, cudaStream_t s)
+{
+    SyrkParams p = syrk_params(m, n, n16);
+    p.ldy = ldy;
+    p.vec = ((uintptr_t)Y % 16 == 0) && (ldy % 2 == 0);
+    const int smem = 2 * 2 * SY_B * SY_LD * (int)sizeof(double);
+    cudaFuncSetAttribute(mrcqr_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    mrcqr_syrk<<<p.pairs * p.ksplit, SY_THREADS, smem, s>>>(p, Y, partials);
+    mrcqr_syrk_reduce<<<p.pairs * (SY_B * SY_B / 32), 1024, 0, s>>>(p, partials, G16);
+    return 2;
+}
+
+} // namespace mrcqr

@@ -68,8 +68,12 @@ int launch_k3_gram(int64_t m, int n, int64_t lda, const double* A, const double*
 int launch_reduce_partials(const double* partials, int n_partials, int n, int n16, double* G16, cudaStream_t s);
 int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double* Rc, double* RcPrep,
                        const double* Rs, double* R, Status* st, cudaStream_t s);   // Rs, R nullable: R = Rc Rs
+// mode 3: Q = (A Rs^-1) Rc^-1; mode 1: Q = A Rs^-1 (store-Y); mode 2: Q = A Rc^-1 (A = the stored Y, may alias Q)
 int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double* RsPrep,
-                    const double* RcPrep, int64_t ldq, double* Q, double* Ydump, cudaStream_t s);
+                    const double* RcPrep, int64_t ldq, double* Q, double* Ydump, int mode, cudaStream_t s);
+// G = Y^T Y of a stored m x n Y (n16 > 128): DMMA SYRK over 128 x 128 blocks with a deterministic split of the rows
+size_t syrk_partials_bytes(int n);
+int launch_syrk(int64_t m, int n, int64_t ldy, const double* Y, double* partials, int n16, double* G16, cudaStream_t s);
 int launch_triu_mul(const double* Rc, const double* Rs, int n, double* R, cudaStream_t s);
 // RsPrep nullable: when given, the kernel also writes the prepared Rs and reports a singular diagonal
 int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* Rs, double* RsPrep, int n16,
