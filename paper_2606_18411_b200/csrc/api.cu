@@ -353,8 +353,10 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
         k += upload_diag(RsPrep, n16, 0, st);
         if (tm) cudaEventRecord(g.ev[3], st);
         const bool store_y = n16 > 128;          // Gram of a stored Y (k3_syrk.cu): Y = A Rs^-1 lives in the Q buffer
+        const bool panels = store_y && panel_pass_usable(m, n, A, lda, Q, ldq);
         if (store_y) {
-            k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 1, st);
+            if (panels) k += launch_panel_solve(m, n, 0, A, lda, RsPrep, Q, ldq, st);
+            else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 1, st);
             if (tm) cudaEventRecord(g.ev[4], st);
             k += launch_syrk(m, n, ldq, Q, part, n16, G16, st);
         } else {
@@ -365,7 +367,8 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
         k += launch_k4_cholesky(G16, n, n16, nullptr, Rc, RcPrep, Rs, R, stat, st);     // + step 9: R = Rc Rs
         k += upload_diag(RcPrep, n16, 1, st);
         if (tm) cudaEventRecord(g.ev[5], st);
-        if (store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);   // q = y Rc^-1 in place
+        if (panels) k += launch_panel_solve(m, n, 1, Q, ldq, RcPrep, Q, ldq, st);                // q = y Rc^-1 in place
+        else if (store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);
         else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 3, st);        // Alg.1 step 3
         if (tm) { cudaEventRecord(g.ev[6], st); cudaEventRecord(g.ev[7], st); }
     }

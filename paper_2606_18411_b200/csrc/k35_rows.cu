@@ -288,6 +288,72 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
     }
 }
 
+// ---- panel passes (n16 > 128, store-Y form) -------------------------------------------------------------
+// One launch solves ONE panel of PB <= 8 column blocks for all rows: every warp streams 32-row slabs
+// (RG = 4), keeps the panel in accumulator registers, adds the contributions of the already solved
+// panels with a left-looking sweep whose A fragments come straight from global memory (lane (g, t)
+// reads row g of column t: 64 contiguous bytes per column, every sector fully used; one step
+// prefetched ahead), then runs the same in-register panel_core as K3 / K5 and stores the solved panel.
+// Shared memory holds only the panel (18 KB per warp), so 10 warps per SM fit at any n; the row is
+// never resident as a whole, which is what limited the in-place slab solve to 8-row groups beyond n = 128.
+template <int FAC, int PB>
+__global__ void __launch_bounds__(320, 1)
+mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, int64_t ld_own,
+                 const double* __restrict__ Yprev, int64_t ldy, const double2* __restrict__ frag,
+                 double* __restrict__ dst, int64_t ldd, int64_t nslabs)
+{
+    extern __shared__ __align__(16) double Ysm[];
+    constexpr int RG = 4, SR = 32, LDS_ = SR + 4;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    double* slab = Ysm + (size_t)warp * (8 * PB) * LDS_;
+    zero_pad_columns<SR>(slab, ncols, 8 * PB, lane);
+    double* yw = slab + t * LDS_ + g;
+    const int64_t stride = (int64_t)gridDim.x * nw;
+    for (int64_t i = (int64_t)blockIdx.x * nw + warp; i < nslabs; i += stride) {
+        const int64_t row0 = i * SR;
+        __syncwarp();
+        load_slab<SR, true>(slab, own, ld_own, m, ncols, row0, lane);
+        // first A fragments of the left-looking sweep are requested while the panel arrives
+        const double* yp = Yprev + (size_t)t * (size_t)ldy + row0 + g;
+        double a0[RG], a1[RG];
+        if (P0 > 0) {
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) { a0[rg] = yp[8 * rg]; a1[rg] = yp[(size_t)4 * ldy + 8 * rg]; }
+        }
+        cp_async_wait_all();
+        __syncwarp();
+        double acc[RG][PB][2];
+#pragma unroll
+        for (int J = 0; J < PB; ++J)
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) {
+                acc[rg][J][0] = yw[(8 * J) * LDS_ + 8 * rg];
+                acc[rg][J][1] = yw[(8 * J + 4) * LDS_ + 8 * rg];
+            }
+        for (int Kg = 0; Kg < P0; ++Kg) {
+            double n0[RG], n1[RG];
+            const int Kn = (Kg + 1 < P0) ? Kg + 1 : Kg;
+            const double* yn = yp + (size_t)(8 * Kn) * (size_t)ldy;
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) { n0[rg] = yn[8 * rg]; n1[rg] = yn[(size_t)4 * ldy + 8 * rg]; }
+#pragma unroll
+            for (int J = 0; J < PB; ++J) {
+                const double2 b = __ldg(fragpair(frag, Kg, P0 + J, lane));
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a0[rg], b.x);
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a1[rg], b.y);
+            }
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) { a0[rg] = n0[rg]; a1[rg] = n1[rg]; }
+        }
+        panel_core<RG, FAC, PB>(acc, SlabXpose<RG>(slab - (size_t)(8 * P0) * LDS_, lane), frag, P0, lane, NoSink());
+        __syncwarp();
+        store_slab<SR, true>(slab, dst, ldd, m, ncols, row0, lane);
+    }
+}
+
 // G16[i,j] (i <= j) = sum over the CTA partials in a FIXED order (deterministic split-m reduction):
 // thread (element, q) adds the partials q, q+32, q+64, ... in ascending order; the 32 per-thread sums of
 // an element are combined by a fixed binary tree in shared memory.  32 elements x 32 lanes per CTA;
@@ -414,6 +480,43 @@ int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double
 #undef K5_CALL
 #undef K5_GO
     return 1;
+}
+
+// Y (or Q) <- solve of all panels with factor `fac` (0: Rs, source A; 1: Rc, source = dst in place).
+// Requires 16-byte aligned operands and m % 32 == 0 (the caller falls back to the slab kernel otherwise).
+bool panel_pass_usable(int64_t m, int n, const double* src, int64_t lds, const double* dstp, int64_t ldd)
+{
+    return round_up(n, 16) > 128 && (m % 32 == 0) && vec_ok(src, lds) && vec_ok(dstp, ldd);
+}
+
+int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds, const double* prep,
+                       double* dstp, int64_t ldd, cudaStream_t s)
+{
+    const int n16 = round_up(n, 16), nB = n16 >> 3;
+    const double2* frag = reinterpret_cast<const double2*>(prep);
+    const int64_t nslabs = m / 32;
+    const int nw = 10;
+    int64_t grid = (nslabs + nw - 1) / nw;
+    if (grid > num_sms()) grid = num_sms();
+    int launches = 0;
+    for (int P0 = 0; P0 < nB; P0 += 8) {
+        const int pb = (nB - P0 >= 8) ? 8 : nB - P0;
+        int ncols = n - 8 * P0;
+        if (ncols > 8 * pb) ncols = 8 * pb;
+        const int smem = nw * (8 * pb) * 36 * 8;
+        const double* own = src + (size_t)(8 * P0) * (size_t)lds;
+        double* out = dstp + (size_t)(8 * P0) * (size_t)ldd;
+#define PP_GO(FAC_, PB_)                                                                            \
+        { auto k = mrcqr_panel_pass<FAC_, PB_>;                                                     \
+          cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);               \
+          k<<<(int)grid, nw * 32, smem, s>>>(m, ncols, P0, own, lds, dstp, ldd, frag, out, ldd, nslabs); }
+#define PP_CALL(PB_) { if (fac == 0) PP_GO(0, PB_) else PP_GO(1, PB_) }
+        if (pb == 8) PP_CALL(8) else if (pb == 6) PP_CALL(6) else if (pb == 4) PP_CALL(4) else PP_CALL(2)
+#undef PP_CALL
+#undef PP_GO
+        ++launches;
+    }
+    return launches;
 }
 
 int launch_reduce_partials(const double* partials, int n_partials, int n, int n16, double* G16, cudaStream_t s)

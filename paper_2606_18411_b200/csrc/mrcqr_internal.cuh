@@ -71,6 +71,10 @@ int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double*
 // mode 3: Q = (A Rs^-1) Rc^-1; mode 1: Q = A Rs^-1 (store-Y); mode 2: Q = A Rc^-1 (A = the stored Y, may alias Q)
 int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double* RsPrep,
                     const double* RcPrep, int64_t ldq, double* Q, double* Ydump, int mode, cudaStream_t s);
+// panel passes of the store-Y form (n16 > 128): dst <- src * R^-1 one 64-column panel per launch
+bool panel_pass_usable(int64_t m, int n, const double* src, int64_t lds, const double* dst, int64_t ldd);
+int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds, const double* prep,
+                       double* dst, int64_t ldd, cudaStream_t s);
 // G = Y^T Y of a stored m x n Y (n16 > 128): DMMA SYRK over 128 x 128 blocks with a deterministic split of the rows
 size_t syrk_partials_bytes(int n);
 int launch_syrk(int64_t m, int n, int64_t ldy, const double* Y, double* partials, int n16, double* G16, cudaStream_t s);
