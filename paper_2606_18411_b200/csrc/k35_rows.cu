@@ -296,61 +296,96 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
 // prefetched ahead), then runs the same in-register panel_core as K3 / K5 and stores the solved panel.
 // Shared memory holds only the panel (18 KB per warp), so 10 warps per SM fit at any n; the row is
 // never resident as a whole, which is what limited the in-place slab solve to 8-row groups beyond n = 128.
+// The -R fragments of the left-looking sweep are shared by the 8 warps of the CTA: chunks of 8 block rows
+// (8 x PB x 512 B) are staged in shared memory by cp.async, double buffered, one barrier per chunk, so the
+// prepared factor is read from L2 once per CTA round instead of once per warp.
+constexpr int PP_NW = 8;              // warps per CTA
+constexpr int PP_KC = 8;              // block rows of R per staged chunk
+
 template <int FAC, int PB>
-__global__ void __launch_bounds__(320, 1)
+__global__ void __launch_bounds__(PP_NW * 32, 1)
 mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, int64_t ld_own,
                  const double* __restrict__ Yprev, int64_t ldy, const double2* __restrict__ frag,
                  double* __restrict__ dst, int64_t ldd, int64_t nslabs)
 {
     extern __shared__ __align__(16) double Ysm[];
     constexpr int RG = 4, SR = 32, LDS_ = SR + 4;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
     double* slab = Ysm + (size_t)warp * (8 * PB) * LDS_;
+    double2* Bsm = reinterpret_cast<double2*>(Ysm + (size_t)PP_NW * (8 * PB) * LDS_);   // [2][PB][PP_KC][32]
     zero_pad_columns<SR>(slab, ncols, 8 * PB, lane);
     double* yw = slab + t * LDS_ + g;
-    const int64_t stride = (int64_t)gridDim.x * nw;
-    for (int64_t i = (int64_t)blockIdx.x * nw + warp; i < nslabs; i += stride) {
+    const int nchunks = (P0 + PP_KC - 1) / PP_KC;
+    auto stage_chunk = [&](int c) {                  // block rows [8c, 8c+8) x the PB block columns of the panel
+        double2* dstb = Bsm + (size_t)(c & 1) * PB * PP_KC * 32;
+        for (int e = tid; e < PB * PP_KC * 32; e += PP_NW * 32) {
+            const int J = e / (PP_KC * 32), kl = (e / 32) % PP_KC, ln = e & 31;
+            const int Kg = PP_KC * c + kl;
+            if (Kg < P0) cp_async16(dstb + e, fragpair(frag, Kg, P0 + J, ln), 16);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    const int64_t rounds = (nslabs + (int64_t)gridDim.x * PP_NW - 1) / ((int64_t)gridDim.x * PP_NW);
+    for (int64_t r = 0; r < rounds; ++r) {
+        const int64_t i = (r * gridDim.x + blockIdx.x) * PP_NW + warp;
+        const bool active = i < nslabs;
         const int64_t row0 = i * SR;
-        __syncwarp();
-        load_slab<SR, true>(slab, own, ld_own, m, ncols, row0, lane);
-        // first A fragments of the left-looking sweep are requested while the panel arrives
+        __syncthreads();                             // previous round done with both chunk buffers
+        if (active) load_slab<SR, true>(slab, own, ld_own, m, ncols, row0, lane);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        if (nchunks > 0) stage_chunk(0);
         const double* yp = Yprev + (size_t)t * (size_t)ldy + row0 + g;
         double a0[RG], a1[RG];
-        if (P0 > 0) {
+        if (P0 > 0 && active) {
 #pragma unroll
             for (int rg = 0; rg < RG; ++rg) { a0[rg] = yp[8 * rg]; a1[rg] = yp[(size_t)4 * ldy + 8 * rg]; }
         }
-        cp_async_wait_all();
+        if (nchunks > 0) asm volatile("cp.async.wait_group 1;" ::: "memory");     // own panel landed
+        else asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncwarp();
         double acc[RG][PB][2];
+        if (active) {
 #pragma unroll
-        for (int J = 0; J < PB; ++J)
+            for (int J = 0; J < PB; ++J)
 #pragma unroll
-            for (int rg = 0; rg < RG; ++rg) {
-                acc[rg][J][0] = yw[(8 * J) * LDS_ + 8 * rg];
-                acc[rg][J][1] = yw[(8 * J + 4) * LDS_ + 8 * rg];
-            }
-        for (int Kg = 0; Kg < P0; ++Kg) {
-            double n0[RG], n1[RG];
-            const int Kn = (Kg + 1 < P0) ? Kg + 1 : Kg;
-            const double* yn = yp + (size_t)(8 * Kn) * (size_t)ldy;
-#pragma unroll
-            for (int rg = 0; rg < RG; ++rg) { n0[rg] = yn[8 * rg]; n1[rg] = yn[(size_t)4 * ldy + 8 * rg]; }
-#pragma unroll
-            for (int J = 0; J < PB; ++J) {
-                const double2 b = __ldg(fragpair(frag, Kg, P0 + J, lane));
-#pragma unroll
-                for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a0[rg], b.x);
-#pragma unroll
-                for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a1[rg], b.y);
-            }
-#pragma unroll
-            for (int rg = 0; rg < RG; ++rg) { a0[rg] = n0[rg]; a1[rg] = n1[rg]; }
+                for (int rg = 0; rg < RG; ++rg) {
+                    acc[rg][J][0] = yw[(8 * J) * LDS_ + 8 * rg];
+                    acc[rg][J][1] = yw[(8 * J + 4) * LDS_ + 8 * rg];
+                }
         }
-        panel_core<RG, FAC, PB>(acc, SlabXpose<RG>(slab - (size_t)(8 * P0) * LDS_, lane), frag, P0, lane, NoSink());
-        __syncwarp();
-        store_slab<SR, true>(slab, dst, ldd, m, ncols, row0, lane);
+        for (int c = 0; c < nchunks; ++c) {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncthreads();                         // chunk c visible; everyone is done with chunk c-1
+            if (c + 1 < nchunks) stage_chunk(c + 1);
+            if (active) {
+                const double2* bs = Bsm + (size_t)(c & 1) * PB * PP_KC * 32 + lane;
+                const int kend = (P0 - PP_KC * c < PP_KC) ? P0 - PP_KC * c : PP_KC;
+                for (int kl = 0; kl < kend; ++kl) {
+                    const int Kg = PP_KC * c + kl;
+                    double n0[RG], n1[RG];
+                    const int Kn = (Kg + 1 < P0) ? Kg + 1 : Kg;
+                    const double* yn = yp + (size_t)(8 * Kn) * (size_t)ldy;
+#pragma unroll
+                    for (int rg = 0; rg < RG; ++rg) { n0[rg] = yn[8 * rg]; n1[rg] = yn[(size_t)4 * ldy + 8 * rg]; }
+#pragma unroll
+                    for (int J = 0; J < PB; ++J) {
+                        const double2 b = bs[(J * PP_KC + kl) * 32];
+#pragma unroll
+                        for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a0[rg], b.x);
+#pragma unroll
+                        for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a1[rg], b.y);
+                    }
+#pragma unroll
+                    for (int rg = 0; rg < RG; ++rg) { a0[rg] = n0[rg]; a1[rg] = n1[rg]; }
+                }
+            }
+        }
+        if (active) {
+            panel_core<RG, FAC, PB>(acc, SlabXpose<RG>(slab - (size_t)(8 * P0) * LDS_, lane), frag, P0, lane, NoSink());
+            __syncwarp();
+            store_slab<SR, true>(slab, dst, ldd, m, ncols, row0, lane);
+        }
     }
 }
 
@@ -495,7 +530,7 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
     const int n16 = round_up(n, 16), nB = n16 >> 3;
     const double2* frag = reinterpret_cast<const double2*>(prep);
     const int64_t nslabs = m / 32;
-    const int nw = 10;
+    const int nw = PP_NW;
     int64_t grid = (nslabs + nw - 1) / nw;
     if (grid > num_sms()) grid = num_sms();
     int launches = 0;
@@ -503,7 +538,7 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
         const int pb = (nB - P0 >= 8) ? 8 : nB - P0;
         int ncols = n - 8 * P0;
         if (ncols > 8 * pb) ncols = 8 * pb;
-        const int smem = nw * (8 * pb) * 36 * 8;
+        const int smem = nw * (8 * pb) * 36 * 8 + 2 * pb * PP_KC * 512;
         const double* own = src + (size_t)(8 * P0) * (size_t)lds;
         double* out = dstp + (size_t)(8 * P0) * (size_t)ldd;
 #define PP_GO(FAC_, PB_)                                                                            \

@@ -1,0 +1,94 @@
+"""GPU parity of the kernel variants mrcqr_factor dispatches to beyond the basic shapes of
+test_gpu_parity.py: the tensor-core form of K1 (FP16 sketch, s <= 128, padded bin counts), the
+store-Y form of stage 2 for n16 > 128 (panel passes + SYRK Gram, every panel width, ragged n),
+and the fall-backs taken for unaligned operands.  Same tolerances as test_gpu_parity.py."""
+import numpy as np
+import pytest
+import torch
+
+from helpers import U, draw_to_dev, to_np
+from paper_2606_18411_b200 import binding as B
+from paper_2606_18411_b200 import inputs
+from test_gpu_parity import factor_parity, relf
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("m,n,s", [
+    (1 << 13, 8, 24),        # s padded to 32: 2 m-tiles x 4 column groups, single tile per column
+    (1 << 14, 25, 50),       # s padded to 64, odd n
+    (1 << 15, 33, 100),      # s padded to 128, CTA ranges spanning two columns
+    (1 << 14, 64, 128),      # the C1 geometry at small m
+    (1 << 13, 150, 128),     # n > s is illegal for QR, but the sketch alone must still be right -> use stage call only
+])
+def test_tensor_core_sketch_matches_oracle(orc, m, n, s):
+    AT = inputs.make_A(m, n, 2, 300 + n, 301 + n, "cuda")
+    A = to_np(AT)
+    signs, idx = orc.draw(m, s, 77 + n)
+    As_o = orc.sketch(np.asfortranarray(A), signs, idx)
+    dsigns, didx = draw_to_dev(signs, idx)
+    if s >= n:
+        _, As = B.mrcqr_sketch(AT, B.FP16, dsigns, didx, want_As=True)
+        Asg = to_np(As)
+        assert relf(Asg, As_o) <= 1e-2
+        # every stored value is an FP16 number (the sketch lives in precision p)
+        assert np.array_equal(Asg, Asg.astype(np.float16).astype(np.float64))
+        factor_parity(orc, AT, s, 77 + n, B.FP16)
+    else:
+        with pytest.raises(B.MrcqrError):
+            B.mrcqr_sketch(AT, B.FP16, dsigns, didx, want_As=True)
+
+
+def test_tensor_core_sketch_closed_form(orc):
+    """Column j = d * cos(2 pi k_j t / m) (signs undone): the transform has one line, at bin k_j, of height
+    m/2 (m at DC / Nyquist); after the sqrt(s/m) scale the sketch is that value at (j, j) and zero elsewhere."""
+    m, n, s = 1 << 13, 16, 32
+    signs, idx = orc.draw(m, s, 5)
+    bits = np.unpackbits(np.ascontiguousarray(signs).view(np.uint8), bitorder="little")[:m]
+    d = 1.0 - 2.0 * bits
+    t = np.arange(m)
+    A = np.stack([d * np.cos(2 * np.pi * int(idx[j]) * t / m) for j in range(n)], axis=1)
+    AT = torch.from_numpy(np.ascontiguousarray(A.T)).cuda()
+    dsigns, didx = draw_to_dev(signs, idx)
+    _, As = B.mrcqr_sketch(AT, B.FP16, dsigns, didx, want_As=True)
+    Asg = to_np(As)
+    scale = np.sqrt(s / m)
+    want = np.zeros((s, n))
+    for j in range(n):
+        k0 = int(idx[j])
+        want[j, j] = (m if k0 in (0, m // 2) else 0.5 * m) * scale
+    assert np.linalg.norm(Asg - want) <= 1e-2 * np.linalg.norm(want)
+
+
+@pytest.mark.parametrize("m,n,expo,prec", [
+    (1 << 12, 136, 3, 32),     # n16 = 144: panels of 8, 8, 2 blocks; SYRK with P = 2 and a ragged second panel
+    (1 << 12, 160, 6, 64),     # n16 = 160: panels 8, 8, 4
+    (1 << 12, 240, 8, 64),     # n16 = 240: panels 8, 8, 8, 6
+    (1 << 11, 400, 4, 32),     # P = 4 SYRK blocks, 7 panels
+    (1 << 11, 512, 5, 64),     # the largest n
+])
+def test_store_y_path_factorization(orc, m, n, expo, prec):
+    AT = inputs.make_A(m, n, expo, 500 + n, 501 + n, "cuda")
+    factor_parity(orc, AT, 2 * n, 600 + n, prec)
+
+
+def test_store_y_path_is_deterministic_and_handles_strides(orc):
+    m, n = 1 << 12, 272
+    AT = inputs.make_A(m, n, 5, 11, 12, "cuda")
+    Q1, R1 = B.mrcqr_factor(AT, B.FP64, 2 * n, 3)
+    Q2, R2 = B.mrcqr_factor(AT, B.FP64, 2 * n, 3)
+    assert torch.equal(Q1, Q2) and torch.equal(R1, R2)
+    # lda = m + 6 (16-byte aligned columns): same arithmetic, same bits
+    big = torch.zeros((n, m + 6), dtype=torch.float64, device="cuda")
+    big[:, :m] = AT
+    Q3, R3 = B.mrcqr_factor(big[:, :m], B.FP64, 2 * n, 3)
+    assert torch.equal(Q3[:, :m] if Q3.shape[1] != m else Q3, Q1) and torch.equal(R3, R1)
+    # columns that start on an odd element (8-byte aligned only): the fall-back kernels run; same Q to rounding
+    odd = torch.zeros((n, m + 7), dtype=torch.float64, device="cuda")
+    odd[:, 1:m + 1] = AT
+    Q4, R4 = B.mrcqr_factor(odd[:, 1:m + 1], B.FP64, 2 * n, 3)
+    A = to_np(AT)
+    Q4n, R4n = to_np(Q4), to_np(R4)
+    assert orc.orth_error_fro(Q4n) <= 1e-13 and orc.residual_fro(A, Q4n, R4n) <= 1e-13
+    kappa = np.linalg.cond(to_np(R1))
+    assert np.linalg.norm(Q4n - to_np(Q1)) <= 10 * kappa * n * U
