@@ -23,6 +23,7 @@
 namespace mrcqr {
 
 constexpr int K1_W = 32;          // t2 values per tile = lanes of a warp
+constexpr int K1_LD = 33;         // row stride of the tile in complex elements (odd: the per-bin gathers of stage 2 spread over the banks)
 constexpr int K1_NT = 256;
 constexpr int K1_NWARP = K1_NT / 32;
 
@@ -69,7 +70,7 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
 {
     extern __shared__ __align__(16) unsigned char smraw[];
     Cx<T>* tile = reinterpret_cast<Cx<T>*>(smraw);                       // [m1][32]
-    Cx<T>* tw = tile + (size_t)p.m1 * K1_W;                              // [m1]  W_m1^e
+    Cx<T>* tw = tile + (size_t)p.m1 * K1_LD;                             // [m1]  W_m1^e
     double* colacc = reinterpret_cast<double*>(tw + p.m1);               // [2][s]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int pair = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
@@ -116,7 +117,7 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
                     if (t1 < m1) {
                         Cx<T> e0{diag_cast<T, PREC>(va[u].x, sg[u] & 1u), diag_cast<T, PREC>(vb[u].x, sg[u] & 1u)};
                         Cx<T> e1{diag_cast<T, PREC>(va[u].y, (sg[u] >> 1) & 1u), diag_cast<T, PREC>(vb[u].y, (sg[u] >> 1) & 1u)};
-                        Cx<T>* dst = tile + (size_t)t1 * K1_W + 2 * pr;
+                        Cx<T>* dst = tile + (size_t)t1 * K1_LD + 2 * pr;
                         dst[0] = e0; dst[1] = e1;
                     }
                 }
@@ -131,7 +132,7 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
                 const unsigned neg = (signs32[(off + t2_0) >> 5] >> lane) & 1u;
                 const double a = __ldcs(colA + off);
                 const double b = has_b ? __ldcs(colB + off) : 0.0;
-                tile[t1 * K1_W + lane] = Cx<T>{diag_cast<T, PREC>(a, neg), diag_cast<T, PREC>(b, neg)};
+                tile[t1 * K1_LD + lane] = Cx<T>{diag_cast<T, PREC>(a, neg), diag_cast<T, PREC>(b, neg)};
             }
         }
         __syncthreads();
@@ -141,53 +142,59 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
             const int q = nb >> 2, tstride = m1 / nb;
             for (int bf = warp; bf < (m1 >> 2); bf += K1_NWARP) {
                 const int blk = bf / q, pos = bf % q;
-                Cx<T>* base = tile + ((size_t)blk * nb + pos) * K1_W + lane;
-                Cx<T> a0 = base[0], a1 = base[(size_t)q * K1_W], a2 = base[(size_t)2 * q * K1_W], a3 = base[(size_t)3 * q * K1_W];
+                Cx<T>* base = tile + ((size_t)blk * nb + pos) * K1_LD + lane;
+                Cx<T> a0 = base[0], a1 = base[(size_t)q * K1_LD], a2 = base[(size_t)2 * q * K1_LD], a3 = base[(size_t)3 * q * K1_LD];
                 const Cx<T> w1 = tw[pos * tstride], w2 = tw[2 * pos * tstride];
                 Cx<T> b0 = cadd(a0, a2), b2 = cmul(csub(a0, a2), w1);
                 Cx<T> b1 = cadd(a1, a3), b3 = cmulmi(cmul(csub(a1, a3), w1));
                 base[0] = cadd(b0, b1);
-                base[(size_t)q * K1_W] = cmul(csub(b0, b1), w2);
-                base[(size_t)2 * q * K1_W] = cadd(b2, b3);
-                base[(size_t)3 * q * K1_W] = cmul(csub(b2, b3), w2);
+                base[(size_t)q * K1_LD] = cmul(csub(b0, b1), w2);
+                base[(size_t)2 * q * K1_LD] = cadd(b2, b3);
+                base[(size_t)3 * q * K1_LD] = cmul(csub(b2, b3), w2);
             }
             nb >>= 2;
             __syncthreads();
         }
         if (nb == 2) {                                 // odd log2(m1): final radix-2 pass, twiddle 1
             for (int bf = warp; bf < (m1 >> 1); bf += K1_NWARP) {
-                Cx<T>* base = tile + (size_t)(2 * bf) * K1_W + lane;
-                Cx<T> a0 = base[0], a1 = base[K1_W];
+                Cx<T>* base = tile + (size_t)(2 * bf) * K1_LD + lane;
+                Cx<T> a0 = base[0], a1 = base[K1_LD];
                 base[0] = cadd(a0, a1);
-                base[K1_W] = csub(a0, a1);
+                base[K1_LD] = csub(a0, a1);
             }
             __syncthreads();
         }
-        // ---- stage 2: sampled bins ------------------------------------------------------------------
-        const int64_t t2 = t2_0 + lane;
-        for (int i = warp; i < p.s; i += K1_NWARP) {
+        // ---- stage 2: sampled bins.  Thread (bin i) walks the 32 t2 values of the tile with the twiddle
+        //      recurrence w <- w * W_m^k, re-seeded every 8 steps from w0 * (W_m^{8k})^j (a few ulp in T);
+        //      one sincospi per bin and tile; no shuffles: a bin's partial sum belongs to one thread.
+        for (int i = tid; i < p.s; i += K1_NT) {
             const int64_t k = idx[i];
             const int k1 = (int)(k & (m1 - 1));
             const int k1n = (m1 - k1) & (m1 - 1);
             const int br = p.log_m1 ? (int)(__brev((unsigned)k1) >> (32 - p.log_m1)) : 0;
             const int brn = p.log_m1 ? (int)(__brev((unsigned)k1n) >> (32 - p.log_m1)) : 0;
-            const Cx<T> P = tile[br * K1_W + lane];
-            const Cx<T> Qn = tile[brn * K1_W + lane];
-            // Z_a = (P + conj Qn)/2, Z_b = -i (P - conj Qn)/2
-            const T zar = (T)0.5 * (P.x + Qn.x), zai = (T)0.5 * (P.y - Qn.y);
-            const T zbr = (T)0.5 * (P.y + Qn.y), zbi = (T)0.5 * (Qn.x - P.x);
-            const int64_t r = (k * t2) & (p.m - 1);    // k t2 mod m, exact
-            T sn, cs;
-            sincospi_t((T)(2.0 * (double)r / (double)p.m), &sn, &cs);
-            // Re( e^{-i theta} Z ) = cos*Zr + sin*Zi
-            double va = (double)fma(cs, zar, sn * zai);
-            double vb = (double)fma(cs, zbr, sn * zbi);
+            const Cx<T>* rowP = tile + (size_t)br * K1_LD;
+            const Cx<T>* rowQ = tile + (size_t)brn * K1_LD;
+            Cx<T> w0, d1, d8;                                  // (cos, sin) of 2 pi k t2_0 / m, 2 pi k / m, 2 pi 8k / m
+            sincospi_t((T)(2.0 * (double)((k * t2_0) & (p.m - 1)) / (double)p.m), &w0.y, &w0.x);
+            sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d1.y, &d1.x);
+            sincospi_t((T)(2.0 * (double)((8 * k) & (p.m - 1)) / (double)p.m), &d8.y, &d8.x);
+            T va = (T)0, vb = (T)0;
+#pragma unroll 1
+            for (int j8 = 0; j8 < K1_W; j8 += 8) {
+                Cx<T> w = w0;
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                va += __shfl_xor_sync(0xffffffffu, va, o);
-                vb += __shfl_xor_sync(0xffffffffu, vb, o);
+                for (int u = 0; u < 8; ++u) {
+                    const Cx<T> P = rowP[j8 + u], Qn = rowQ[j8 + u];
+                    // 2 Z_a = P + conj Qn, 2 Z_b = -i (P - conj Qn);  Re(e^{-i th} Z) = cos*Zr + sin*Zi
+                    va = fma(w.x, P.x + Qn.x, va); va = fma(w.y, P.y - Qn.y, va);
+                    vb = fma(w.x, P.y + Qn.y, vb); vb = fma(w.y, Qn.x - P.x, vb);
+                    w = cmul(w, d1);
+                }
+                w0 = cmul(w0, d8);
             }
-            if (lane == 0) { colacc[i] += va; colacc[p.s + i] += vb; }
+            colacc[i] += 0.5 * (double)va;
+            colacc[p.s + i] += 0.5 * (double)vb;
         }
     }
     __syncthreads();
@@ -244,7 +251,7 @@ template <typename T, int PREC>
 static void k1_launch_t(const K1Params& p, const double* A, const uint64_t* signs, const int64_t* idx,
                         double* partial, double* As, Status* st, cudaStream_t stream)
 {
-    const size_t smem = (size_t)p.m1 * K1_W * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + 2 * (size_t)p.s * sizeof(double);
+    const size_t smem = (size_t)p.m1 * K1_LD * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + 2 * (size_t)p.s * sizeof(double);
     auto k = mrcqr_k1_srtt<T, PREC>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int grid = ((p.n + 1) / 2) * p.chunks;
