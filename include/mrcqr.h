@@ -129,6 +129,15 @@ int mrcqr_set_timing(int on);
 int mrcqr_last_timing(float* ms_out_host);
 
 /*
+ * Variant switch of mrcqr_factor / mrcqr_factor_host ("store-Y"): off (default), stage 2a
+ * keeps Y = A R_s^-1 on chip and stage 2b recomputes it bit-identically (4 passes over m x n, 4 m n^2 flops);
+ * on, stage 2a also writes Y into Q's buffer and stage 2b solves it in place against R_c (5 passes,
+ * 3 m n^2 flops: the paper's own TrsmPre / TrsmFin order).  For n > 128 Y is always
+ * stored (the Gram matrix no longer fits one SM).  Returns 0.
+ */
+int mrcqr_set_store_y(int on);
+
+/*
  * Test hook for the "bit-identical Y" requirement: runs the stage-2a and the stage-2b
  * tile solves and dumps the Y = A R_s^-1 each of them computed (m x n, ld = m).  The two dumps
  * must be equal bit for bit.

@@ -49,10 +49,11 @@ def lib():
         L.mrcqr_debug_dump_y.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
         L.mrcqr_shutdown.restype = None
         L.mrcqr_set_timing.argtypes = [ci]
+        L.mrcqr_set_store_y.argtypes = [ci]
         L.mrcqr_last_timing.argtypes = [vp]
         for f in ("mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
                   "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
-                  "mrcqr_set_timing", "mrcqr_last_timing"):
+                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y"):
             getattr(L, f).restype = ci
         _lib = L
     return _lib
@@ -60,7 +61,7 @@ def lib():
 
 EXPORTS = ["mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
-           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing"]
+           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y"]
 
 STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "reduce_k4_chol", "k5_form_q", "r_mul"]
 
@@ -178,6 +179,11 @@ def mrcqr_last_launch_count():
 
 def mrcqr_shutdown():
     lib().mrcqr_shutdown()
+
+
+def mrcqr_set_store_y(on):
+    """Store-Y variant of stage 2 also for n <= 128 (default off: Y stays on chip and is recomputed)."""
+    lib().mrcqr_set_store_y(1 if on else 0)
 
 
 def mrcqr_set_timing(on):

@@ -76,6 +76,7 @@ struct Ctx {
     int last_info = 0, last_launches = 0;
     bool timing = false; cudaEvent_t ev[8] = {}; bool ev_ok = false; float stage_ms[8] = {};
     bool have_device = false, probed = false;
+    bool store_y = false;                    // mrcqr_set_store_y: store-Y variant also for n16 <= 128
 };
 static Ctx g;
 
@@ -149,7 +150,7 @@ static int enqueue_gram(const Layout& L, int64_t m, int n, int64_t lda, const do
     int np = 0;
     int k = launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st);
     k += upload_diag(RsPrep, n16, 0, st);
-    k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, Ydump, st);
+    k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, Ydump, nullptr, 0, st);
     k += launch_reduce_partials(part, np, n, n16, G16, st);
     k += launch_k4_cholesky(G16, n, n16, G_out, Rc, RcPrep, nullptr, nullptr, stat, st);
     k += upload_diag(RcPrep, n16, 1, st);
@@ -312,6 +313,7 @@ static bool timing_events()
 }
 
 extern "C" int mrcqr_set_timing(int on) { g.timing = (on != 0); return 0; }
+extern "C" int mrcqr_set_store_y(int on) { g.store_y = (on != 0); return 0; }
 
 extern "C" int mrcqr_last_timing(float* ms_out_host)
 {
@@ -360,7 +362,7 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
             if (tm) cudaEventRecord(g.ev[4], st);
             k += launch_syrk(m, n, ldq, Q, part, n16, G16, st);
         } else {
-            k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, st);
+            k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, g.store_y ? Q : nullptr, ldq, st);
             if (tm) cudaEventRecord(g.ev[4], st);
             k += launch_reduce_partials(part, np, n, n16, G16, st);
         }
@@ -369,6 +371,7 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
         if (tm) cudaEventRecord(g.ev[5], st);
         if (panels) k += launch_panel_solve(m, n, 1, Q, ldq, RcPrep, Q, ldq, st);                // q = y Rc^-1 in place
         else if (store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);
+        else if (g.store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);  // variant: stored Y
         else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 3, st);        // Alg.1 step 3
         if (tm) { cudaEventRecord(g.ev[6], st); cudaEventRecord(g.ev[7], st); }
     }

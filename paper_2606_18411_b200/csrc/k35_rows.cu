@@ -155,7 +155,7 @@ template <int RG, int NW, int NB, bool VEC>
 __global__ void __launch_bounds__(NW * 32, (RG == 4 && NW == 4) ? 3 : 1)
 mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__ A,
               const double2* __restrict__ fragS, double* __restrict__ partials,
-              int64_t ntiles, double* __restrict__ Ydump)
+              int64_t ntiles, double* __restrict__ Ydump, double* __restrict__ Ystore, int64_t ldys)
 {
     extern __shared__ __align__(16) double Ysm[];
     constexpr int SR = 8 * RG, LDS_ = SR + 4, TM = SR * NW;
@@ -183,6 +183,7 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
             __syncwarp();
             solve_slab<RG, 0, NBc>(slab, fragS, nB, lane);
             if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); }
+            if (Ystore) { __syncwarp(); store_slab<SR, VEC>(slab, Ystore, ldys, m, n, row0, lane); }   // store-Y variant
             __syncthreads();
 #define GRAM_ACC(R_) gram_accumulate<NBc, NW, R_, SR, NW, MAXOWN>(acc, Ysm, slab_stride, lane);
             MRCQR_ROLE_SWITCH(GRAM_ACC)
@@ -459,17 +460,17 @@ static int grid_for(K kernel, int threads, int smem, int64_t ntiles)
 static bool vec_ok(const void* p, int64_t ld) { return ((uintptr_t)p % 16 == 0) && (ld % 2 == 0); }
 
 int launch_k3_gram(int64_t m, int n, int64_t lda, const double* A, const double* RsPrep,
-                   double* partials, int* n_partials_out, double* Ydump, cudaStream_t s)
+                   double* partials, int* n_partials_out, double* Ydump, double* Ystore, int64_t ldys, cudaStream_t s)
 {
     RowCfg c = row_config(n);
     const int TM = 8 * c.RG * c.NW;
     const int64_t ntiles = (m + TM - 1) / TM;
-    const bool vec = vec_ok(A, lda);
+    const bool vec = vec_ok(A, lda) && (!Ystore || vec_ok(Ystore, ldys));
     const double2* frag = reinterpret_cast<const double2*>(RsPrep);
 #define K3_GO(RG_, NW_, NB_, V_)                                                                    \
     { auto k = mrcqr_k3_gram<RG_, NW_, NB_, V_>;                                                    \
       int grid = grid_for(k, NW_ * 32, c.smem_bytes, ntiles); *n_partials_out = grid;               \
-      k<<<grid, NW_ * 32, c.smem_bytes, s>>>(m, n, c.n16, lda, A, frag, partials, ntiles, Ydump); }
+      k<<<grid, NW_ * 32, c.smem_bytes, s>>>(m, n, c.n16, lda, A, frag, partials, ntiles, Ydump, Ystore, ldys); }
 #define K3_CALL(RG_, NW_, NB_) { if (vec) K3_GO(RG_, NW_, NB_, true) else K3_GO(RG_, NW_, NB_, false) }
     switch (c.n16) {
         case 16:  K3_CALL(4, 4, 2) break;   case 32:  K3_CALL(4, 4, 4) break;

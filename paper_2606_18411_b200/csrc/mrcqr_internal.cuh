@@ -63,8 +63,9 @@ __device__ __forceinline__ double prep_value(const double* R, int ldr, int n, in
 // launchers (each returns the number of kernel launches it enqueued)
 int launch_prep_R(const double* R, int n, double* Rprep, int n16, Status* st, int err_code, cudaStream_t s);
 int upload_diag(const double* prep, int n16, int fac, cudaStream_t s);      // prepared diagonal blocks -> constant memory
+// Ystore (nullable, n16 <= 128 only): also write Y = A Rs^-1 (store-Y variant)
 int launch_k3_gram(int64_t m, int n, int64_t lda, const double* A, const double* RsPrep,
-                   double* partials, int* n_partials_out, double* Ydump, cudaStream_t s);
+                   double* partials, int* n_partials_out, double* Ydump, double* Ystore, int64_t ldys, cudaStream_t s);
 int launch_reduce_partials(const double* partials, int n_partials, int n, int n16, double* G16, cudaStream_t s);
 int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double* Rc, double* RcPrep,
                        const double* Rs, double* R, Status* st, cudaStream_t s);   // Rs, R nullable: R = Rc Rs

@@ -92,3 +92,18 @@ def test_store_y_path_is_deterministic_and_handles_strides(orc):
     assert orc.orth_error_fro(Q4n) <= 1e-13 and orc.residual_fro(A, Q4n, R4n) <= 1e-13
     kappa = np.linalg.cond(to_np(R1))
     assert np.linalg.norm(Q4n - to_np(Q1)) <= 10 * kappa * n * U
+
+
+@pytest.mark.parametrize("m,n,prec", [(1 << 14, 64, 16), (1 << 13, 100, 32), (1 << 13, 20, 64)])
+def test_store_y_variant_below_128_columns(orc, m, n, prec):
+    """mrcqr_set_store_y(1): stage 2a writes Y into Q's buffer, stage 2b solves it in place.
+    Same factorization as the default (recompute) form: the stored Y is the Y the Gram matrix saw, so Q is
+    bit-identical to the default path's."""
+    AT = inputs.make_A(m, n, 4, 900 + n, 901 + n, "cuda")
+    Q0, R0 = B.mrcqr_factor(AT, prec, 2 * n, 31)
+    B.mrcqr_set_store_y(True)
+    try:
+        Q1, R1 = factor_parity(orc, AT, 2 * n, 31, prec)
+    finally:
+        B.mrcqr_set_store_y(False)
+    assert torch.equal(Q0, Q1) and torch.equal(R0, R1)
