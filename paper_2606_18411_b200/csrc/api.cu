@@ -43,7 +43,7 @@ static void draw_bins_host(int64_t m, int s, uint64_t seed, int64_t* idx)
 
 // ---- workspace -----------------------------------------------------------------------------------
 struct Layout {
-    size_t status, signs, idx, As, Rs, RsPrep, RcPrep, G16, Rc, k1, k3, total;
+    size_t status, signs, idx, As, Rs, RsPrep, RcPrep, G16, Rc, betas, k1, k3, total;
 };
 
 static size_t al(size_t x) { return (x + 255) / 256 * 256; }
@@ -62,6 +62,7 @@ static Layout make_layout(int64_t m, int n, int s, int prec)
     L.RcPrep = o; o += al(n16 * n16 * 8);
     L.G16 = o;    o += al(n16 * n16 * 8);
     L.Rc = o;     o += al((size_t)n * n * 8);
+    L.betas = o;  o += al((size_t)n * 8);
     L.k1 = o;     o += al(s > 0 ? k1_workspace_bytes(m, n, s, prec) : 0);
     L.k3 = o;     o += al(std::max(k3_partials_bytes(n), syrk_partials_bytes(n)));
     L.total = o;
@@ -134,7 +135,8 @@ static int enqueue_sketch(const Layout& L, int64_t m, int n, int64_t lda, const 
     double* As = reinterpret_cast<double*>(g.ws + L.As);
     int k = launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);
     if (As_out) cudaMemcpyAsync(As_out, As, sizeof(double) * (size_t)s * n, cudaMemcpyDeviceToDevice, st);
-    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16), stat, st);
+    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
+                             reinterpret_cast<double*>(g.ws + L.betas), stat, st);
     return k;
 }
 
@@ -343,7 +345,8 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
     if (tm) cudaEventRecord(g.ev[0], st);
     k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);     // steps 2-4
     if (tm) cudaEventRecord(g.ev[1], st);
-    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16), stat, st); // steps 5-6
+    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
+                             reinterpret_cast<double*>(g.ws + L.betas), stat, st);                              // steps 5-6
     if (tm) cudaEventRecord(g.ev[2], st);
     {                                                                                      // step 7 + Alg.1 steps 1-2
         const int n16 = round_up(n, 16);

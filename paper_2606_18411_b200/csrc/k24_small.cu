@@ -256,18 +256,6 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-// epilogue shared by both K2 variants: Rs (just written by this CTA) -> prepared Rs, singular check
-__device__ __forceinline__ void k2_prepare(const double* Rs, int n, double* RsPrep, int n16, Status* st)
-{
-    if (!RsPrep) return;
-    __syncthreads();
-    const int nB = n16 >> 3;
-    const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
-    int bad = -1;
-    for (size_t o = threadIdx.x; o < total; o += blockDim.x) RsPrep[o] = prep_value(Rs, n, n, nB, o, &bad);
-    if (bad >= 0) report(st, 2, bad);
-}
-
 __global__ void __launch_bounds__(SMALL_NT)
 mrcqr_k2_sketch_qr(double* __restrict__ As, int s, int n, int use_smem, double* __restrict__ Rs,
                    double* __restrict__ RsPrep, int n16, Status* st)
@@ -460,7 +448,7 @@ int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double*
 }
 
 int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* Rs, double* RsPrep, int n16,
-                        Status* st, cudaStream_t s)
+                        double* betas, Status* st, cudaStream_t s)
 {
     if (n <= 64 && s_rows <= 256) {
         if (n <= 32 && s_rows <= 128) mrcqr_k2_sketch_qr_reg<1, 4><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
@@ -468,6 +456,8 @@ int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* Rs, double*
         else mrcqr_k2_sketch_qr_reg<2, 8><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
         return 1;
     }
+    if (k2_blocked_usable(s_rows, n) && betas)
+        return launch_k2_blocked(const_cast<double*>(As), s_rows, n, betas, Rs, RsPrep, n16, st, s);
     size_t need = ((size_t)n + 2 + (size_t)s_rows * n) * sizeof(double);
     const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
     const size_t smem = use_smem ? need : ((size_t)n + 2) * sizeof(double);

@@ -80,9 +80,26 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
 size_t syrk_partials_bytes(int n);
 int launch_syrk(int64_t m, int n, int64_t ldy, const double* Y, double* partials, int n16, double* G16, cudaStream_t s);
 int launch_triu_mul(const double* Rc, const double* Rs, int n, double* R, cudaStream_t s);
-// RsPrep nullable: when given, the kernel also writes the prepared Rs and reports a singular diagonal
+// RsPrep nullable: when given, the kernel also writes the prepared Rs and reports a singular diagonal.
+// betas: n doubles of workspace (nullable: then the single-CTA kernels are used for every n).
+// NOTE: for n > 64 the sketch `As` is overwritten (factored in place by the blocked kernel).
 int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* Rs, double* RsPrep, int n16,
-                        Status* st, cudaStream_t s);
+                        double* betas, Status* st, cudaStream_t s);
+bool k2_blocked_usable(int s_rows, int n);
+int launch_k2_blocked(double* As, int s_rows, int n, double* betas, double* Rs, double* RsPrep, int n16,
+                      Status* st, cudaStream_t stream);
+
+// epilogue shared by the K2 kernels: Rs (just written by this CTA) -> prepared Rs, singular check
+__device__ __forceinline__ void k2_prepare(const double* Rs, int n, double* RsPrep, int n16, Status* st)
+{
+    if (!RsPrep) return;
+    __syncthreads();
+    const int nB = n16 >> 3;
+    const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
+    int bad = -1;
+    for (size_t o = threadIdx.x; o < total; o += blockDim.x) RsPrep[o] = prep_value(Rs, n, n, nB, o, &bad);
+    if (bad >= 0) report(st, 2, bad);
+}
 
 // K1: sampled transform.  Returns launches.  As (s x n, ld = s) receives precision-p values in FP64.
 size_t k1_workspace_bytes(int64_t m, int n, int s, int prec);
