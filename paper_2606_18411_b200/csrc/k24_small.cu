@@ -441,6 +441,7 @@ int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double*
 #undef K4_GO
         return 1;
     }
+    return launch_k4_coop(const_cast<double*>(G16), n, n16, G_out, Rc, RcPrep, Rs, R, st, s);
     const int threads = n16 <= 64 ? 256 : (n16 <= 128 ? 512 : SMALL_NT);
     cudaFuncSetAttribute(mrcqr_k4_cholesky, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     mrcqr_k4_cholesky<<<1, threads, smem, s>>>(const_cast<double*>(G16), n, n16, use_smem, G_out, Rc, RcPrep, Rs, R, st);

@@ -8,7 +8,7 @@
 //
 // G is cut into 128 x 128 blocks (I <= J); a CTA owns one block and one contiguous range of rows
 // (deterministic split of m), streams 32-row chunks of the two 128-column panels of Y through a
-// double-buffered shared-memory tile (cp.async) and accumulates on DMMA: 8 warps as 4 x 2, each
+// triple-buffered shared-memory tile (cp.async, one barrier per chunk) and accumulates on DMMA: 8 warps as 4 x 2, each
 // 32 x 64 of the block (4 x 8 accumulators, 12 fragment loads per 32 DMMA).  Accumulator chains are
 // flushed to the CTA's partial every 1024 rows (reading R7); a reduction kernel adds the
 // partials of a block in a fixed order.  No atomics: bit-reproducible.
@@ -46,19 +46,24 @@ __device__ __forceinline__ void sy_pair(int p, int& I, int& J)      // p -> (I <
     J = j; I = p - j * (j + 1) / 2;
 }
 
-// loads rows [r0, r0+32) of the 128-column panel `pan` of Y into dst[col][SY_LD]; zero fill outside m x n
+// loads rows [r0, r0+32) of the 128-column panel `pan` of Y into dst[col][SY_LD]; zero fill outside m x n.
+// VEC: thread (col0 = tid / 16, r2 = 2 (tid % 16)) copies 16 bytes of the columns col0, col0 + 16, ...:
+// the source pointer advances by a constant, colmask (bit k: column col0 + 16 k exists) is per kernel.
 __device__ __forceinline__ void sy_load_panel(double* dst, const SyrkParams& p, const double* __restrict__ Y,
-                                              int pan, int64_t r0, int tid)
+                                              int pan, int64_t r0, int tid, unsigned colmask)
 {
     const int64_t left = p.m - r0;
     if (p.vec) {
-        for (int e = tid; e < SY_B * (SY_KC / 2); e += SY_THREADS) {
-            const int col = e / (SY_KC / 2), r2 = (e % (SY_KC / 2)) * 2;
-            const int gc = pan * SY_B + col;
-            const int64_t avail = (gc < p.n) ? left - r2 : 0;
-            const int bytes = avail >= 2 ? 16 : (avail == 1 ? 8 : 0);
-            const double* src = Y + (bytes ? (size_t)gc * (size_t)p.ldy + r0 + r2 : 0);
-            sy_cp16(dst + col * SY_LD + r2, src, bytes);
+        const int col0 = tid >> 4, r2 = (tid & 15) * 2;
+        const int64_t avail = left - r2;
+        const int rb = avail >= 2 ? 16 : (avail == 1 ? 8 : 0);
+        const double* src = Y + (size_t)(pan * SY_B + col0) * (size_t)p.ldy + r0 + r2;
+        double* d = dst + col0 * SY_LD + r2;
+        const size_t step = (size_t)16 * (size_t)p.ldy;
+#pragma unroll
+        for (int k = 0; k < SY_B / 16; ++k) {
+            const int bytes = ((colmask >> k) & 1u) ? rb : 0;
+            sy_cp16(d + k * 16 * SY_LD, bytes ? src + k * step : Y, bytes);
         }
     } else {
         for (int e = tid; e < SY_B * SY_KC; e += SY_THREADS) {
@@ -72,7 +77,7 @@ __device__ __forceinline__ void sy_load_panel(double* dst, const SyrkParams& p, 
 __global__ void __launch_bounds__(SY_THREADS, 1)
 mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ partials)
 {
-    extern __shared__ __align__(16) double sy_sm[];        // [2 stages][2 panels][128 * SY_LD]
+    extern __shared__ __align__(16) double sy_sm[];        // [3 stages][2 panels][128 * SY_LD]
     constexpr int PAN = SY_B * SY_LD;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
     const int pair = blockIdx.x / p.ksplit, ks_id = blockIdx.x % p.ksplit;
@@ -94,10 +99,16 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
 #pragma unroll
         for (int b = 0; b < 8; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
     bool first = true;
-    auto issue = [&](int c) {
-        double* st = sy_sm + (size_t)(c & 1) * 2 * PAN;
-        sy_load_panel(st, p, Y, I, k0 + (int64_t)c * SY_KC, tid);
-        if (!diag) sy_load_panel(st + PAN, p, Y, J, k0 + (int64_t)c * SY_KC, tid);
+    unsigned maskI = 0, maskJ = 0;
+#pragma unroll
+    for (int k = 0; k < SY_B / 16; ++k) {
+        if (I * SY_B + (tid >> 4) + 16 * k < p.n) maskI |= 1u << k;
+        if (J * SY_B + (tid >> 4) + 16 * k < p.n) maskJ |= 1u << k;
+    }
+    auto issue = [&](int c) {                        // chunk c -> stage c % 3
+        double* st = sy_sm + (size_t)(c % 3) * 2 * PAN;
+        sy_load_panel(st, p, Y, I, k0 + (int64_t)c * SY_KC, tid, maskI);
+        if (!diag) sy_load_panel(st + PAN, p, Y, J, k0 + (int64_t)c * SY_KC, tid, maskJ);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     auto flush = [&]() {
@@ -114,13 +125,17 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
         }
         first = false;
     };
+    // three stages, ONE barrier per chunk: the barrier of iteration c also proves that every warp is done
+    // with chunk c-1, whose stage chunk c+2 is about to overwrite
     if (nchunks > 0) issue(0);
+    if (nchunks > 1) issue(1);
     for (int c = 0; c < nchunks; ++c) {
-        if (c + 1 < nchunks) { issue(c + 1); asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+        if (c + 1 < nchunks) asm volatile("cp.async.wait_group 1;" ::: "memory");
         else asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();
+        if (c + 2 < nchunks) issue(c + 2);
         if (!skip) {
-            const double* pI = sy_sm + (size_t)(c & 1) * 2 * PAN;
+            const double* pI = sy_sm + (size_t)(c % 3) * 2 * PAN;
             const double* pJ = diag ? pI : pI + PAN;
             const double* fi = pI + (32 * wi + g) * SY_LD + t;
             const double* fj = pJ + (64 * wj + g) * SY_LD + t;
@@ -137,7 +152,6 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
                     for (int b = 0; b < 8; ++b) sy_dmma(acc[a][b], fI[a], fJ[b]);
             }
         }
-        __syncthreads();
         if ((c + 1) % SY_FLUSH == 0 || c + 1 == nchunks) flush();
     }
     if (nchunks == 0) flush();                               // an empty range still owns a (zero) partial
@@ -203,7 +217,7 @@ int launch_syrk(int64_t m, int n, int64_t ldy, const double* Y, double* partials
     SyrkParams p = syrk_params(m, n, n16);
     p.ldy = ldy;
     p.vec = ((uintptr_t)Y % 16 == 0) && (ldy % 2 == 0);
-    const int smem = 2 * 2 * SY_B * SY_LD * (int)sizeof(double);
+    const int smem = 3 * 2 * SY_B * SY_LD * (int)sizeof(double);
     cudaFuncSetAttribute(mrcqr_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     mrcqr_syrk<<<p.pairs * p.ksplit, SY_THREADS, smem, s>>>(p, Y, partials);
     mrcqr_syrk_reduce<<<p.pairs * (SY_B * SY_B / 32), 1024, 0, s>>>(p, partials, G16);

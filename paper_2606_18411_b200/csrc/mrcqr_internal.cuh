@@ -85,6 +85,8 @@ int launch_triu_mul(const double* Rc, const double* Rs, int n, double* R, cudaSt
 // NOTE: for n > 64 the sketch `As` is overwritten (factored in place by the blocked kernel).
 int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* Rs, double* RsPrep, int n16,
                         double* betas, Status* st, cudaStream_t s);
+int launch_k4_coop(double* G16, int n, int n16, double* G_out, double* Rc, double* RcPrep, const double* Rs,
+                   double* R, Status* st, cudaStream_t stream);
 bool k2_blocked_usable(int s_rows, int n);
 int launch_k2_blocked(double* As, int s_rows, int n, double* betas, double* Rs, double* RsPrep, int n16,
                       Status* st, cudaStream_t stream);
