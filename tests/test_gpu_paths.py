@@ -107,3 +107,46 @@ def test_store_y_variant_below_128_columns(orc, m, n, prec):
     finally:
         B.mrcqr_set_store_y(False)
     assert torch.equal(Q0, Q1) and torch.equal(R0, R1)
+
+
+def test_large_n_kernels_report_breakdown(orc):
+    """The cooperative-grid Cholesky (n16 > 160) and the blocked sketch QR (n > 64) report what the small
+    kernels report: a non-positive pivot -> code 3 with its index; a zero R_s diagonal -> code 2 with its index."""
+    from helpers import colmajor_to_dev
+    m, n = 2048, 200
+    rng = np.random.default_rng(3)
+    A = np.asfortranarray(rng.standard_normal((m, n)))
+    A[:, 150] = 0.0                                            # with R_s = I: G[150,150] = 0 exactly
+    with pytest.raises(B.MrcqrError) as e:
+        B.mrcqr_precondition_gram(colmajor_to_dev(A), colmajor_to_dev(np.eye(n)))
+    assert e.value.code == 3 and e.value.info == 150
+    # the stage call returns G and R_c of a healthy matrix through the same kernel
+    A[:, 150] = rng.standard_normal(m)
+    Rc, G = B.mrcqr_precondition_gram(colmajor_to_dev(A), colmajor_to_dev(np.eye(n)), want_G=True)
+    Gn, Rcn = to_np(G), to_np(Rc)
+    assert np.linalg.norm(Gn - A.T @ A) <= 1e-13 * np.linalg.norm(Gn)
+    assert np.linalg.norm(Rcn.T @ Rcn - Gn) <= 1e-13 * np.linalg.norm(Gn)
+    assert np.all(np.diag(Rcn) > 0) and np.array_equal(np.tril(Rcn, -1), np.zeros((n, n)))
+    # blocked sketch QR: the last column of an odd-n matrix is exactly zero -> its sketch is exactly zero
+    m2, n2 = 1 << 13, 131
+    A2 = np.asfortranarray(rng.standard_normal((m2, n2)))
+    A2[:, 130] = 0.0
+    rc = B.mrcqr_factor(colmajor_to_dev(A2), B.FP64, 2 * n2, 1, check=False)
+    assert rc == 2 and B.mrcqr_last_info() == 130
+
+
+def test_blocked_sketch_qr_is_a_qr_of_the_sketch(orc):
+    """R_s^T R_s = A_s^T A_s to n u ||A_s||^2, upper triangular, diag > 0, for the blocked kernel's shapes
+    (panel remainders: n = 100 -> last panel of 4; s not a multiple of 256; s = 3n)."""
+    for m, n, s in [(1 << 13, 100, 200), (1 << 13, 72, 216), (1 << 12, 300, 600)]:
+        AT = inputs.make_A(m, n, 6, 40 + n, 41 + n, "cuda")
+        signs, idx = orc.draw(m, s, 9)
+        dsigns, didx = draw_to_dev(signs, idx)
+        Rs, As = B.mrcqr_sketch(AT, B.FP64, dsigns, didx, want_As=True)
+        Rsn, Asn = to_np(Rs), to_np(As)
+        assert np.all(np.diag(Rsn) > 0) and np.array_equal(np.tril(Rsn, -1), np.zeros((n, n)))
+        assert np.linalg.norm(Rsn.T @ Rsn - Asn.T @ Asn) <= 100 * n * U * np.linalg.norm(Asn) ** 2
+        # same R as the oracle's Householder QR of the oracle's sketch, to kappa(A_s) u
+        o = orc.factor_from_draw(to_np(AT), signs, idx, want_intermediates=True)
+        kap = np.linalg.cond(o["Rs"])
+        assert np.linalg.norm(Rsn - o["Rs"]) <= 100 * n * U * kap * np.linalg.norm(o["Rs"])
