@@ -290,6 +290,51 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """--sweep: BASELINE.json configs[0..3] and the column sweep configs[4] (m = 2^21, n in 16..512, three sketch
+    precisions): per-stage CUDA-event times and both roofline floors, one markdown table row per point (not the
+    bench contract's JSON line; used for profiles/ and DESIGN.md)."""
+    import torch
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import gpu_orth_error_fro, gpu_residual_fro
+    from paper_2606_18411_b200 import binding as B
+    from paper_2606_18411_b200 import inputs
+    hbm_peak, _ = measured_peaks()
+    points = [(k, dict(inputs.CONFIGS[k])) for k in ("C0", "C1", "C2", "C3")]
+    for n in (16, 32, 64, 128, 256, 512):
+        for prec in (16, 32, 64):
+            points.append(("C4 n=%d fp%d" % (n, prec), inputs.sweep_config(n, prec)))
+    print("| config | m | n | sketch | total ms | K1 | K2 | K3 / solve | reduce+K4 (+SYRK) | K5 / solve | HBM floor | FP64 floor | orth | resid |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    for name, cfg in points:
+        AT = inputs.make_config(cfg, "cuda")
+        n, m = AT.shape
+        QT = torch.empty_like(AT)
+        R = torch.empty((n, n), dtype=torch.float64, device="cuda")
+        B.mrcqr_set_timing(True)
+        acc = {}
+        for it in range(3 + args.steps):
+            B.mrcqr_factor(AT, cfg["prec"], cfg["s"], cfg["seed_draw"], QT=QT, R=R)
+            if it >= 3:
+                for k, v in B.mrcqr_last_timing().items():
+                    acc[k] = acc.get(k, 0.0) + v / args.steps
+        B.mrcqr_set_timing(False)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            B.mrcqr_factor(AT, cfg["prec"], cfg["s"], cfg["seed_draw"], QT=QT, R=R)
+        e1.record()
+        torch.cuda.synchronize()
+        tot = e0.elapsed_time(e1) / args.steps
+        flop = (3.0 if n > 128 else 4.0) * m * n * n
+        print("| %s | %d | %d | fp%d | %.3f | %.3f | %.3f | %.3f | %.3f | %.3f | %.3f | %.3f | %.1e | %.1e |" % (
+            name, m, n, cfg["prec"], tot, acc["k1_srtt"], acc["k2_sketch_qr"], acc["k3_gram"], acc["reduce_k4_chol"],
+            acc["k5_form_q"], 32.0 * m * n / (hbm_peak * 1e9) * 1e3, flop / (FP64_DMMA_PEAK_TFLOPS * 1e12) * 1e3,
+            gpu_orth_error_fro(QT), gpu_residual_fro(AT, QT, R)), flush=True)
+        del AT, QT
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -298,7 +343,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="per-stage table over BASELINE.json configs 0-4 instead of the JSON line")
     args = ap.parse_args()
+    if args.sweep:
+        args.steps = min(args.steps, 5)
+        return run_sweep(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
