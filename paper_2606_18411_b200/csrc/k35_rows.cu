@@ -152,7 +152,7 @@ __device__ __forceinline__ void sb_to_pq(int sb, int& p, int& q)
 // NB > 0: n16 = 8*NB <= 128, compile-time Gram ownership, accumulators live in registers across tiles.
 // NB = 0: n16 > 128, 16x16 super-blocks in sweeps, flushed to the L2-resident partial every tile.
 template <int RG, int NW, int NB, bool VEC>
-__global__ void __launch_bounds__(NW * 32, (RG == 4 && NW == 4) ? 3 : 1)
+__global__ void __launch_bounds__(NW * 32, (RG == 4 && NW == 4) ? (NB == 2 ? 5 : (NB == 4 ? 4 : 3)) : 1)
 mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__ A,
               const double2* __restrict__ fragS, double* __restrict__ partials,
               int64_t ntiles, double* __restrict__ Ydump, double* __restrict__ Ystore, int64_t ldys)
@@ -262,8 +262,11 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
 // K5: every warp streams its own slabs (slab i belongs to global warp i mod (grid * NW)); no CTA barrier.
 // mode 3: both solves (y = a Rs^-1, q = y Rc^-1); mode 1: only the first (store-Y form of stage 2a for
 // n16 > 128, Y goes to the Q buffer); mode 2: only the second, in place on the stored Y.
+// warps per CTA by panel size: small panels need few registers, and a 4 KB slab needs many warps in flight
+constexpr int k5_max_warps(int nbt) { return nbt == 2 ? 20 : (nbt == 4 ? 16 : 12); }
+
 template <int RG, int NBT, bool VEC>
-__global__ void __launch_bounds__(384, 1)
+__global__ void __launch_bounds__(32 * k5_max_warps(NBT), 1)
 mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict__ A,
                const double2* __restrict__ fragS, const double2* __restrict__ fragC,
                int64_t ldq, double* __restrict__ Q, int64_t nslabs, double* __restrict__ Ydump, int mode)
@@ -433,8 +436,8 @@ int num_sms()
 size_t k3_partials_bytes(int n)
 {
     RowCfg c = row_config(n);
-    // at most 4 resident CTAs per SM are ever launched
-    return (size_t)num_sms() * 4 * (size_t)c.n16 * c.n16 * sizeof(double);
+    // at most 4 (8 for n16 <= 32) resident CTAs per SM are ever launched
+    return (size_t)num_sms() * (c.n16 <= 32 ? 8 : 4) * (size_t)c.n16 * c.n16 * sizeof(double);
 }
 
 int upload_diag(const double* prep, int n16, int fac, cudaStream_t s)
@@ -446,13 +449,13 @@ int upload_diag(const double* prep, int n16, int fac, cudaStream_t s)
 }
 
 template <typename K>
-static int grid_for(K kernel, int threads, int smem, int64_t ntiles)
+static int grid_for(K kernel, int threads, int smem, int64_t ntiles, int cap)
 {
     cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     int occ = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem);
     if (occ < 1) occ = 1;
-    if (occ > 4) occ = 4;
+    if (occ > cap) occ = cap;
     int64_t g = (int64_t)occ * num_sms();
     return (int)(g < ntiles ? g : ntiles);
 }
@@ -469,7 +472,7 @@ int launch_k3_gram(int64_t m, int n, int64_t lda, const double* A, const double*
     const double2* frag = reinterpret_cast<const double2*>(RsPrep);
 #define K3_GO(RG_, NW_, NB_, V_)                                                                    \
     { auto k = mrcqr_k3_gram<RG_, NW_, NB_, V_>;                                                    \
-      int grid = grid_for(k, NW_ * 32, c.smem_bytes, ntiles); *n_partials_out = grid;               \
+      int grid = grid_for(k, NW_ * 32, c.smem_bytes, ntiles, c.n16 <= 32 ? 8 : 4); *n_partials_out = grid;               \
       k<<<grid, NW_ * 32, c.smem_bytes, s>>>(m, n, c.n16, lda, A, frag, partials, ntiles, Ydump, Ystore, ldys); }
 #define K3_CALL(RG_, NW_, NB_) { if (vec) K3_GO(RG_, NW_, NB_, true) else K3_GO(RG_, NW_, NB_, false) }
     switch (c.n16) {
@@ -492,7 +495,8 @@ int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double
     const int SR = 8 * c.RG;
     const int slab_bytes = c.n16 * (SR + 4) * 8;
     int nw = SMEM_CAP / slab_bytes;
-    if (nw > 12) nw = 12;
+    const int wcap = k5_max_warps(c.n16 <= 64 ? c.n16 / 8 : 0);
+    if (nw > wcap) nw = wcap;
     if (nw < 1) nw = 1;
     const int smem = nw * slab_bytes;
     const int64_t nslabs = (m + SR - 1) / SR;
