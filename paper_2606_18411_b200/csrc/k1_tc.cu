@@ -157,26 +157,35 @@ mrcqr_k1_tc(K1TcParams p, const __grid_constant__ CUtensorMap tmapA, const uint3
     if (tid == 0) { mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
-    unsigned sgs[2] = {0u, 0u};                       // this thread's sign bits of the tile in each stage
-    auto issue_tile = [&](int64_t id, int stg) {      // tile id -> raw stage stg; sign words -> registers
-        const int j = (int)(id / tpc), tl = (int)(id % tpc);
+    // sign bits of this thread's 16 rows (4 per row pair).  The 16 words of the NEXT tile are requested before the
+    // current tile is multiplied and packed after its second stage, so their L2 latency hides under the MMAs.
+    unsigned sg_cur = 0u, sw[16];
+    auto issue_tile = [&](int64_t id, int stg) {      // tile id -> raw stage stg (one TMA box)
         if (tid == 0) {
+            const int j = (int)(id / tpc), tl = (int)(id % tpc);
             mbar_arrive_expect_tx(&mbar[stg], TC_M1 * TC_NT * 8);
             tma_load_3d(raw_sm + (size_t)stg * (TC_M1 * TC_NT * 8), &tmapA, tl * TC_NT, 0, j, &mbar[stg]);
         }
-        unsigned sg = 0;
+    };
+    auto sign_load = [&](int64_t id) {
+        const int tl = (int)(id % tpc);
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             const int t1 = rgp + 16 * u, t1m = (t1 == 0) ? 128 : TC_M1 - t1;
-            const unsigned w0 = (signs32[((int64_t)t1 * p.m2 + (int64_t)tl * TC_NT) >> 5] >> (2 * c16)) & 3u;
-            const unsigned w1 = (signs32[((int64_t)t1m * p.m2 + (int64_t)tl * TC_NT) >> 5] >> (2 * c16)) & 3u;
-            sg |= (w0 | (w1 << 2)) << (4 * u);
+            sw[2 * u] = signs32[((int64_t)t1 * p.m2 + (int64_t)tl * TC_NT) >> 5];
+            sw[2 * u + 1] = signs32[((int64_t)t1m * p.m2 + (int64_t)tl * TC_NT) >> 5];
         }
-        sgs[stg] = sg;
+    };
+    auto sign_pack = [&]() {
+        unsigned sg = 0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            sg |= (((sw[2 * u] >> (2 * c16)) & 3u) | (((sw[2 * u + 1] >> (2 * c16)) & 3u) << 2)) << (4 * u);
+        return sg;
     };
     auto convert_tile = [&](int b) {                 // DiagMult + fold + round to FP16: raw[b] -> X[b]
         const double2* raw = reinterpret_cast<const double2*>(raw_sm + (size_t)b * (TC_M1 * TC_NT * 8)) + c16;
-        const unsigned sg = b ? sgs[1] : sgs[0];
+        const unsigned sg = sg_cur;
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             const int t1 = rgp + 16 * u, t1m = (t1 == 0) ? 128 : TC_M1 - t1;
@@ -206,14 +215,15 @@ mrcqr_k1_tc(K1TcParams p, const __grid_constant__ CUtensorMap tmapA, const uint3
             accb[h] = 0.0f;
         }
     };
-    if (lo < hi) issue_tile(lo, 0);
+    if (lo < hi) { issue_tile(lo, 0); sign_load(lo); sg_cur = sign_pack(); }
     if (lo + 1 < hi) issue_tile(lo + 1, 1);
     for (int64_t id = lo; id < hi; ++id) {
         const int b = (int)(id - lo) & 1;
         mbar_wait(&mbar[b], (unsigned)((id - lo) >> 1) & 1u);
         convert_tile(b);
         __syncthreads();                              // X[b] complete; raw[b] and X[b^1] free
-        if (id + 2 < hi) { if (b == 0) issue_tile(id + 2, 0); else issue_tile(id + 2, 1); }
+        if (id + 2 < hi) issue_tile(id + 2, b);
+        if (id + 1 < hi) sign_load(id + 1);
         // ---- first stage on the tensor cores: (Cc, Cs) = F * X~ for this warp's 16 bins x 8 NTW columns
         float accC[NTW][4], accS[NTW][4];
 #pragma unroll
@@ -265,6 +275,7 @@ mrcqr_k1_tc(K1TcParams p, const __grid_constant__ CUtensorMap tmapA, const uint3
             sincospif(2.0f * (float)r / (float)p.m, &st, &ct);
             accb[h] += ct * S1 - st * S2;
         }
+        if (id + 1 < hi) sg_cur = sign_pack();
     }
     if (lo < hi) flush();
 }
