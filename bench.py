@@ -340,6 +340,34 @@ def run_sweep(args):
         torch.cuda.empty_cache()
 
 
+def run_stability(args):
+    """--stability: the MRCQR curves of the paper's Fig. 1 on its own test matrices (eq. (3):
+    A = U Sigma V^T, m = 2^17, n = 50, kappa = 1e2 .. 1e16, s = 3n): ||I - Q^T Q||_F and ||A - QR||_F / ||A||_F for the
+    three sketch precisions, plus the self-correcting wrapper started at FP16.  Markdown table."""
+    import torch
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import gpu_residual_fro
+    from paper_2606_18411_b200 import binding as B
+    from paper_2606_18411_b200 import inputs
+    m, n = 1 << 17, 50
+    print("| kappa | fp16 orth | fp16 resid | fp32 orth | fp32 resid | fp64 orth | fp64 resid | auto: precision used, orth |")
+    print("|---|---|---|---|---|---|---|---|")
+    for e in range(2, 17, 2):
+        AT = inputs.make_paper_eq3(m, n, 10.0 ** e, 100 + e, 200 + e, "cuda")
+        QT = torch.empty_like(AT)
+        R = torch.empty((n, n), dtype=torch.float64, device="cuda")
+        cells = []
+        for prec in (16, 32, 64):
+            rc = B.mrcqr_factor(AT, prec, 3 * n, 7, QT, R, check=False)
+            if rc != 0:
+                cells += ["code %d" % rc, "-"]
+            else:
+                cells += ["%.1e" % B.mrcqr_orth_error(QT), "%.1e" % gpu_residual_fro(AT, QT, R)]
+        rc, used, orth = B.mrcqr_factor_auto(AT, 16, 3 * n, 7, 0.0, QT, R, check=False)
+        cells.append("fp%d, %.1e%s" % (used, orth, "" if rc == 0 else " (code %d)" % rc))
+        print("| 1e%d | %s |" % (e, " | ".join(cells)), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -348,8 +376,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--stability", action="store_true", help="orthogonality / residual vs kappa on the paper's eq.(3) matrices")
     ap.add_argument("--sweep", action="store_true", help="per-stage table over BASELINE.json configs 0-4 instead of the JSON line")
     args = ap.parse_args()
+    if args.stability:
+        return run_stability(args)
     if args.sweep:
         args.steps = min(args.steps, 5)
         return run_sweep(args)

@@ -39,7 +39,8 @@ enum {
     MRCQR_ERR_NONFINITE = 1,  /* non-finite value in the sketch (e.g. FP16 overflow of fl_p(D A))        */
     MRCQR_ERR_SINGULAR  = 2,  /* R_s has a zero / non-finite diagonal: A rank deficient   */
     MRCQR_ERR_BREAKDOWN = 3,  /* Cholesky pivot <= 0 or NaN; index: mrcqr_last_info() */
-    MRCQR_ERR_CUDA      = 4   /* CUDA runtime error, or no device                                        */
+    MRCQR_ERR_CUDA      = 4,  /* CUDA runtime error, or no device                                        */
+    MRCQR_ERR_NOT_ORTHOGONAL = 5  /* mrcqr_factor_auto: ||I - Q^T Q||_F > tol even with the FP64 sketch       */
 };
 
 /*
@@ -127,6 +128,27 @@ int mrcqr_last_launch_count(void);
  */
 int mrcqr_set_timing(int on);
 int mrcqr_last_timing(float* ms_out_host);
+
+/*
+ * ||I - Q^T Q||_F of a column-major m x n Q (device), the quantity the paper monitors (Frobenius
+ * instead of the 2-norm, R13).  Q^T Q is accumulated on the FP64 tensor cores in chains of 1024 rows with a
+ * fixed-order reduction (a plain long accumulation adds ~1e-14 of its own at m = 2^20).  err_host: one double (host).
+ * Returns 0 or -1 m, -2 n, -3 ldq, -4 Q, -5 err_host, 4.
+ */
+int mrcqr_orth_error(int64_t m, int n, int64_t ldq, const double* Q, double* err_host, void* stream);
+
+/*
+ * Self-correcting MRCQR ("the remedy is to rerun MRCQR at the next higher precision level"):
+ * factor with the sketch precision first_prec; if the factorization reports a positive code or
+ * ||I - Q^T Q||_F > tol, rerun at the next precision (half -> single -> double).  tol <= 0 means 1e-13.
+ * prec_used_host / orth_host (nullable, host): the precision of the returned (Q, R) and its measured
+ * ||I - Q^T Q||_F (-1 if that run reported a positive code).  Returns 0; a negative argument index as
+ * mrcqr_factor; or the outcome at FP64: codes 1-3, or MRCQR_ERR_NOT_ORTHOGONAL with the FP64 result in (Q, R).
+ * Nothing is hidden: every escalation is visible through prec_used_host.
+ */
+int mrcqr_factor_auto(int64_t m, int n, int64_t lda, const double* A, double* Q, double* R,
+                      mrcqr_prec_t first_prec, int s, uint64_t seed, double tol,
+                      int* prec_used_host, double* orth_host, void* stream);
 
 /*
  * Variant switch of mrcqr_factor / mrcqr_factor_host ("store-Y"): off (default), stage 2a

@@ -17,7 +17,7 @@ from . import build as _build
 
 FP16, FP32, FP64 = 16, 32, 64
 ERRORS = {1: "non-finite value in the sketch", 2: "R_s singular (A rank deficient)",
-          3: "Cholesky breakdown", 4: "CUDA error / no device"}
+          3: "Cholesky breakdown", 4: "CUDA error / no device", 5: "not orthogonal to tolerance at FP64"}
 
 _lib = None
 
@@ -49,11 +49,13 @@ def lib():
         L.mrcqr_debug_dump_y.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
         L.mrcqr_shutdown.restype = None
         L.mrcqr_set_timing.argtypes = [ci]
+        L.mrcqr_orth_error.argtypes = [i64, ci, i64, vp, vp, vp]
+        L.mrcqr_factor_auto.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64, C.c_double, vp, vp, vp]
         L.mrcqr_set_store_y.argtypes = [ci]
         L.mrcqr_last_timing.argtypes = [vp]
         for f in ("mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
                   "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
-                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y"):
+                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto"):
             getattr(L, f).restype = ci
         _lib = L
     return _lib
@@ -61,7 +63,7 @@ def lib():
 
 EXPORTS = ["mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
-           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y"]
+           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto"]
 
 STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "reduce_k4_chol", "k5_form_q", "r_mul"]
 
@@ -179,6 +181,30 @@ def mrcqr_last_launch_count():
 
 def mrcqr_shutdown():
     lib().mrcqr_shutdown()
+
+
+def mrcqr_orth_error(QT, stream=None):
+    """||I - Q^T Q||_F of the column-major Q held in QT (n, m), computed on the device."""
+    m, n, ldq, pQ = _mat(QT)
+    err = C.c_double(0.0)
+    _chk(lib().mrcqr_orth_error(m, n, ldq, pQ, C.byref(err), _stream(stream)))
+    return float(err.value)
+
+
+def mrcqr_factor_auto(AT, first_prec, s, seed, tol=0.0, QT=None, R=None, stream=None, check=True):
+    """Self-correcting MRCQR.  Returns (QT, R, prec_used, orth) (or (rc, prec_used, orth) if check=False)."""
+    m, n, lda, pA = _mat(AT)
+    if QT is None:
+        QT = torch.empty_strided((n, m), (lda, 1), dtype=torch.float64, device=AT.device)
+    if R is None:
+        R = torch.empty((n, n), dtype=torch.float64, device=AT.device)
+    used, orth = C.c_int(0), C.c_double(0.0)
+    rc = lib().mrcqr_factor_auto(m, n, lda, pA, QT.data_ptr(), R.data_ptr(), first_prec, s, seed, float(tol),
+                                 C.byref(used), C.byref(orth), _stream(stream))
+    if not check:
+        return rc, int(used.value), float(orth.value)
+    _chk(rc)
+    return QT, R, int(used.value), float(orth.value)
 
 
 def mrcqr_set_store_y(on):

@@ -94,7 +94,7 @@ static bool device_ok()
 
 static bool ensure_ws(size_t bytes)
 {
-    if (!g.h_status && cudaMallocHost(&g.h_status, 64) != cudaSuccess) return false;
+    if (!g.h_status && cudaMallocHost(&g.h_status, 64) != cudaSuccess) return false;   // [0..1] status, [2..3] a double
     if (bytes <= g.ws_bytes) return true;
     if (g.ws) { cudaDeviceSynchronize(); cudaFree(g.ws); g.ws = nullptr; g.ws_bytes = 0; }
     if (cudaMalloc(&g.ws, bytes) != cudaSuccess) { cudaGetLastError(); return false; }
@@ -397,6 +397,68 @@ extern "C" int mrcqr_factor(int64_t m, int n, int64_t lda, const double* A, doub
     if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX) return -8;
     if (!device_ok()) return MRCQR_ERR_CUDA;
     return factor_device(m, n, lda, A, lda, Q, R, (int)sketch_prec, s, seed, (cudaStream_t)stream);
+}
+
+// ||I - Q^T Q||_F on the device: DMMA SYRK of Q (deterministic row split, chains flushed every 1024 rows) + norm
+static int orth_error_device(int64_t m, int n, int64_t ldq, const double* Q, double* err_host, cudaStream_t st)
+{
+    Layout L = make_layout(m, n, 0, 64);
+    if (!ensure_ws(L.total)) return MRCQR_ERR_CUDA;
+    const int n16 = round_up(n, 16);
+    double* G16 = reinterpret_cast<double*>(g.ws + L.G16);
+    double* part = reinterpret_cast<double*>(g.ws + L.k3);
+    double* err = reinterpret_cast<double*>(g.ws + L.betas);          // n doubles of scratch: [0] receives the norm
+    mrcqr_reset_status<<<1, 1, 0, st>>>(reinterpret_cast<Status*>(g.ws + L.status));
+    int k = 1 + launch_syrk(m, n, ldq, Q, part, n16, G16, st);
+    k += launch_orth_norm(G16, n, n16, err, st);
+    cudaMemcpyAsync(g.h_status + 2, err, sizeof(double), cudaMemcpyDeviceToHost, st);
+    const int rc = finish(L, st, k);
+    if (rc == 0) std::memcpy(err_host, g.h_status + 2, sizeof(double));
+    return rc;
+}
+
+extern "C" int mrcqr_orth_error(int64_t m, int n, int64_t ldq, const double* Q, double* err_host, void* stream)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (m < n) return -1;
+    if (ldq < m) return -3;
+    if (!Q) return -4;
+    if (!err_host) return -5;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    return orth_error_device(m, n, ldq, Q, err_host, (cudaStream_t)stream);
+}
+
+extern "C" int mrcqr_factor_auto(int64_t m, int n, int64_t lda, const double* A, double* Q, double* R,
+                                 mrcqr_prec_t first_prec, int s, uint64_t seed, double tol,
+                                 int* prec_used_host, double* orth_host, void* stream)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (!is_pow2(m) || m < n || m < 32) return -1;
+    if (lda < m) return -3;
+    if (!A) return -4;
+    if (!Q) return -5;
+    if (!R) return -6;
+    if (!prec_ok((int)first_prec)) return -7;
+    if (s <= 0) s = 3 * n;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX) return -8;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    if (!(tol > 0.0)) tol = 1e-13;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = 0;
+    for (int p = (int)first_prec; p <= 64; p *= 2) {         // half -> single -> double
+        rc = factor_device(m, n, lda, A, lda, Q, R, p, s, seed, st);
+        if (rc < 0 || rc == MRCQR_ERR_CUDA) return rc;
+        double orth = -1.0;
+        if (rc == 0) {
+            const int rc2 = orth_error_device(m, n, lda, Q, &orth, st);
+            if (rc2 != 0) return rc2;
+        }
+        if (prec_used_host) *prec_used_host = p;
+        if (orth_host) *orth_host = orth;
+        if (rc == 0 && orth <= tol) return 0;                 // NaN fails the comparison: escalates
+        if (rc == 0) rc = MRCQR_ERR_NOT_ORTHOGONAL;
+    }
+    return rc;                                               // the outcome at the highest precision
 }
 
 extern "C" int mrcqr_factor_host(int64_t m, int n, int64_t lda, const double* A_host, double* Q_host,

@@ -205,11 +205,38 @@ static SyrkParams syrk_params(int64_t m, int n, int n16)
 size_t syrk_partials_bytes(int n)
 {
     const int n16 = round_up(n, 16);
-    if (n16 <= 128) return 0;
     const int P = (n16 + SY_B - 1) / SY_B, pairs = P * (P + 1) / 2;
     int ks = num_sms() / pairs;
     if (ks < 1) ks = 1;
     return (size_t)pairs * ks * SY_B * SY_B * sizeof(double);
+}
+
+// err[0] = || I - G ||_F for the symmetric n x n matrix held in G16 (upper triangle read), fixed summation order
+__global__ void __launch_bounds__(1024)
+mrcqr_orth_norm(const double* __restrict__ G16, int n, int n16, double* __restrict__ err)
+{
+    __shared__ double sm[1024];
+    double acc = 0.0;
+    for (int e = threadIdx.x; e < n * n; e += 1024) {
+        const int i = e % n, j = e / n;
+        if (i <= j) {
+            const double d = G16[(size_t)j * n16 + i] - (i == j ? 1.0 : 0.0);
+            acc = fma(i == j ? 1.0 : 2.0, d * d, acc);
+        }
+    }
+    sm[threadIdx.x] = acc;
+    __syncthreads();
+    for (int h = 512; h > 0; h >>= 1) {
+        if (threadIdx.x < h) sm[threadIdx.x] += sm[threadIdx.x + h];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) err[0] = sqrt(sm[0]);
+}
+
+int launch_orth_norm(const double* G16, int n, int n16, double* err, cudaStream_t s)
+{
+    mrcqr_orth_norm<<<1, 1024, 0, s>>>(G16, n, n16, err);
+    return 1;
 }
 
 int launch_syrk(int64_t m, int n, int64_t ldy, const double* Y, double* partials, int n16, double* G16, cudaStream_t s)

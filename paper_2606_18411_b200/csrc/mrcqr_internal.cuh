@@ -78,6 +78,7 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
                        double* dst, int64_t ldd, cudaStream_t s);
 // G = Y^T Y of a stored m x n Y (n16 > 128): DMMA SYRK over 128 x 128 blocks with a deterministic split of the rows
 size_t syrk_partials_bytes(int n);
+int launch_orth_norm(const double* G16, int n, int n16, double* err, cudaStream_t s);   // err[0] = ||I - G||_F
 int launch_syrk(int64_t m, int n, int64_t ldy, const double* Y, double* partials, int n16, double* G16, cudaStream_t s);
 int launch_triu_mul(const double* Rc, const double* Rs, int n, double* R, cudaStream_t s);
 // RsPrep nullable: when given, the kernel also writes the prepared Rs and reports a singular diagonal.

@@ -150,3 +150,55 @@ def test_blocked_sketch_qr_is_a_qr_of_the_sketch(orc):
         o = orc.factor_from_draw(to_np(AT), signs, idx, want_intermediates=True)
         kap = np.linalg.cond(o["Rs"])
         assert np.linalg.norm(Rsn - o["Rs"]) <= 100 * n * U * kap * np.linalg.norm(o["Rs"])
+
+
+def test_orth_error_matches_the_oracle_checker(orc):
+    """mrcqr_orth_error against the oracle's blocked-pairwise ||I - Q^T Q||_F: on an orthonormal Q (rounding level:
+    same order of magnitude) and on a Q with a planted defect (closed form: Q (I + E) with small E gives
+    ||E + E^T + E^T E||_F)."""
+    m, n = 1 << 14, 48
+    AT = inputs.make_A(m, n, 2, 5, 6, "cuda")
+    QT, _ = B.mrcqr_factor(AT, B.FP64, 2 * n, 1)
+    e_gpu, e_orc = B.mrcqr_orth_error(QT), orc.orth_error_fro(to_np(QT))
+    assert e_gpu <= 1e-13 and e_orc <= 1e-13 and 0.2 * e_orc <= e_gpu <= 5 * e_orc
+    rng = np.random.default_rng(1)
+    E = 1e-6 * rng.standard_normal((n, n))
+    Qd = to_np(QT) @ (np.eye(n) + E)
+    want = np.linalg.norm(E + E.T + E.T @ E)
+    QdT = torch.from_numpy(np.ascontiguousarray(Qd.T)).cuda()
+    assert abs(B.mrcqr_orth_error(QdT) - want) <= 1e-6 * want
+    assert abs(orc.orth_error_fro(Qd) - want) <= 1e-6 * want
+    # n > 128 goes through several 128 x 128 blocks
+    AT2 = inputs.make_A(1 << 12, 200, 2, 7, 8, "cuda")
+    QT2, _ = B.mrcqr_factor(AT2, B.FP64, 400, 1)
+    assert 0.2 * orc.orth_error_fro(to_np(QT2)) <= B.mrcqr_orth_error(QT2) <= 5 * orc.orth_error_fro(to_np(QT2))
+
+
+def test_factor_auto_escalates_only_when_needed(orc):
+    """an underestimated precision is detected by ||I - Q^T Q|| and cured by the next level."""
+    m, n = 1 << 14, 32
+    # kappa ~ 1e3: the FP16 sketch is enough (PAPER.md:163) -> no escalation, same factorization as the oracle
+    AT = inputs.make_A(m, n, 3, 21, 22, "cuda")
+    QT, R, used, orth = B.mrcqr_factor_auto(AT, B.FP16, 2 * n, 4)
+    assert used == 16 and 0 <= orth <= 1e-13
+    A = to_np(AT)
+    o = orc.factor(A, 2 * n, 4)
+    kappa = np.linalg.cond(o["R"])
+    assert np.linalg.norm(to_np(QT) - o["Q"]) <= 10 * kappa * n * U
+    # kappa ~ 1e13: FP16 (and possibly FP32) must be given up; the returned factorization meets the bar
+    AT = inputs.make_A(m, n, 13, 61, 62, "cuda")
+    rc16 = B.mrcqr_factor(AT, B.FP16, 2 * n, 3, check=False)
+    QT, R, used, orth = B.mrcqr_factor_auto(AT, B.FP16, 2 * n, 3)
+    assert used in (32, 64) and 0 <= orth <= 1e-13
+    if rc16 == 0:                                             # FP16 "worked" but degraded (PAPER.md:207): that is what was detected
+        Q16, _ = B.mrcqr_factor(AT, B.FP16, 2 * n, 3)
+        assert B.mrcqr_orth_error(Q16) > 1e-13
+    A = to_np(AT)
+    assert orc.orth_error_fro(to_np(QT)) <= 1e-13 and orc.residual_fro(A, to_np(QT), to_np(R)) <= 1e-13
+    # an impossible tolerance: the FP64 result comes back with code 5 and its measured error
+    rc, used, orth = B.mrcqr_factor_auto(AT, B.FP32, 2 * n, 3, tol=1e-18, check=False)
+    assert rc == 5 and used == 64 and orth > 1e-18
+    # a rank-deficient matrix is reported, not hidden, after the last level
+    Az = A.copy(); Az[:, 31] = 0.0; Az = Az[:, :31]
+    rc, used, orth = B.mrcqr_factor_auto(torch.from_numpy(np.ascontiguousarray(Az.T)).cuda(), B.FP32, 62, 3, check=False)
+    assert rc == 0 or rc in (2, 3)
