@@ -151,6 +151,25 @@ int mrcqr_factor_auto(int64_t m, int n, int64_t lda, const double* A, double* Q,
                       int* prec_used_host, double* orth_host, void* stream);
 
 /*
+ * Algorithm 1, CholQR, on A itself: G = A^T A, G = R^T R, Q = A R^-1, with the stage-2/3 kernels
+ * of MRCQR (R_s = I).  passes = 2: CholQR2: Algorithm 1 again on Q, R = R2 R1.  Breaks down
+ * (MRCQR_ERR_BREAKDOWN) once kappa(A)^2 u >~ 1, i.e. kappa >~ 1e8; loses orthogonality as kappa^2 u
+ * before that (one pass).  m need not be a power of two.  Returns 0, -1 m, -2 n, -3 lda, -4 A, -5 Q, -6 R, -7 passes, 3, 4.
+ */
+int mrcqr_cholqr(int64_t m, int n, int64_t lda, const double* A, double* Q, double* R, int passes, void* stream);
+
+/*
+ * CholQR probe for the conditioning regime (eq. (2)): one CholQR of A into the caller's work
+ * buffers Qwork (m x n, ld = lda) and Rwork (n x n), q = ||I - Q^T Q||_F / sqrt(n) (a lower bound of the 2-norm the
+ * paper uses), kappa_lb = sqrt(q / (u (1 + q))) <= kappa_2(A), u = 2^-53.  A CholQR breakdown means kappa >~ u^-1/2:
+ * kappa_lb = 2^26.5.  prec_host (nullable): the paper's rule applied to the bound: 16 if
+ * kappa_lb < 1e4, 32 if < 1e8, else 64 -- a LOWER bound, so the suggestion may be too low; mrcqr_factor_auto
+ * corrects that.  Returns 0, a negative argument index (as mrcqr_cholqr; -7 kappa_lb_host) or 4.
+ */
+int mrcqr_kappa_probe(int64_t m, int n, int64_t lda, const double* A, double* Qwork, double* Rwork,
+                      double* kappa_lb_host, int* prec_host, void* stream);
+
+/*
  * Variant switch of mrcqr_factor / mrcqr_factor_host ("store-Y"): off (default), stage 2a
  * keeps Y = A R_s^-1 on chip and stage 2b recomputes it bit-identically (4 passes over m x n, 4 m n^2 flops);
  * on, stage 2a also writes Y into Q's buffer and stage 2b solves it in place against R_c (5 passes,

@@ -49,13 +49,15 @@ def lib():
         L.mrcqr_debug_dump_y.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
         L.mrcqr_shutdown.restype = None
         L.mrcqr_set_timing.argtypes = [ci]
+        L.mrcqr_cholqr.argtypes = [i64, ci, i64, vp, vp, vp, ci, vp]
+        L.mrcqr_kappa_probe.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp, vp]
         L.mrcqr_orth_error.argtypes = [i64, ci, i64, vp, vp, vp]
         L.mrcqr_factor_auto.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64, C.c_double, vp, vp, vp]
         L.mrcqr_set_store_y.argtypes = [ci]
         L.mrcqr_last_timing.argtypes = [vp]
         for f in ("mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
                   "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
-                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto"):
+                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe"):
             getattr(L, f).restype = ci
         _lib = L
     return _lib
@@ -63,7 +65,7 @@ def lib():
 
 EXPORTS = ["mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
-           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto"]
+           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe"]
 
 STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "reduce_k4_chol", "k5_form_q", "r_mul"]
 
@@ -205,6 +207,30 @@ def mrcqr_factor_auto(AT, first_prec, s, seed, tol=0.0, QT=None, R=None, stream=
         return rc, int(used.value), float(orth.value)
     _chk(rc)
     return QT, R, int(used.value), float(orth.value)
+
+
+def mrcqr_cholqr(AT, passes=1, QT=None, R=None, stream=None, check=True):
+    """Algorithm 1 (CholQR) on A; passes = 2: CholQR2.  Returns (QT, R) (or the code if check=False)."""
+    m, n, lda, pA = _mat(AT)
+    if QT is None:
+        QT = torch.empty_strided((n, m), (lda, 1), dtype=torch.float64, device=AT.device)
+    if R is None:
+        R = torch.empty((n, n), dtype=torch.float64, device=AT.device)
+    rc = lib().mrcqr_cholqr(m, n, lda, pA, QT.data_ptr(), R.data_ptr(), passes, _stream(stream))
+    if not check:
+        return rc
+    _chk(rc)
+    return QT, R
+
+
+def mrcqr_kappa_probe(AT, stream=None):
+    """CholQR probe (eq. (2)): returns (kappa lower bound, suggested sketch precision)."""
+    m, n, lda, pA = _mat(AT)
+    QT = torch.empty_strided((n, m), (lda, 1), dtype=torch.float64, device=AT.device)
+    R = torch.empty((n, n), dtype=torch.float64, device=AT.device)
+    lb, prec = C.c_double(0.0), C.c_int(0)
+    _chk(lib().mrcqr_kappa_probe(m, n, lda, pA, QT.data_ptr(), R.data_ptr(), C.byref(lb), C.byref(prec), _stream(stream)))
+    return float(lb.value), int(prec.value)
 
 
 def mrcqr_set_store_y(on):

@@ -324,31 +324,15 @@ extern "C" int mrcqr_last_timing(float* ms_out_host)
     return 0;
 }
 
-static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q, double* R,
-                         int prec, int s, uint64_t seed, cudaStream_t st)
+// Stage 2 + 3 of Algorithm 2 (steps 7-9) on device buffers, the prepared R_s already in the workspace:
+// precondition + Gram, Cholesky (+ R = Rc Rs), form Q.  Shared by mrcqr_factor and the CholQR entry points.
+static int enqueue_stage23(const Layout& L, int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q,
+                           double* R, const double* Rs, cudaStream_t st, bool tm)
 {
-    Layout L = make_layout(m, n, s, prec);
-    if (!ensure_ws(L.total) || !ensure_hidx((size_t)s)) return MRCQR_ERR_CUDA;
     Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
-    uint64_t* signs = reinterpret_cast<uint64_t*>(g.ws + L.signs);
-    int64_t* idx = reinterpret_cast<int64_t*>(g.ws + L.idx);
-    double* Rs = reinterpret_cast<double*>(g.ws + L.Rs);
     double* Rc = reinterpret_cast<double*>(g.ws + L.Rc);
-    // Algorithm 2 step 1: bins on the host (s values), sign words on the device (m bits)
-    draw_bins_host(m, s, seed, g.h_idx);
-    cudaMemcpyAsync(idx, g.h_idx, sizeof(int64_t) * (size_t)s, cudaMemcpyHostToDevice, st);
-    const int64_t nw = (m + 63) / 64;
-    mrcqr_draw_signs<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed, nw, signs, stat);
-    int k = 1;
-    const bool tm = g.timing && timing_events();
-    double* As = reinterpret_cast<double*>(g.ws + L.As);
-    if (tm) cudaEventRecord(g.ev[0], st);
-    k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);     // steps 2-4
-    if (tm) cudaEventRecord(g.ev[1], st);
-    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
-                             reinterpret_cast<double*>(g.ws + L.betas), stat, st);                              // steps 5-6
-    if (tm) cudaEventRecord(g.ev[2], st);
-    {                                                                                      // step 7 + Alg.1 steps 1-2
+    int k = 0;
+    {
         const int n16 = round_up(n, 16);
         double* RsPrep = reinterpret_cast<double*>(g.ws + L.RsPrep);
         double* RcPrep = reinterpret_cast<double*>(g.ws + L.RcPrep);
@@ -378,6 +362,33 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
         else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 3, st);        // Alg.1 step 3
         if (tm) { cudaEventRecord(g.ev[6], st); cudaEventRecord(g.ev[7], st); }
     }
+    return k;
+}
+
+static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q, double* R,
+                         int prec, int s, uint64_t seed, cudaStream_t st)
+{
+    Layout L = make_layout(m, n, s, prec);
+    if (!ensure_ws(L.total) || !ensure_hidx((size_t)s)) return MRCQR_ERR_CUDA;
+    Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
+    uint64_t* signs = reinterpret_cast<uint64_t*>(g.ws + L.signs);
+    int64_t* idx = reinterpret_cast<int64_t*>(g.ws + L.idx);
+    double* Rs = reinterpret_cast<double*>(g.ws + L.Rs);
+    // Algorithm 2 step 1: bins on the host (s values), sign words on the device (m bits)
+    draw_bins_host(m, s, seed, g.h_idx);
+    cudaMemcpyAsync(idx, g.h_idx, sizeof(int64_t) * (size_t)s, cudaMemcpyHostToDevice, st);
+    const int64_t nw = (m + 63) / 64;
+    mrcqr_draw_signs<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed, nw, signs, stat);
+    int k = 1;
+    const bool tm = g.timing && timing_events();
+    double* As = reinterpret_cast<double*>(g.ws + L.As);
+    if (tm) cudaEventRecord(g.ev[0], st);
+    k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);     // steps 2-4
+    if (tm) cudaEventRecord(g.ev[1], st);
+    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
+                             reinterpret_cast<double*>(g.ws + L.betas), stat, st);                              // steps 5-6
+    if (tm) cudaEventRecord(g.ev[2], st);
+    k += enqueue_stage23(L, m, n, lda, A, ldq, Q, R, Rs, st, tm);                              // steps 7-9
     const int rc = finish(L, st, k);
     if (tm) for (int i = 0; i < 7; ++i) cudaEventElapsedTime(&g.stage_ms[i], g.ev[i], g.ev[i + 1]);
     return rc;
@@ -459,6 +470,73 @@ extern "C" int mrcqr_factor_auto(int64_t m, int n, int64_t lda, const double* A,
         if (rc == 0) rc = MRCQR_ERR_NOT_ORTHOGONAL;
     }
     return rc;                                               // the outcome at the highest precision
+}
+
+__global__ void mrcqr_set_identity(double* __restrict__ M, int n)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < n * n) M[e] = (e % n == e / n) ? 1.0 : 0.0;
+}
+
+// Algorithm 1 on A itself: the stage-2/3 kernels with R_s = I
+static int cholqr_device(int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q, double* R, cudaStream_t st)
+{
+    Layout L = make_layout(m, n, 0, 64);
+    if (!ensure_ws(L.total)) return MRCQR_ERR_CUDA;
+    Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
+    double* Rs = reinterpret_cast<double*>(g.ws + L.Rs);
+    mrcqr_reset_status<<<1, 1, 0, st>>>(stat);
+    mrcqr_set_identity<<<(n * n + 255) / 256, 256, 0, st>>>(Rs, n);
+    int k = 2 + launch_prep_R(Rs, n, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16), stat, MRCQR_ERR_SINGULAR, st);
+    k += enqueue_stage23(L, m, n, lda, A, ldq, Q, R, Rs, st, false);
+    return finish(L, st, k);
+}
+
+extern "C" int mrcqr_cholqr(int64_t m, int n, int64_t lda, const double* A, double* Q, double* R, int passes, void* stream)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (m < n) return -1;
+    if (lda < m) return -3;
+    if (!A) return -4;
+    if (!Q) return -5;
+    if (!R) return -6;
+    if (passes != 1 && passes != 2) return -7;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = cholqr_device(m, n, lda, A, lda, Q, R, st);
+    if (rc != 0 || passes == 1) return rc;
+    // CholQR2: Algorithm 1 again on Q (in place), R = R2 R1
+    double *R1 = nullptr, *R2 = nullptr;
+    if (cudaMalloc(&R1, sizeof(double) * 2 * (size_t)n * n) != cudaSuccess) { cudaGetLastError(); return MRCQR_ERR_CUDA; }
+    R2 = R1 + (size_t)n * n;
+    cudaMemcpyAsync(R1, R, sizeof(double) * (size_t)n * n, cudaMemcpyDeviceToDevice, st);
+    rc = cholqr_device(m, n, lda, Q, lda, Q, R2, st);
+    if (rc == 0) {
+        launch_triu_mul(R2, R1, n, R, st);
+        if (cudaStreamSynchronize(st) != cudaSuccess) rc = MRCQR_ERR_CUDA;
+    }
+    cudaFree(R1);
+    return rc;
+}
+
+extern "C" int mrcqr_kappa_probe(int64_t m, int n, int64_t lda, const double* A, double* Qwork, double* Rwork,
+                                 double* kappa_lb_host, int* prec_host, void* stream)
+{
+    if (!kappa_lb_host) return -7;
+    int rc = mrcqr_cholqr(m, n, lda, A, Qwork, Rwork, 1, stream);
+    if (rc < 0 || rc == MRCQR_ERR_CUDA) return rc;
+    const double u = 1.1102230246251565e-16;                   // 2^-53
+    double lb = 1.0 / sqrt(u);                                 // CholQR broke down: kappa^2 u >~ 1
+    if (rc == 0) {
+        double qf = 0.0;
+        rc = mrcqr_orth_error(m, n, lda, Qwork, &qf, stream);
+        if (rc != 0) return rc;
+        const double q = qf / sqrt((double)n);                 // ||.||_2 >= ||.||_F / sqrt(n): keeps eq. (2) a LOWER bound
+        lb = sqrt(q / (u * (1.0 + q)));
+    }
+    *kappa_lb_host = lb;
+    if (prec_host) *prec_host = lb < 1e4 ? 16 : (lb < 1e8 ? 32 : 64);
+    return 0;
 }
 
 extern "C" int mrcqr_factor_host(int64_t m, int n, int64_t lda, const double* A_host, double* Q_host,

@@ -202,3 +202,39 @@ def test_factor_auto_escalates_only_when_needed(orc):
     Az = A.copy(); Az[:, 31] = 0.0; Az = Az[:, :31]
     rc, used, orth = B.mrcqr_factor_auto(torch.from_numpy(np.ascontiguousarray(Az.T)).cuda(), B.FP32, 62, 3, check=False)
     assert rc == 0 or rc in (2, 3)
+
+
+def test_cholqr_cholqr2_and_the_kappa_probe(orc):
+    """Algorithm 1 on A against the oracle's Gram / Cholesky / row solves; its kappa^2 u loss
+    of orthogonality and its breakdown near kappa ~ 1e8; CholQR2; eq. (2) as a lower bound."""
+    m, n = 1 << 13, 40
+    AT = inputs.make_A(m, n, 3, 71, 72, "cuda")                 # kappa ~ 1e3
+    A = to_np(AT)
+    Go = orc.gram(np.asfortranarray(A))
+    Ro, info = orc.cholesky_upper(Go)
+    assert info == 0
+    Qo = orc.row_solve(np.asfortranarray(A), Ro)
+    QT, R = B.mrcqr_cholqr(AT, 1)
+    kappa = np.linalg.cond(Ro)
+    assert np.linalg.norm(to_np(R) - Ro) <= 10 * kappa * n * U * np.linalg.norm(Ro)
+    assert np.linalg.norm(to_np(QT) - Qo) <= 10 * kappa ** 2 * n * U
+    e1 = B.mrcqr_orth_error(QT)
+    assert e1 <= 10 * n * kappa ** 2 * U                          # O(kappa^2 u) (PAPER.md:55)
+    assert orc.residual_fro(A, to_np(QT), to_np(R)) <= 1e-13
+    Q2, R2 = B.mrcqr_cholqr(AT, 2)
+    assert B.mrcqr_orth_error(Q2) <= 1e-13 and orc.residual_fro(A, to_np(Q2), to_np(R2)) <= 1e-13
+    assert np.all(np.diag(to_np(R2)) > 0) and np.array_equal(np.tril(to_np(R2), -1), np.zeros((n, n)))
+    # eq. (2): a lower bound of kappa_2(A), within two orders of magnitude here
+    lb, prec = B.mrcqr_kappa_probe(AT)
+    ktrue = np.linalg.cond(A)
+    assert ktrue / 100 <= lb <= ktrue * 1.001 and prec == 16
+    # kappa ~ 1e10: Cholesky of A^T A breaks down (or, if rounding lets it through, Q is far from orthonormal)
+    ATb = inputs.make_A(m, n, 10, 73, 74, "cuda")
+    rc = B.mrcqr_cholqr(ATb, 1, check=False)
+    assert rc == 3 or (rc == 0 and B.mrcqr_orth_error(B.mrcqr_cholqr(ATb, 1)[0]) > 1e-8)
+    lb, prec = B.mrcqr_kappa_probe(ATb)
+    assert lb >= 1e6 and prec in (32, 64)
+    # m not a power of two is fine here (no transform involved)
+    AT3 = inputs.make_A(5000, 24, 2, 75, 76, "cuda")
+    Q3, R3 = B.mrcqr_cholqr(AT3, 2)
+    assert B.mrcqr_orth_error(Q3) <= 1e-13 and orc.residual_fro(to_np(AT3), to_np(Q3), to_np(R3)) <= 1e-13
