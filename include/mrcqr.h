@@ -179,6 +179,15 @@ int mrcqr_kappa_probe(int64_t m, int n, int64_t lda, const double* A, double* Qw
 int mrcqr_set_store_y(int on);
 
 /*
+ * Repeated-call mode (block Arnoldi, randomized-SVD power iteration, time stepping): on, the
+ * kernels, copies and the status read-back of mrcqr_factor are captured ONCE into a CUDA graph per (m, n, lda, A, Q, R,
+ * precision, s) and replayed by later calls with the same arguments; the seed and the drawn bins are data of the graph
+ * (read from pinned host memory at replay), so they may change from call to call.  Same results bit for bit.  Per-kernel
+ * timing (mrcqr_set_timing) takes the ordinary path.  Returns 0.
+ */
+int mrcqr_set_graph(int on);
+
+/*
  * Test hook for the "bit-identical Y" requirement: runs the stage-2a and the stage-2b
  * tile solves and dumps the Y = A R_s^-1 each of them computed (m x n, ld = m).  The two dumps
  * must be equal bit for bit.

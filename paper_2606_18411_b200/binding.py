@@ -54,10 +54,11 @@ def lib():
         L.mrcqr_orth_error.argtypes = [i64, ci, i64, vp, vp, vp]
         L.mrcqr_factor_auto.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64, C.c_double, vp, vp, vp]
         L.mrcqr_set_store_y.argtypes = [ci]
+        L.mrcqr_set_graph.argtypes = [ci]
         L.mrcqr_last_timing.argtypes = [vp]
         for f in ("mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
                   "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
-                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe"):
+                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph"):
             getattr(L, f).restype = ci
         _lib = L
     return _lib
@@ -65,7 +66,7 @@ def lib():
 
 EXPORTS = ["mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
-           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe"]
+           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph"]
 
 STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "reduce_k4_chol", "k5_form_q", "r_mul"]
 
@@ -231,6 +232,11 @@ def mrcqr_kappa_probe(AT, stream=None):
     lb, prec = C.c_double(0.0), C.c_int(0)
     _chk(lib().mrcqr_kappa_probe(m, n, lda, pA, QT.data_ptr(), R.data_ptr(), C.byref(lb), C.byref(prec), _stream(stream)))
     return float(lb.value), int(prec.value)
+
+
+def mrcqr_set_graph(on):
+    """Repeated-call mode: mrcqr_factor replays a CUDA graph captured per (shape, buffers)."""
+    lib().mrcqr_set_graph(1 if on else 0)
 
 
 def mrcqr_set_store_y(on):

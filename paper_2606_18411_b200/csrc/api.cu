@@ -27,6 +27,15 @@ __global__ void mrcqr_draw_signs(uint64_t seed, int64_t nwords, uint64_t* __rest
 
 __global__ void mrcqr_reset_status(Status* st) { st->code = 0; st->info = 0; }
 
+// same as mrcqr_draw_signs with the seed read from device memory (graph replay: the seed is data, not a launch parameter)
+__global__ void mrcqr_draw_signs_p(const uint64_t* __restrict__ seedp, int64_t nwords, uint64_t* __restrict__ signs, Status* st)
+{
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t seed = *seedp;
+    if (w == 0 && st) { st->code = 0; st->info = 0; }
+    if (w < nwords) signs[w] = splitmix64_at(seed, (uint64_t)w);
+}
+
 static void draw_bins_host(int64_t m, int s, uint64_t seed, int64_t* idx)
 {
     const uint64_t nw = (uint64_t)((m + 63) / 64), B = (uint64_t)(m / 2 + 1);
@@ -78,8 +87,17 @@ struct Ctx {
     bool timing = false; cudaEvent_t ev[8] = {}; bool ev_ok = false; float stage_ms[8] = {};
     bool have_device = false, probed = false;
     bool store_y = false;                    // mrcqr_set_store_y: store-Y variant also for n16 <= 128
+    // mrcqr_set_graph: the whole enqueue sequence of mrcqr_factor captured once per (shape, buffers) and replayed
+    bool use_graph = false;
+    cudaGraphExec_t gexec = nullptr; int glaunches = 0; uint64_t* h_seed = nullptr;
+    struct { int64_t m, lda; int n, prec, s; const void *A, *Q, *R, *ws, *hidx; bool store_y; } gkey = {};
 };
 static Ctx g;
+
+static void drop_graph()
+{
+    if (g.gexec) { cudaGraphExecDestroy(g.gexec); g.gexec = nullptr; }
+}
 
 static bool device_ok()
 {
@@ -96,7 +114,7 @@ static bool ensure_ws(size_t bytes)
 {
     if (!g.h_status && cudaMallocHost(&g.h_status, 64) != cudaSuccess) return false;   // [0..1] status, [2..3] a double
     if (bytes <= g.ws_bytes) return true;
-    if (g.ws) { cudaDeviceSynchronize(); cudaFree(g.ws); g.ws = nullptr; g.ws_bytes = 0; }
+    if (g.ws) { cudaDeviceSynchronize(); drop_graph(); cudaFree(g.ws); g.ws = nullptr; g.ws_bytes = 0; }
     if (cudaMalloc(&g.ws, bytes) != cudaSuccess) { cudaGetLastError(); return false; }
     g.ws_bytes = bytes;
     return true;
@@ -208,6 +226,8 @@ extern "C" void mrcqr_shutdown(void)
 {
     if (!g.probed || !g.have_device) return;
     cudaDeviceSynchronize();
+    drop_graph();
+    if (g.h_seed) cudaFreeHost(g.h_seed);
     if (g.ws) cudaFree(g.ws);
     if (g.h_status) cudaFreeHost(g.h_status);
     if (g.h_idx) cudaFreeHost(g.h_idx);
@@ -316,6 +336,7 @@ static bool timing_events()
 
 extern "C" int mrcqr_set_timing(int on) { g.timing = (on != 0); return 0; }
 extern "C" int mrcqr_set_store_y(int on) { g.store_y = (on != 0); return 0; }
+extern "C" int mrcqr_set_graph(int on) { g.use_graph = (on != 0); if (!on) drop_graph(); return 0; }
 
 extern "C" int mrcqr_last_timing(float* ms_out_host)
 {
@@ -365,22 +386,21 @@ static int enqueue_stage23(const Layout& L, int64_t m, int n, int64_t lda, const
     return k;
 }
 
-static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q, double* R,
-                         int prec, int s, uint64_t seed, cudaStream_t st)
+// enqueues steps 1-9 on st.  seed_dev != nullptr: the seed and the bins are read from seed_dev / the pinned
+// staging buffers when the work RUNS (graph capture); otherwise they are taken now.
+static int enqueue_factor(const Layout& L, int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q,
+                          double* R, int prec, int s, uint64_t seed, const uint64_t* seed_dev, cudaStream_t st, bool tm)
 {
-    Layout L = make_layout(m, n, s, prec);
-    if (!ensure_ws(L.total) || !ensure_hidx((size_t)s)) return MRCQR_ERR_CUDA;
     Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
     uint64_t* signs = reinterpret_cast<uint64_t*>(g.ws + L.signs);
     int64_t* idx = reinterpret_cast<int64_t*>(g.ws + L.idx);
     double* Rs = reinterpret_cast<double*>(g.ws + L.Rs);
     // Algorithm 2 step 1: bins on the host (s values), sign words on the device (m bits)
-    draw_bins_host(m, s, seed, g.h_idx);
     cudaMemcpyAsync(idx, g.h_idx, sizeof(int64_t) * (size_t)s, cudaMemcpyHostToDevice, st);
     const int64_t nw = (m + 63) / 64;
-    mrcqr_draw_signs<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed, nw, signs, stat);
+    if (seed_dev) mrcqr_draw_signs_p<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed_dev, nw, signs, stat);
+    else mrcqr_draw_signs<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed, nw, signs, stat);
     int k = 1;
-    const bool tm = g.timing && timing_events();
     double* As = reinterpret_cast<double*>(g.ws + L.As);
     if (tm) cudaEventRecord(g.ev[0], st);
     k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);     // steps 2-4
@@ -389,6 +409,49 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
                              reinterpret_cast<double*>(g.ws + L.betas), stat, st);                              // steps 5-6
     if (tm) cudaEventRecord(g.ev[2], st);
     k += enqueue_stage23(L, m, n, lda, A, ldq, Q, R, Rs, st, tm);                              // steps 7-9
+    return k;
+}
+
+static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q, double* R,
+                         int prec, int s, uint64_t seed, cudaStream_t st)
+{
+    Layout L = make_layout(m, n, s, prec);
+    if (!ensure_ws(L.total) || !ensure_hidx((size_t)s)) return MRCQR_ERR_CUDA;
+    draw_bins_host(m, s, seed, g.h_idx);
+    const bool tm = g.timing && timing_events();
+    if (g.use_graph && !tm) {
+        if (!g.h_seed && cudaMallocHost(&g.h_seed, 64) != cudaSuccess) { cudaGetLastError(); g.h_seed = nullptr; }
+        const bool same = g.gexec && g.gkey.m == m && g.gkey.lda == lda && g.gkey.n == n && g.gkey.prec == prec &&
+                          g.gkey.s == s && g.gkey.A == A && g.gkey.Q == Q && g.gkey.R == R && g.gkey.ws == g.ws &&
+                          g.gkey.hidx == g.h_idx && g.gkey.store_y == g.store_y;
+        if (g.h_seed && !same) {
+            drop_graph();
+            uint64_t* seed_dev = reinterpret_cast<uint64_t*>(g.ws + L.status) + 2;        // Status::pad
+            cudaGraph_t graph = nullptr;
+            if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                cudaMemcpyAsync(seed_dev, g.h_seed, sizeof(uint64_t), cudaMemcpyHostToDevice, st);
+                g.glaunches = enqueue_factor(L, m, n, lda, A, ldq, Q, R, prec, s, 0, seed_dev, st, false);
+                cudaMemcpyAsync(g.h_status, g.ws + L.status, 8, cudaMemcpyDeviceToHost, st);
+                if (cudaStreamEndCapture(st, &graph) != cudaSuccess || !graph ||
+                    cudaGraphInstantiate(&g.gexec, graph, 0) != cudaSuccess) g.gexec = nullptr;
+                if (graph) cudaGraphDestroy(graph);
+            }
+            cudaGetLastError();
+            if (g.gexec) {
+                g.gkey.m = m; g.gkey.lda = lda; g.gkey.n = n; g.gkey.prec = prec; g.gkey.s = s; g.gkey.A = A; g.gkey.Q = Q;
+                g.gkey.R = R; g.gkey.ws = g.ws; g.gkey.hidx = g.h_idx; g.gkey.store_y = g.store_y;
+            }
+        }
+        if (g.gexec) {
+            *g.h_seed = seed;
+            g.last_launches = g.glaunches;
+            if (cudaGraphLaunch(g.gexec, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess ||
+                cudaGetLastError() != cudaSuccess) return MRCQR_ERR_CUDA;
+            g.last_info = g.h_status[1];
+            return g.h_status[0];
+        }
+    }
+    const int k = enqueue_factor(L, m, n, lda, A, ldq, Q, R, prec, s, seed, nullptr, st, tm);
     const int rc = finish(L, st, k);
     if (tm) for (int i = 0; i < 7; ++i) cudaEventElapsedTime(&g.stage_ms[i], g.ev[i], g.ev[i + 1]);
     return rc;

