@@ -13,6 +13,7 @@
 // flushed to the CTA's partial every 1024 rows (reading R7); a reduction kernel adds the
 // partials of a block in a fixed order.  No atomics: bit-reproducible.
 #include "mrcqr_internal.cuh"
+#include "gram_roles.cuh"
 
 namespace mrcqr {
 
@@ -34,10 +35,36 @@ __device__ __forceinline__ void sy_cp16(void* dst, const void* src, int bytes)
 
 struct SyrkParams {
     int64_t m, ldy;
-    int n, n16, P, pairs, ksplit;
-    int64_t rows_per_split;           // multiple of SY_KC
+    int n, n16, P, pairs;
+    int ks_diag, ks_off;              // row ranges per diagonal / off-diagonal block (a diagonal block costs 18/32)
+    int64_t rows_diag, rows_off;      // rows per range, multiples of SY_KC
     int vec;
 };
+
+// CTA b -> (pair, range index); CTAs are ordered by pair, a pair owns ks_diag or ks_off consecutive CTAs
+__host__ __device__ __forceinline__ void sy_locate(const SyrkParams& p, int b, int& pair, int& ks_id, int& ks_n)
+{
+    int off = 0;
+    for (int q = 0; q < p.pairs; ++q) {
+        int j = 0;
+        while ((j + 1) * (j + 2) / 2 <= q) ++j;
+        const int i = q - j * (j + 1) / 2;
+        const int k = (i == j) ? p.ks_diag : p.ks_off;
+        if (b < off + k) { pair = q; ks_id = b - off; ks_n = k; return; }
+        off += k;
+    }
+    pair = p.pairs - 1; ks_id = 0; ks_n = 1;
+}
+__host__ __device__ __forceinline__ int sy_pair_offset(const SyrkParams& p, int pair)
+{
+    int off = 0;
+    for (int q = 0; q < pair; ++q) {
+        int j = 0;
+        while ((j + 1) * (j + 2) / 2 <= q) ++j;
+        off += (q - j * (j + 1) / 2 == j) ? p.ks_diag : p.ks_off;
+    }
+    return off;
+}
 
 __device__ __forceinline__ void sy_pair(int p, int& I, int& J)      // p -> (I <= J), column-major over the upper triangle
 {
@@ -80,25 +107,20 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
     extern __shared__ __align__(16) double sy_sm[];        // [3 stages][2 panels][128 * SY_LD]
     constexpr int PAN = SY_B * SY_LD;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-    const int pair = blockIdx.x / p.ksplit, ks_id = blockIdx.x % p.ksplit;
+    int pair, ks_id, ks_n;
+    sy_locate(p, blockIdx.x, pair, ks_id, ks_n);
     int I, J;
     sy_pair(pair, I, J);
     const bool diag = (I == J);
     const int wi = warp & 3, wj = warp >> 2;
-    const bool skip = diag && (32 * wi >= 64 * wj + 64);    // sub-block strictly below the diagonal
     const int64_t mpad = (p.m + SY_KC - 1) / SY_KC * SY_KC;
-    const int64_t k0 = (int64_t)ks_id * p.rows_per_split;
-    int64_t k1 = k0 + p.rows_per_split;
+    const int64_t rps = diag ? p.rows_diag : p.rows_off;
+    const int64_t k0 = (int64_t)ks_id * rps;
+    int64_t k1 = k0 + rps;
     if (k1 > mpad) k1 = mpad;
     const int nchunks = k1 > k0 ? (int)((k1 - k0) / SY_KC) : 0;
     double* part = partials + (size_t)blockIdx.x * SY_B * SY_B;
 
-    double acc[4][8][2];
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-        for (int b = 0; b < 8; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
-    bool first = true;
     unsigned maskI = 0, maskJ = 0;
 #pragma unroll
     for (int k = 0; k < SY_B / 16; ++k) {
@@ -111,32 +133,63 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
         if (!diag) sy_load_panel(st + PAN, p, Y, J, k0 + (int64_t)c * SY_KC, tid, maskJ);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    auto flush = [&]() {
-        if (!skip) {
-#pragma unroll
-            for (int a = 0; a < 4; ++a)
-#pragma unroll
-                for (int b = 0; b < 8; ++b) {
-                    double* dst = part + (size_t)(64 * wj + 8 * b + 2 * t) * SY_B + 32 * wi + 8 * a + g;
-                    if (first) { dst[0] = acc[a][b][0]; dst[SY_B] = acc[a][b][1]; }
-                    else { dst[0] += acc[a][b][0]; dst[SY_B] += acc[a][b][1]; }
-                    acc[a][b][0] = acc[a][b][1] = 0.0;
-                }
-        }
-        first = false;
-    };
     // three stages, ONE barrier per chunk: the barrier of iteration c also proves that every warp is done
     // with chunk c-1, whose stage chunk c+2 is about to overwrite
     if (nchunks > 0) issue(0);
     if (nchunks > 1) issue(1);
+    bool first = true;
+    if (diag) {
+        // diagonal block: only the upper triangle, 136 8x8 blocks split 18,18,18,18,16,16,16,16 over the warps
+        // (gram_roles.cuh, the ownership table of K3 at n = 128)
+        constexpr int MAXOWN = gram_maxown<16, 8>();
+        double acc[MAXOWN][2];
+#pragma unroll
+        for (int b = 0; b < MAXOWN; ++b) acc[b][0] = acc[b][1] = 0.0;
+        for (int c = 0; c < nchunks; ++c) {
+            if (c + 1 < nchunks) asm volatile("cp.async.wait_group 1;" ::: "memory");
+            else asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncthreads();
+            if (c + 2 < nchunks) issue(c + 2);
+            const double* pI = sy_sm + (size_t)(c % 3) * 2 * PAN;
+            const bool fl = ((c + 1) % SY_FLUSH == 0 || c + 1 == nchunks);
+#define SY_ROLE(R_) { gram_accumulate<16, 8, R_, SY_KC, 1, MAXOWN>(acc, pI, 0, lane); \
+                      if (fl) gram_flush<16, 8, R_, MAXOWN>(acc, part, SY_B, first, lane); }
+            switch (warp) {
+                case 0: SY_ROLE(0) break; case 1: SY_ROLE(1) break; case 2: SY_ROLE(2) break; case 3: SY_ROLE(3) break;
+                case 4: SY_ROLE(4) break; case 5: SY_ROLE(5) break; case 6: SY_ROLE(6) break; default: SY_ROLE(7) break;
+            }
+#undef SY_ROLE
+            if (fl) first = false;
+        }
+        if (nchunks == 0)                            // an empty range still owns a (zero) partial
+            for (int e = tid; e < SY_B * SY_B; e += SY_THREADS) part[e] = 0.0;
+        return;
+    }
+    double acc[4][8][2];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 8; ++b) acc[a][b][0] = acc[a][b][1] = 0.0;
+    auto flush = [&]() {
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 8; ++b) {
+                double* dst = part + (size_t)(64 * wj + 8 * b + 2 * t) * SY_B + 32 * wi + 8 * a + g;
+                if (first) { dst[0] = acc[a][b][0]; dst[SY_B] = acc[a][b][1]; }
+                else { dst[0] += acc[a][b][0]; dst[SY_B] += acc[a][b][1]; }
+                acc[a][b][0] = acc[a][b][1] = 0.0;
+            }
+        first = false;
+    };
     for (int c = 0; c < nchunks; ++c) {
         if (c + 1 < nchunks) asm volatile("cp.async.wait_group 1;" ::: "memory");
         else asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();
         if (c + 2 < nchunks) issue(c + 2);
-        if (!skip) {
+        {
             const double* pI = sy_sm + (size_t)(c % 3) * 2 * PAN;
-            const double* pJ = diag ? pI : pI + PAN;
+            const double* pJ = pI + PAN;
             const double* fi = pI + (32 * wi + g) * SY_LD + t;
             const double* fj = pJ + (64 * wj + g) * SY_LD + t;
 #pragma unroll 2
@@ -170,9 +223,10 @@ mrcqr_syrk_reduce(SyrkParams p, const double* __restrict__ partials, double* __r
     const int i = e % SY_B, j = e / SY_B;
     const int gi = SY_B * I + i, gj = SY_B * J + j;
     const bool live = gi <= gj && gj < p.n16;
+    const int ksn = (I == J) ? p.ks_diag : p.ks_off, base = sy_pair_offset(p, pair);
     double total = 0.0;
     if (live)
-        for (int c = q; c < p.ksplit; c += 32) total += partials[((size_t)pair * p.ksplit + c) * SY_B * SY_B + e];
+        for (int c = q; c < ksn; c += 32) total += partials[((size_t)base + c) * SY_B * SY_B + e];
     sm[q][el] = total;
     __syncthreads();
 #pragma unroll
@@ -193,12 +247,17 @@ static SyrkParams syrk_params(int64_t m, int n, int n16)
     p.m = m; p.n = n; p.n16 = n16;
     p.P = (n16 + SY_B - 1) / SY_B;
     p.pairs = p.P * (p.P + 1) / 2;
-    int ks = num_sms() / p.pairs;
-    if (ks < 1) ks = 1;
+    const int pd = p.P, po = p.pairs - p.P, sms = num_sms();
     const int64_t chunks = (m + SY_KC - 1) / SY_KC;
-    if (ks > chunks) ks = (int)chunks;
-    p.ksplit = ks;
-    p.rows_per_split = (chunks + ks - 1) / ks * SY_KC;
+    int ko = po > 0 ? (int)(sms / (po + 0.5625 * pd)) : 0;
+    if (po > 0 && ko < 1) ko = 1;
+    int kd = (sms - po * ko) / pd;
+    if (kd < 1) kd = 1;
+    if (ko > chunks) ko = (int)chunks;
+    if (kd > chunks) kd = (int)chunks;
+    p.ks_diag = kd; p.ks_off = ko > 0 ? ko : 1;
+    p.rows_diag = (chunks + kd - 1) / kd * SY_KC;
+    p.rows_off = (chunks + p.ks_off - 1) / p.ks_off * SY_KC;
     return p;
 }
 
@@ -206,9 +265,7 @@ size_t syrk_partials_bytes(int n)
 {
     const int n16 = round_up(n, 16);
     const int P = (n16 + SY_B - 1) / SY_B, pairs = P * (P + 1) / 2;
-    int ks = num_sms() / pairs;
-    if (ks < 1) ks = 1;
-    return (size_t)pairs * ks * SY_B * SY_B * sizeof(double);
+    return (size_t)(num_sms() + pairs) * SY_B * SY_B * sizeof(double);      // one partial per CTA
 }
 
 // err[0] = || I - G ||_F for the symmetric n x n matrix held in G16 (upper triangle read), fixed summation order
@@ -246,7 +303,7 @@ int launch_syrk(int64_t m, int n, int64_t ldy, const double* Y, double* partials
     p.vec = ((uintptr_t)Y % 16 == 0) && (ldy % 2 == 0);
     const int smem = 3 * 2 * SY_B * SY_LD * (int)sizeof(double);
     cudaFuncSetAttribute(mrcqr_syrk, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    mrcqr_syrk<<<p.pairs * p.ksplit, SY_THREADS, smem, s>>>(p, Y, partials);
+    mrcqr_syrk<<<p.P * p.ks_diag + (p.pairs - p.P) * p.ks_off, SY_THREADS, smem, s>>>(p, Y, partials);
     mrcqr_syrk_reduce<<<p.pairs * (SY_B * SY_B / 32), 1024, 0, s>>>(p, partials, G16);
     return 2;
 }
