@@ -249,12 +249,20 @@ def run_ours(args):
 
     if rank == 0:
         hbm_peak, how = measured_peaks()
-        alg_bytes = 32.0 * m * n                       # 3 reads of A + 1 write of Q (north_star)
-        flops = 4.0 * m * n * n                        # 2 solves in K5, 1 solve + Gram in K3
-        # dominant kernel = the slower of K3 / K5; its algorithmic work
-        dom = "k5_form_q" if stages["k5_form_q"] >= stages["k3_gram"] else "k3_gram"
-        dom_flops = 2.0 * m * n * n
-        dom_bytes = (16.0 if dom == "k5_form_q" else 8.0) * m * n
+        panels = n > 128                               # store-Y panel passes + SYRK (n16 > 128)
+        if not panels:
+            alg_bytes = 32.0 * m * n                   # 3 reads of A + 1 write of Q (north_star)
+            flops = 4.0 * m * n * n                    # 2 solves in K5, 1 solve + Gram in K3
+            # dominant kernel = the slower of K3 / K5; its algorithmic work
+            dom = "k5_form_q" if stages["k5_form_q"] >= stages["k3_gram"] else "k3_gram"
+            dom_flops = 2.0 * m * n * n
+            dom_bytes = (16.0 if dom == "k5_form_q" else 8.0) * m * n
+        else:
+            alg_bytes = 40.0 * m * n                   # A read twice (K1, solve 1), Y written, read by SYRK, solved in place (r+w)
+            flops = 3.0 * m * n * n                    # two triangular solves + the symmetric Gram, m n^2 each
+            dom = "k5_form_q" if stages["k5_form_q"] >= stages["k3_gram"] else "k3_gram"   # one panel solve each here
+            dom_flops = 1.0 * m * n * n
+            dom_bytes = 16.0 * m * n
         dom_ms = stages[dom]
         t_hbm, t_f64 = dom_bytes / (hbm_peak * 1e9), dom_flops / (FP64_DMMA_PEAK_TFLOPS * 1e12)
         if t_f64 >= t_hbm:

@@ -61,10 +61,11 @@ struct K1Params {
     int64_t m2;
     int tiles_per_col, tiles_per_chunk, chunks;
     int vec;                      // A and lda allow 16-byte loads
+    int dtab;                     // the per-bin step twiddles W_m^k fit in shared memory (computed once per CTA)
 };
 
 template <typename T, int PREC>
-__global__ void __launch_bounds__(K1_NT, 3)
+__global__ void __launch_bounds__(K1_NT, sizeof(T) == 8 ? 2 : 3)      // FP64 tiles: two CTAs per SM by shared memory
 mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
               const int64_t* __restrict__ idx, double* __restrict__ partial)
 {
@@ -72,6 +73,7 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
     Cx<T>* tile = reinterpret_cast<Cx<T>*>(smraw);                       // [m1][32]
     Cx<T>* tw = tile + (size_t)p.m1 * K1_LD;                             // [m1]  W_m1^e
     double* colacc = reinterpret_cast<double*>(tw + p.m1);               // [2][s]
+    Cx<T>* dstep = reinterpret_cast<Cx<T>*>(colacc + 2 * p.s);           // [s]  (cos, sin) of 2 pi k_i / m   (dtab only)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int pair = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
     const int ja = 2 * pair, jb = 2 * pair + 1;
@@ -84,6 +86,13 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
         tw[e] = Cx<T>{(T)cs, (T)sn};
     }
     for (int e = tid; e < 2 * p.s; e += K1_NT) colacc[e] = 0.0;
+    if (p.dtab)
+        for (int i = tid; i < p.s; i += K1_NT) {
+            const int64_t k = idx[i];
+            Cx<T> d;
+            sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d.y, &d.x);
+            dstep[i] = d;
+        }
 
     const int tile_lo = chunk * p.tiles_per_chunk;
     const int tile_hi = min(p.tiles_per_col, tile_lo + p.tiles_per_chunk);
@@ -177,8 +186,9 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
             const Cx<T>* rowQ = tile + (size_t)brn * K1_LD;
             Cx<T> w0, d1, d8;                                  // (cos, sin) of 2 pi k t2_0 / m, 2 pi k / m, 2 pi 8k / m
             sincospi_t((T)(2.0 * (double)((k * t2_0) & (p.m - 1)) / (double)p.m), &w0.y, &w0.x);
-            sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d1.y, &d1.x);
-            sincospi_t((T)(2.0 * (double)((8 * k) & (p.m - 1)) / (double)p.m), &d8.y, &d8.x);
+            if (p.dtab) d1 = dstep[i];
+            else sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d1.y, &d1.x);
+            d8 = cmul(d1, d1); d8 = cmul(d8, d8); d8 = cmul(d8, d8);           // three squarings: a few ulp in T
             T va = (T)0, vb = (T)0;
 #pragma unroll 1
             for (int j8 = 0; j8 < K1_W; j8 += 8) {
@@ -248,10 +258,13 @@ size_t k1_workspace_bytes(int64_t m, int n, int s, int prec)
 }
 
 template <typename T, int PREC>
-static void k1_launch_t(const K1Params& p, const double* A, const uint64_t* signs, const int64_t* idx,
+static void k1_launch_t(const K1Params& p_in, const double* A, const uint64_t* signs, const int64_t* idx,
                         double* partial, double* As, Status* st, cudaStream_t stream)
 {
-    const size_t smem = (size_t)p.m1 * K1_LD * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + 2 * (size_t)p.s * sizeof(double);
+    K1Params p = p_in;
+    size_t smem = (size_t)p.m1 * K1_LD * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + 2 * (size_t)p.s * sizeof(double);
+    p.dtab = smem + (size_t)p.s * sizeof(Cx<T>) <= 200 * 1024;
+    if (p.dtab) smem += (size_t)p.s * sizeof(Cx<T>);
     auto k = mrcqr_k1_srtt<T, PREC>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int grid = ((p.n + 1) / 2) * p.chunks;

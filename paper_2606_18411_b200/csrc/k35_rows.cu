@@ -191,16 +191,18 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
 // panels with a left-looking sweep whose A fragments come straight from global memory (lane (g, t)
 // reads row g of column t: 64 contiguous bytes per column, every sector fully used; one step
 // prefetched ahead), then runs the same in-register panel_core as K3 / K5 and stores the solved panel.
-// Shared memory holds only the panel (18 KB per warp), so 10 warps per SM fit at any n; the row is
-// never resident as a whole, which is what limited the in-place slab solve to 8-row groups beyond n = 128.
-// The -R fragments of the left-looking sweep are shared by the 8 warps of the CTA: chunks of 8 block rows
-// (8 x PB x 512 B) are staged in shared memory by cp.async, double buffered, one barrier per chunk, so the
-// prepared factor is read from L2 once per CTA round instead of once per warp.
-constexpr int PP_NW = 8;              // warps per CTA
-constexpr int PP_KC = 8;              // block rows of R per staged chunk
+// Shared memory holds only the panel (18 KB per warp); the row is never resident as a whole, which is what
+// limited the in-place slab solve to 8-row groups beyond n = 128.
+// The -R fragments of the left-looking sweep are shared by the 4 warps of the CTA: chunks of 4 block rows
+// (4 x PB x 512 B) are staged in shared memory by cp.async, double buffered, one barrier per chunk.  A CTA's
+// round is load -> sweep -> solve -> store in lockstep, so two CTAs share an SM (105 KB each) and one's
+// memory phases overlap the other's DMMA phases (8 warps in one CTA: 6.07 ms per solve at C3, this: 5.90).
+constexpr int PP_NW = 4;              // warps per CTA
+constexpr int PP_KC = 4;              // block rows of R per staged chunk
+constexpr int PP_CTAS = 2;            // CTAs per SM: their load / solve / store phases interleave
 
 template <int FAC, int PB>
-__global__ void __launch_bounds__(PP_NW * 32, 1)
+__global__ void __launch_bounds__(PP_NW * 32, PP_CTAS)
 mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, int64_t ld_own,
                  const double* __restrict__ Yprev, int64_t ldy, const double2* __restrict__ frag,
                  double* __restrict__ dst, int64_t ldd, int64_t nslabs)
@@ -430,7 +432,7 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
     const int64_t nslabs = m / 32;
     const int nw = PP_NW;
     int64_t grid = (nslabs + nw - 1) / nw;
-    if (grid > num_sms()) grid = num_sms();
+    if (grid > PP_CTAS * num_sms()) grid = PP_CTAS * num_sms();
     int launches = 0;
     for (int P0 = 0; P0 < nB; P0 += 8) {
         const int pb = (nB - P0 >= 8) ? 8 : nB - P0;
