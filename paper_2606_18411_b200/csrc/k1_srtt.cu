@@ -5,8 +5,8 @@
 // wanted, so this kernel uses the four-step split m = m1*m2, t = t1*m2 + t2, k = k1 + m1*k2:
 //     X[k] = sum_{t2} W_m^{k t2} Z[k1, t2],     Z[k1, t2] = sum_{t1} x~[t1*m2 + t2] W_m1^{k1 t1},
 // and never materialises Z or X in HBM:
-//   stage 1  a CTA stages an m1 x 32 tile (32 consecutive t2, all t1; 256-byte coalesced row
-//            segments of the column-major A), applying the sign bit and the cast to p on the way
+//   stage 1  a CTA stages an m1 x W tile (W = 32 or 16 consecutive t2, all t1; 256- or 128-byte coalesced
+//            row segments of the column-major A), applying the sign bit and the cast to p on the way
 //            in (DiagMult), and runs the 32 length-m1 FFTs in shared memory with
 //            radix-4 decimation-in-frequency passes (output left in bit-reversed order).  Two real
 //            columns ride in one complex transform (re = column 2c, im = column 2c+1).
@@ -22,8 +22,9 @@
 
 namespace mrcqr {
 
-constexpr int K1_W = 32;          // t2 values per tile = lanes of a warp
-constexpr int K1_LD = 33;         // row stride of the tile in complex elements (odd: the per-bin gathers of stage 2 spread over the banks)
+// W = t2 values per tile (32: a warp instruction covers one tile row; 16: two rows, used for FP64 so that m1 = 256
+// fits the same 68 KB and the per-bin work of stage 2, which scales with s * m / m1, halves); the row stride of the
+// tile is W + 1 complex elements (odd: the per-bin gathers of stage 2 spread over the banks)
 constexpr int K1_NT = 256;
 constexpr int K1_NWARP = K1_NT / 32;
 
@@ -64,17 +65,19 @@ struct K1Params {
     int dtab;                     // the per-bin step twiddles W_m^k fit in shared memory (computed once per CTA)
 };
 
-template <typename T, int PREC>
+template <typename T, int PREC, int W>
 __global__ void __launch_bounds__(K1_NT, sizeof(T) == 8 ? 2 : 3)      // FP64 tiles: two CTAs per SM by shared memory
 mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
               const int64_t* __restrict__ idx, double* __restrict__ partial)
 {
+    constexpr int K1_W = W, K1_LD = W + 1, SUB = 32 / W;          // SUB tile rows per warp instruction
     extern __shared__ __align__(16) unsigned char smraw[];
-    Cx<T>* tile = reinterpret_cast<Cx<T>*>(smraw);                       // [m1][32]
+    Cx<T>* tile = reinterpret_cast<Cx<T>*>(smraw);                       // [m1][W + 1]
     Cx<T>* tw = tile + (size_t)p.m1 * K1_LD;                             // [m1]  W_m1^e
     double* colacc = reinterpret_cast<double*>(tw + p.m1);               // [2][s]
     Cx<T>* dstep = reinterpret_cast<Cx<T>*>(colacc + 2 * p.s);           // [s]  (cos, sin) of 2 pi k_i / m   (dtab only)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tcol = lane % W, sub = lane / W;
     const int pair = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
     const int ja = 2 * pair, jb = 2 * pair + 1;
     const bool has_b = jb < p.n;
@@ -102,27 +105,28 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
         // ---- load + DiagMult: 16-byte loads, a warp covers two 256-byte rows per instruction, eight
         //      row pairs (16 loads per thread) in flight before the first conversion ------------------
         if (p.vec) {
-            const int half = lane >> 4, pr = lane & 15;           // row within the pair, double2 index
+            constexpr int PRL = W / 2, RPI = 32 / PRL;            // lanes per row (double2 each), rows per instruction
+            const int half = lane / PRL, pr = lane % PRL;         // row within the group, double2 index
             const double2* colA = reinterpret_cast<const double2*>(A + (size_t)ja * (size_t)p.lda + t2_0) + pr;
             const double2* colB = reinterpret_cast<const double2*>(A + (size_t)(has_b ? jb : ja) * (size_t)p.lda + t2_0) + pr;
             const int64_t m2h = p.m2 >> 1;                          // row stride in double2
-            for (int t1b = 2 * warp; t1b < m1; t1b += 2 * K1_NWARP * 8) {
+            for (int t1b = RPI * warp; t1b < m1; t1b += RPI * K1_NWARP * 8) {
                 double2 va[8], vb[8];
                 unsigned sg[8];
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
-                    const int t1 = t1b + u * 2 * K1_NWARP + half;
+                    const int t1 = t1b + u * RPI * K1_NWARP + half;
                     va[u] = make_double2(0.0, 0.0); vb[u] = va[u]; sg[u] = 0;
                     if (t1 < m1) {
                         const int64_t off = (int64_t)t1 * m2h;
                         va[u] = __ldcs(colA + off);
                         if (has_b) vb[u] = __ldcs(colB + off);
-                        sg[u] = signs32[((int64_t)t1 * p.m2 + t2_0) >> 5] >> (2 * pr);
+                        sg[u] = signs32[((int64_t)t1 * p.m2 + t2_0) >> 5] >> ((int)(t2_0 & 31) + 2 * pr);
                     }
                 }
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
-                    const int t1 = t1b + u * 2 * K1_NWARP + half;
+                    const int t1 = t1b + u * RPI * K1_NWARP + half;
                     if (t1 < m1) {
                         Cx<T> e0{diag_cast<T, PREC>(va[u].x, sg[u] & 1u), diag_cast<T, PREC>(vb[u].x, sg[u] & 1u)};
                         Cx<T> e1{diag_cast<T, PREC>(va[u].y, (sg[u] >> 1) & 1u), diag_cast<T, PREC>(vb[u].y, (sg[u] >> 1) & 1u)};
@@ -133,15 +137,15 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
             }
         }
         else {                                                    // unaligned A: 8-byte loads
-            const double* colA = A + (size_t)ja * (size_t)p.lda + t2_0 + lane;
-            const double* colB = A + (size_t)(has_b ? jb : ja) * (size_t)p.lda + t2_0 + lane;
+            const double* colA = A + (size_t)ja * (size_t)p.lda + t2_0 + tcol;
+            const double* colB = A + (size_t)(has_b ? jb : ja) * (size_t)p.lda + t2_0 + tcol;
 #pragma unroll 4
-            for (int t1 = warp; t1 < m1; t1 += K1_NWARP) {
+            for (int t1 = warp * SUB + sub; t1 < m1; t1 += K1_NWARP * SUB) {
                 const int64_t off = (int64_t)t1 * p.m2;
-                const unsigned neg = (signs32[(off + t2_0) >> 5] >> lane) & 1u;
+                const unsigned neg = (signs32[(off + t2_0) >> 5] >> ((int)(t2_0 & 31) + tcol)) & 1u;
                 const double a = __ldcs(colA + off);
                 const double b = has_b ? __ldcs(colB + off) : 0.0;
-                tile[t1 * K1_LD + lane] = Cx<T>{diag_cast<T, PREC>(a, neg), diag_cast<T, PREC>(b, neg)};
+                tile[t1 * K1_LD + tcol] = Cx<T>{diag_cast<T, PREC>(a, neg), diag_cast<T, PREC>(b, neg)};
             }
         }
         __syncthreads();
@@ -149,9 +153,9 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
         int nb = m1;                                   // current block size
         while (nb >= 4) {
             const int q = nb >> 2, tstride = m1 / nb;
-            for (int bf = warp; bf < (m1 >> 2); bf += K1_NWARP) {
+            for (int bf = warp * SUB + sub; bf < (m1 >> 2); bf += K1_NWARP * SUB) {
                 const int blk = bf / q, pos = bf % q;
-                Cx<T>* base = tile + ((size_t)blk * nb + pos) * K1_LD + lane;
+                Cx<T>* base = tile + ((size_t)blk * nb + pos) * K1_LD + tcol;
                 Cx<T> a0 = base[0], a1 = base[(size_t)q * K1_LD], a2 = base[(size_t)2 * q * K1_LD], a3 = base[(size_t)3 * q * K1_LD];
                 const Cx<T> w1 = tw[pos * tstride], w2 = tw[2 * pos * tstride];
                 Cx<T> b0 = cadd(a0, a2), b2 = cmul(csub(a0, a2), w1);
@@ -165,8 +169,8 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
             __syncthreads();
         }
         if (nb == 2) {                                 // odd log2(m1): final radix-2 pass, twiddle 1
-            for (int bf = warp; bf < (m1 >> 1); bf += K1_NWARP) {
-                Cx<T>* base = tile + (size_t)(2 * bf) * K1_LD + lane;
+            for (int bf = warp * SUB + sub; bf < (m1 >> 1); bf += K1_NWARP * SUB) {
+                Cx<T>* base = tile + (size_t)(2 * bf) * K1_LD + tcol;
                 Cx<T> a0 = base[0], a1 = base[K1_LD];
                 base[0] = cadd(a0, a1);
                 base[K1_LD] = csub(a0, a1);
@@ -229,11 +233,21 @@ __global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial
     As[e] = v;
 }
 
+// tile width: 16 doubles m1 at the same tile size (FP64: 256, FP32 arithmetic: 512).  Taken for FP64, and for
+// FP16/FP32 sketches with s >= 1024 where stage 2 dominates, when the matrix is long enough for whole sign words
+// per tile row (m2 % 32 == 0)
+static int k1_tile_w(int64_t m, int prec, int s)
+{
+    if (prec == 64) return m >= 256 * 32 ? 16 : 32;
+    return (s >= 1024 && m >= 512 * 32) ? 16 : 32;     // measured: s = 256 slower (0.50 -> 0.58 ms at C2), 512 equal, 1024 6.9 -> 6.0 ms
+}
+
 static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec)
 {
     K1Params p;
     p.m = m; p.lda = lda; p.n = n; p.s = s;
-    const int m1max = (prec == 64) ? 128 : 256;      // 64 KB tile: three CTAs per SM
+    const int K1_W = k1_tile_w(m, prec, s);
+    const int m1max = ((prec == 64) ? 128 : 256) * (32 / K1_W);    // 68 KB tile
     int64_t m1 = m / K1_W;
     if (m1 > m1max) m1 = m1max;
     if (m1 < 1) m1 = 1;
@@ -257,15 +271,15 @@ size_t k1_workspace_bytes(int64_t m, int n, int s, int prec)
     return fft > tc ? fft : tc;
 }
 
-template <typename T, int PREC>
+template <typename T, int PREC, int W>
 static void k1_launch_t(const K1Params& p_in, const double* A, const uint64_t* signs, const int64_t* idx,
                         double* partial, double* As, Status* st, cudaStream_t stream)
 {
     K1Params p = p_in;
-    size_t smem = (size_t)p.m1 * K1_LD * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + 2 * (size_t)p.s * sizeof(double);
+    size_t smem = (size_t)p.m1 * (W + 1) * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + 2 * (size_t)p.s * sizeof(double);
     p.dtab = smem + (size_t)p.s * sizeof(Cx<T>) <= 200 * 1024;
     if (p.dtab) smem += (size_t)p.s * sizeof(Cx<T>);
-    auto k = mrcqr_k1_srtt<T, PREC>;
+    auto k = mrcqr_k1_srtt<T, PREC, W>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int grid = ((p.n + 1) / 2) * p.chunks;
     k<<<grid, K1_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
@@ -283,9 +297,13 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
     K1Params p = k1_params(m, n, lda, s, prec);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
     double* partial = reinterpret_cast<double*>(k1_work);
-    if (prec == 16) k1_launch_t<float, 16>(p, A, signs, idx, partial, As, st, stream);
-    else if (prec == 32) k1_launch_t<float, 32>(p, A, signs, idx, partial, As, st, stream);
-    else k1_launch_t<double, 64>(p, A, signs, idx, partial, As, st, stream);
+    const bool w16 = k1_tile_w(m, prec, s) == 16;
+    if (prec == 16) { if (w16) k1_launch_t<float, 16, 16>(p, A, signs, idx, partial, As, st, stream);
+                      else k1_launch_t<float, 16, 32>(p, A, signs, idx, partial, As, st, stream); }
+    else if (prec == 32) { if (w16) k1_launch_t<float, 32, 16>(p, A, signs, idx, partial, As, st, stream);
+                           else k1_launch_t<float, 32, 32>(p, A, signs, idx, partial, As, st, stream); }
+    else { if (w16) k1_launch_t<double, 64, 16>(p, A, signs, idx, partial, As, st, stream);
+           else k1_launch_t<double, 64, 32>(p, A, signs, idx, partial, As, st, stream); }
     return 2;
 }
 

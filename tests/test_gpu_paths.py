@@ -60,6 +60,24 @@ def test_tensor_core_sketch_closed_form(orc):
     assert np.linalg.norm(Asg - want) <= 1e-2 * np.linalg.norm(want)
 
 
+@pytest.mark.parametrize("m,n,s,prec,tol", [
+    (1 << 13, 5, 40, 64, 1e-12),       # FP64: 16-wide tiles, m1 = 256, m2 = 32 (one sign word per tile row pair)
+    (1 << 15, 6, 96, 64, 1e-12),       # FP64: several tiles per chunk, even n
+    (1 << 14, 3, 1024, 32, 5e-5),      # FP32, s >= 1024: 16-wide tiles, m1 = 512, odd n
+    (1 << 15, 4, 1030, 16, 1e-2),      # FP16 rounding of the same form, ragged s
+    (1 << 12, 5, 40, 64, 1e-12),       # FP64 below the 16-wide threshold: 32-wide tiles, m1 = 128
+])
+def test_fft_sketch_tile_widths_match_oracle(orc, m, n, s, prec, tol):
+    """The FFT form of K1 (k1_srtt.cu) picks the tile width from (m, prec, s); every choice is the same transform."""
+    AT = inputs.make_A(m, n, 3, 500 + n, 501 + n, "cuda")
+    A = to_np(AT)
+    signs, idx = orc.draw(m, s, 900 + n)
+    As_o = orc.sketch(np.asfortranarray(A), signs, idx)        # the oracle's sketch is the double one
+    dsigns, didx = draw_to_dev(signs, idx)
+    _, As = B.mrcqr_sketch(AT, {16: B.FP16, 32: B.FP32, 64: B.FP64}[prec], dsigns, didx, want_As=True)
+    assert relf(to_np(As), As_o) <= tol
+
+
 @pytest.mark.parametrize("m,n,expo,prec", [
     (1 << 12, 136, 3, 32),     # n16 = 144: panels of 8, 8, 2 blocks; SYRK with P = 2 and a ragged second panel
     (1 << 12, 160, 6, 64),     # n16 = 160: panels 8, 8, 4
