@@ -233,12 +233,13 @@ __global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial
     As[e] = v;
 }
 
-// tile width: 16 doubles m1 at the same tile size (FP64: 256, FP32 arithmetic: 512).  Taken for FP64, and for
+// tile width: 16 doubles m1 at the same tile size (FP64: 256, FP32 arithmetic: 512), 8 doubles it again (FP64 with
+// s >= 512: C3 3.40 -> 3.30 ms, n = 512 9.8 -> 9.0 ms; 64-byte row segments).  16 is taken for FP64, and for
 // FP16/FP32 sketches with s >= 1024 where stage 2 dominates, when the matrix is long enough for whole sign words
 // per tile row (m2 % 32 == 0)
 static int k1_tile_w(int64_t m, int prec, int s)
 {
-    if (prec == 64) return m >= 256 * 32 ? 16 : 32;
+    if (prec == 64) return (s >= 512 && m >= 512 * 32) ? 8 : (m >= 256 * 32 ? 16 : 32);
     return (s >= 1024 && m >= 512 * 32) ? 16 : 32;     // measured: s = 256 slower (0.50 -> 0.58 ms at C2), 512 equal, 1024 6.9 -> 6.0 ms
 }
 
@@ -247,7 +248,7 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec)
     K1Params p;
     p.m = m; p.lda = lda; p.n = n; p.s = s;
     const int K1_W = k1_tile_w(m, prec, s);
-    const int m1max = ((prec == 64) ? 128 : 256) * (32 / K1_W);    // 68 KB tile
+    const int m1max = ((prec == 64) ? 128 : 256) * (32 / K1_W);    // 68 KB tile (W = 8: 74 KB)
     int64_t m1 = m / K1_W;
     if (m1 > m1max) m1 = m1max;
     if (m1 < 1) m1 = 1;
@@ -297,12 +298,14 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
     K1Params p = k1_params(m, n, lda, s, prec);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
     double* partial = reinterpret_cast<double*>(k1_work);
-    const bool w16 = k1_tile_w(m, prec, s) == 16;
+    const int tw_ = k1_tile_w(m, prec, s);
+    const bool w16 = tw_ == 16;
     if (prec == 16) { if (w16) k1_launch_t<float, 16, 16>(p, A, signs, idx, partial, As, st, stream);
                       else k1_launch_t<float, 16, 32>(p, A, signs, idx, partial, As, st, stream); }
     else if (prec == 32) { if (w16) k1_launch_t<float, 32, 16>(p, A, signs, idx, partial, As, st, stream);
                            else k1_launch_t<float, 32, 32>(p, A, signs, idx, partial, As, st, stream); }
-    else { if (w16) k1_launch_t<double, 64, 16>(p, A, signs, idx, partial, As, st, stream);
+    else { if (tw_ == 8) k1_launch_t<double, 64, 8>(p, A, signs, idx, partial, As, st, stream);
+           else if (w16) k1_launch_t<double, 64, 16>(p, A, signs, idx, partial, As, st, stream);
            else k1_launch_t<double, 64, 32>(p, A, signs, idx, partial, As, st, stream); }
     return 2;
 }

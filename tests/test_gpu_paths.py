@@ -63,6 +63,7 @@ def test_tensor_core_sketch_closed_form(orc):
 @pytest.mark.parametrize("m,n,s,prec,tol", [
     (1 << 13, 5, 40, 64, 1e-12),       # FP64: 16-wide tiles, m1 = 256, m2 = 32 (one sign word per tile row pair)
     (1 << 15, 6, 96, 64, 1e-12),       # FP64: several tiles per chunk, even n
+    (1 << 14, 4, 520, 64, 1e-12),      # FP64, s >= 512: 8-wide tiles, m1 = 512
     (1 << 14, 3, 1024, 32, 5e-5),      # FP32, s >= 1024: 16-wide tiles, m1 = 512, odd n
     (1 << 15, 4, 1030, 16, 1e-2),      # FP16 rounding of the same form, ragged s
     (1 << 12, 5, 40, 64, 1e-12),       # FP64 below the 16-wide threshold: 32-wide tiles, m1 = 128
