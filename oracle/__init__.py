@@ -27,6 +27,7 @@ def lib():
         L.orc_fft_radix2.restype = None
         L.orc_fft_radix2.argtypes = [i64, vp, vp]
         L.orc_sketch.argtypes = [i64, C.c_int, i64, vp, vp, C.c_int, vp, vp]
+        L.orc_sketch_reim.argtypes = [i64, C.c_int, i64, vp, vp, C.c_int, vp, vp]
         L.orc_householder_r.argtypes = [C.c_int, C.c_int, vp, vp]
         L.orc_row_solve.restype = None
         L.orc_row_solve.argtypes = [i64, C.c_int, i64, vp, vp, i64, vp]
@@ -97,6 +98,18 @@ def sketch(A, signs, idx):
     idx = np.ascontiguousarray(idx, dtype=np.int64)
     As = _new((s, n))
     lib().orc_sketch(m, n, m, _p(A), _p(signs), s, _p(idx), _p(As))
+    return As
+
+
+def sketch_reim(A, signs, idx):
+    """Re+Im variant: (2s, n) sketch, rows [0, s) = sqrt(s/m) Re X[S], rows [s, 2s) = sqrt(s/m) Im X[S]."""
+    A = _f(A)
+    m, n = A.shape
+    s = int(len(idx))
+    signs = np.ascontiguousarray(signs, dtype=np.uint64)
+    idx = np.ascontiguousarray(idx, dtype=np.int64)
+    As = _new((2 * s, n))
+    lib().orc_sketch_reim(m, n, m, _p(A), _p(signs), s, _p(idx), _p(As))
     return As
 
 

@@ -155,6 +155,57 @@ int orc_sketch(int64_t m, int n, int64_t lda, const double *A, const uint64_t *s
 }
 
 /* ------------------------------------------------------------------------------------------
+ * o4'. Re+Im variant of the sketch ("retain both real and imaginary parts, yielding a
+ * 2c x n sketch at no extra FFT cost but doubling the sketch QR cost"; the authors measured it and
+ * kept Re-only).  With X = FFT(D a_j), X_k = sum_t x~_t exp(-2 pi i k t / m):
+ *   As[i, j]     = sqrt(s/m) * Re X[k_i],   As[s + i, j] = sqrt(s/m) * Im X[k_i],   i < s.
+ * Reading R11: the paper gives neither the row order nor a scale for this variant; the
+ * Re rows keep their place and scale, the Im rows follow (a common factor only scales R_s).
+ * As is 2s x n column-major, ld = 2s.  Returns 0.
+ * pin: brute-force sine sum, pure-sine closed form, Im = 0 at DC / Nyquist, Re rows equal o2-o4.
+ * ------------------------------------------------------------------------------------------ */
+int orc_sketch_reim(int64_t m, int n, int64_t lda, const double *A, const uint64_t *signs,
+                    int s, const int64_t *idx, double *As)
+{
+    const double scale = sqrt((double)s / (double)m);
+    const size_t ld = 2 * (size_t)s;
+    if (is_pow2(m)) {
+        #pragma omp parallel
+        {
+            double *re = (double *)malloc(sizeof(double) * (size_t)m);
+            double *im = (double *)malloc(sizeof(double) * (size_t)m);
+            #pragma omp for schedule(dynamic, 1)
+            for (int j = 0; j < n; ++j) {
+                const double *a = A + (size_t)j * (size_t)lda;
+                for (int64_t t = 0; t < m; ++t) { re[t] = sign_of(signs, t) * a[t]; im[t] = 0.0; }
+                orc_fft_radix2(m, re, im);
+                for (int i = 0; i < s; ++i) {
+                    As[(size_t)j * ld + i] = scale * re[idx[i]];
+                    As[(size_t)j * ld + s + i] = scale * im[idx[i]];
+                }
+            }
+            free(re); free(im);
+        }
+    } else {
+        #pragma omp parallel for collapse(2) schedule(static)
+        for (int j = 0; j < n; ++j)
+            for (int i = 0; i < s; ++i) {
+                const double *a = A + (size_t)j * (size_t)lda;
+                double accr = 0.0, acci = 0.0;
+                for (int64_t t = 0; t < m; ++t) {
+                    int64_t r = (int64_t)(((unsigned __int128)idx[i] * (unsigned __int128)t) % (unsigned __int128)m);
+                    const double x = sign_of(signs, t) * a[t], th = 2.0 * ORC_PI * (double)r / (double)m;
+                    accr += x * cos(th);
+                    acci -= x * sin(th);
+                }
+                As[(size_t)j * ld + i] = scale * accr;
+                As[(size_t)j * ld + s + i] = scale * acci;
+            }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
  * o5. R-factor of the Householder QR of the s x n sketch (Algorithm 2 step 5), then
  * rows negated so that diag(R_s) > 0 (reading R6: the paper is silent; positive diagonals make
  * (Q,R) unique as north_star requires).  Unblocked textbook Householder (Golub & Van Loan

@@ -170,3 +170,63 @@ def test_sketch_impulse_and_sign_flip(orc):
     assert np.max(np.abs(As[:, 0] - want0)) < 1e-14
     want1 = np.where(idx == 0, np.sqrt(s / m) * m, 0.0)
     assert np.max(np.abs(As[:, 1] - want1)) < 1e-11
+
+
+# ---- Re+Im variant of the sketch -------------------------------------------------
+def sketch_im_brute(A, signs, idx):
+    """sqrt(s/m) * Im sum_t d_t a_t exp(-2 pi i k_i t/m) = -sqrt(s/m) sum_t d_t a_t sin(2 pi k_i t/m)."""
+    m, n = A.shape
+    s = len(idx)
+    d = np.array([-1.0 if (int(signs[t >> 6]) >> (t & 63)) & 1 else 1.0 for t in range(m)])
+    t = np.arange(m)
+    out = np.zeros((s, n))
+    for i, k in enumerate(idx):
+        sn = np.sin(2.0 * np.pi * ((int(k) * t) % m) / m)
+        for j in range(n):
+            out[i, j] = -np.sqrt(s / m) * float(np.sum(np.longdouble(d * A[:, j]) * np.longdouble(sn)))
+    return out
+
+
+@pytest.mark.parametrize("m,n,s", [(4096, 5, 12), (256, 3, 129), (1000, 4, 9), (96, 2, 5)])
+def test_sketch_reim_vs_bruteforce(orc, m, n, s):
+    rng = np.random.default_rng(3 * m + n)
+    A = np.asfortranarray(rng.standard_normal((m, n)))
+    signs, idx = orc.draw(m, s, 19)
+    got = orc.sketch_reim(A, signs, idx)
+    assert got.shape == (2 * s, n)
+    # the Re rows are the Re-only sketch, bit for bit (same transform, same gather, same scale)
+    assert np.array_equal(got[:s], orc.sketch(A, signs, idx)) or m & (m - 1)
+    want_re, want_im = sketch_brute(A, signs, idx), sketch_im_brute(A, signs, idx)
+    tol = 1e-13 * np.sqrt(m)
+    assert np.linalg.norm(got[:s] - want_re) <= tol * np.linalg.norm(want_re)
+    assert np.linalg.norm(got[s:] - want_im) <= tol * max(np.linalg.norm(want_im), np.linalg.norm(want_re))
+
+
+def test_sketch_reim_closed_forms(orc):
+    """Column j = d * sin(2 pi k_j t/m): X[k_j] = -i m/2, so Im = -m/2 at (s + j, j) and nothing else (bins are
+    distinct and below m/2 or at 0 / m/2); a constant column d * 1 has Im = 0 everywhere; Im X[0] = Im X[m/2] = 0."""
+    m, n, s = 1024, 6, 24
+    signs, idx = orc.draw(m, s, 11)
+    d = np.array([-1.0 if (int(signs[t >> 6]) >> (t & 63)) & 1 else 1.0 for t in range(m)])
+    t = np.arange(m)
+    cols, live = [], []
+    for j in range(n - 1):
+        k0 = int(idx[j])
+        cols.append(d * np.sin(2 * np.pi * k0 * t / m))
+        live.append(k0 not in (0, m // 2))
+    cols.append(d.copy())
+    A = np.asfortranarray(np.stack(cols, axis=1))
+    As = orc.sketch_reim(A, signs, idx)
+    scale = np.sqrt(s / m)
+    want = np.zeros((2 * s, n))
+    for j in range(n - 1):
+        if live[j]:
+            want[s + j, j] = -0.5 * m * scale
+    want[:s, n - 1] = np.where(idx == 0, m * scale, 0.0)
+    assert np.max(np.abs(As - want)) < 1e-10
+    # a generic real column: the imaginary part vanishes at DC and Nyquist
+    rng = np.random.default_rng(5)
+    B = np.asfortranarray(rng.standard_normal((m, 1)))
+    idx2 = np.array([0, m // 2, 3], dtype=np.int64)
+    As2 = orc.sketch_reim(B, signs, idx2)
+    assert abs(As2[3, 0]) < 1e-12 and abs(As2[4, 0]) < 1e-12 and abs(As2[5, 0]) > 1e-6
