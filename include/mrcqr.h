@@ -179,6 +179,17 @@ int mrcqr_kappa_probe(int64_t m, int n, int64_t lda, const double* A, double* Qw
 int mrcqr_set_store_y(int on);
 
 /*
+ * Variant switch of the sketch (SURVEY.md 8(f)3 iii; "retain both real and imaginary parts,
+ * yielding a 2c x n sketch at no extra FFT cost but doubling the sketch QR cost" -- measured by the authors,
+ * who kept Re-only).  On, every call that sketches (mrcqr_sketch, mrcqr_factor, mrcqr_factor_host,
+ * mrcqr_factor_auto) forms the 2s x n matrix  [ sqrt(s/m) Re X[S] ; sqrt(s/m) Im X[S] ]  (reading R11: Re rows
+ * first, same scale) in the FFT form of K1 and QR-factors that; the As argument of mrcqr_sketch then receives
+ * 2s x n values (column-major, ld = 2s).  Requires 2s <= 4096 (else the s argument is reported invalid).
+ * Off (default): Algorithm 2 as printed.  Returns 0.
+ */
+int mrcqr_set_sketch_reim(int on);
+
+/*
  * Repeated-call mode (block Arnoldi, randomized-SVD power iteration, time stepping): on, the
  * kernels, copies and the status read-back of mrcqr_factor are captured ONCE into a CUDA graph per (m, n, lda, A, Q, R,
  * precision, s) and replayed by later calls with the same arguments; the seed and the drawn bins are data of the graph

@@ -54,11 +54,12 @@ def lib():
         L.mrcqr_orth_error.argtypes = [i64, ci, i64, vp, vp, vp]
         L.mrcqr_factor_auto.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64, C.c_double, vp, vp, vp]
         L.mrcqr_set_store_y.argtypes = [ci]
+        L.mrcqr_set_sketch_reim.argtypes = [ci]
         L.mrcqr_set_graph.argtypes = [ci]
         L.mrcqr_last_timing.argtypes = [vp]
         for f in ("mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
                   "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
-                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph"):
+                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"):
             getattr(L, f).restype = ci
         _lib = L
     return _lib
@@ -66,7 +67,7 @@ def lib():
 
 EXPORTS = ["mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
-           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph"]
+           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"]
 
 STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "reduce_k4_chol", "k5_form_q", "r_mul"]
 
@@ -103,7 +104,7 @@ def mrcqr_sketch(AT, prec, signs, idx, want_As=False, stream=None):
     m, n, lda, pA = _mat(AT)
     s = idx.numel()
     Rs = torch.empty((n, n), dtype=torch.float64, device=AT.device)
-    As = torch.empty((n, s), dtype=torch.float64, device=AT.device) if want_As else None
+    As = torch.empty((n, 2 * s if _reim else s), dtype=torch.float64, device=AT.device) if want_As else None
     rc = lib().mrcqr_sketch(m, n, lda, pA, prec, s, signs.data_ptr(), idx.data_ptr(),
                             As.data_ptr() if want_As else None, Rs.data_ptr(), _stream(stream))
     _chk(rc)
@@ -237,6 +238,16 @@ def mrcqr_kappa_probe(AT, stream=None):
 def mrcqr_set_graph(on):
     """Repeated-call mode: mrcqr_factor replays a CUDA graph captured per (shape, buffers)."""
     lib().mrcqr_set_graph(1 if on else 0)
+
+
+_reim = False
+
+
+def mrcqr_set_sketch_reim(on):
+    """Re+Im sketch variant: 2s sketch rows; mrcqr_sketch(want_As=True) then returns (n, 2s)."""
+    global _reim
+    lib().mrcqr_set_sketch_reim(1 if on else 0)
+    _reim = bool(on)
 
 
 def mrcqr_set_store_y(on):

@@ -65,7 +65,7 @@ static Layout make_layout(int64_t m, int n, int s, int prec)
     L.status = o; o += al(sizeof(Status));
     L.signs = o;  o += al((size_t)((m + 63) / 64) * 8);
     L.idx = o;    o += al((size_t)std::max(s, 1) * 8);
-    L.As = o;     o += al((size_t)std::max(s, 1) * n * 8);
+    L.As = o;     o += al((size_t)2 * std::max(s, 1) * n * 8);       // 2s rows in the Re+Im variant
     L.Rs = o;     o += al((size_t)n * n * 8);
     L.RsPrep = o; o += al(n16 * n16 * 8);
     L.RcPrep = o; o += al(n16 * n16 * 8);
@@ -87,10 +87,11 @@ struct Ctx {
     bool timing = false; cudaEvent_t ev[8] = {}; bool ev_ok = false; float stage_ms[8] = {};
     bool have_device = false, probed = false;
     bool store_y = false;                    // mrcqr_set_store_y: store-Y variant also for n16 <= 128
+    bool reim = false;                       // mrcqr_set_sketch_reim: Re+Im sketch (2s rows)
     // mrcqr_set_graph: the whole enqueue sequence of mrcqr_factor captured once per (shape, buffers) and replayed
     bool use_graph = false;
     cudaGraphExec_t gexec = nullptr; int glaunches = 0; uint64_t* h_seed = nullptr;
-    struct { int64_t m, lda; int n, prec, s; const void *A, *Q, *R, *ws, *hidx; bool store_y; } gkey = {};
+    struct { int64_t m, lda; int n, prec, s; const void *A, *Q, *R, *ws, *hidx; bool store_y, reim; } gkey = {};
 };
 static Ctx g;
 
@@ -151,9 +152,10 @@ static int enqueue_sketch(const Layout& L, int64_t m, int n, int64_t lda, const 
 {
     Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
     double* As = reinterpret_cast<double*>(g.ws + L.As);
-    int k = launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);
-    if (As_out) cudaMemcpyAsync(As_out, As, sizeof(double) * (size_t)s * n, cudaMemcpyDeviceToDevice, st);
-    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
+    const int rows = g.reim ? 2 * s : s;
+    int k = launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st, g.reim);
+    if (As_out) cudaMemcpyAsync(As_out, As, sizeof(double) * (size_t)rows * n, cudaMemcpyDeviceToDevice, st);
+    k += launch_k2_sketch_qr(As, rows, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
                              reinterpret_cast<double*>(g.ws + L.betas), stat, st);
     return k;
 }
@@ -247,7 +249,7 @@ extern "C" int mrcqr_sketch(int64_t m, int n, int64_t lda, const double* A, mrcq
     if (lda < m) return -3;
     if (!A) return -4;
     if (!prec_ok((int)prec)) return -5;
-    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX) return -6;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX || (g.reim && 2 * s > S_MAX)) return -6;
     if (!signs) return -7;
     if (!idx) return -8;
     if (!Rs) return -10;
@@ -336,6 +338,7 @@ static bool timing_events()
 
 extern "C" int mrcqr_set_timing(int on) { g.timing = (on != 0); return 0; }
 extern "C" int mrcqr_set_store_y(int on) { g.store_y = (on != 0); return 0; }
+extern "C" int mrcqr_set_sketch_reim(int on) { g.reim = (on != 0); return 0; }
 extern "C" int mrcqr_set_graph(int on) { g.use_graph = (on != 0); if (!on) drop_graph(); return 0; }
 
 extern "C" int mrcqr_last_timing(float* ms_out_host)
@@ -403,9 +406,9 @@ static int enqueue_factor(const Layout& L, int64_t m, int n, int64_t lda, const 
     int k = 1;
     double* As = reinterpret_cast<double*>(g.ws + L.As);
     if (tm) cudaEventRecord(g.ev[0], st);
-    k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st);     // steps 2-4
+    k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st, g.reim);     // steps 2-4
     if (tm) cudaEventRecord(g.ev[1], st);
-    k += launch_k2_sketch_qr(As, s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
+    k += launch_k2_sketch_qr(As, g.reim ? 2 * s : s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
                              reinterpret_cast<double*>(g.ws + L.betas), stat, st);                              // steps 5-6
     if (tm) cudaEventRecord(g.ev[2], st);
     k += enqueue_stage23(L, m, n, lda, A, ldq, Q, R, Rs, st, tm);                              // steps 7-9
@@ -423,7 +426,7 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
         if (!g.h_seed && cudaMallocHost(&g.h_seed, 64) != cudaSuccess) { cudaGetLastError(); g.h_seed = nullptr; }
         const bool same = g.gexec && g.gkey.m == m && g.gkey.lda == lda && g.gkey.n == n && g.gkey.prec == prec &&
                           g.gkey.s == s && g.gkey.A == A && g.gkey.Q == Q && g.gkey.R == R && g.gkey.ws == g.ws &&
-                          g.gkey.hidx == g.h_idx && g.gkey.store_y == g.store_y;
+                          g.gkey.hidx == g.h_idx && g.gkey.store_y == g.store_y && g.gkey.reim == g.reim;
         if (g.h_seed && !same) {
             drop_graph();
             uint64_t* seed_dev = reinterpret_cast<uint64_t*>(g.ws + L.status) + 2;        // Status::pad
@@ -439,7 +442,7 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
             cudaGetLastError();
             if (g.gexec) {
                 g.gkey.m = m; g.gkey.lda = lda; g.gkey.n = n; g.gkey.prec = prec; g.gkey.s = s; g.gkey.A = A; g.gkey.Q = Q;
-                g.gkey.R = R; g.gkey.ws = g.ws; g.gkey.hidx = g.h_idx; g.gkey.store_y = g.store_y;
+                g.gkey.R = R; g.gkey.ws = g.ws; g.gkey.hidx = g.h_idx; g.gkey.store_y = g.store_y; g.gkey.reim = g.reim;
             }
         }
         if (g.gexec) {
@@ -468,7 +471,7 @@ extern "C" int mrcqr_factor(int64_t m, int n, int64_t lda, const double* A, doub
     if (!R) return -6;
     if (!prec_ok((int)sketch_prec)) return -7;
     if (s <= 0) s = 3 * n;
-    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX) return -8;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX || (g.reim && 2 * s > S_MAX)) return -8;
     if (!device_ok()) return MRCQR_ERR_CUDA;
     return factor_device(m, n, lda, A, lda, Q, R, (int)sketch_prec, s, seed, (cudaStream_t)stream);
 }
@@ -514,7 +517,7 @@ extern "C" int mrcqr_factor_auto(int64_t m, int n, int64_t lda, const double* A,
     if (!R) return -6;
     if (!prec_ok((int)first_prec)) return -7;
     if (s <= 0) s = 3 * n;
-    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX) return -8;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX || (g.reim && 2 * s > S_MAX)) return -8;
     if (!device_ok()) return MRCQR_ERR_CUDA;
     if (!(tol > 0.0)) tol = 1e-13;
     cudaStream_t st = (cudaStream_t)stream;
@@ -613,7 +616,7 @@ extern "C" int mrcqr_factor_host(int64_t m, int n, int64_t lda, const double* A_
     if (!R_host) return -6;
     if (!prec_ok((int)sketch_prec)) return -7;
     if (s <= 0) s = 3 * n;
-    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX) return -8;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX || (g.reim && 2 * s > S_MAX)) return -8;
     if (!device_ok()) return MRCQR_ERR_CUDA;
     const size_t bytes = sizeof(double) * (size_t)lda * n, rbytes = sizeof(double) * (size_t)n * n;
     if (bytes > g.hA_bytes) {

@@ -62,10 +62,11 @@ struct K1Params {
     int64_t m2;
     int tiles_per_col, tiles_per_chunk, chunks;
     int vec;                      // A and lda allow 16-byte loads
+    int reim;                     // Re+Im variant: 2s sketch rows, Im X[S] below Re X[S]
     int dtab;                     // the per-bin step twiddles W_m^k fit in shared memory (computed once per CTA)
 };
 
-template <typename T, int PREC, int W>
+template <typename T, int PREC, int W, bool REIM>
 __global__ void __launch_bounds__(K1_NT, sizeof(T) == 8 ? 2 : 3)      // FP64 tiles: two CTAs per SM by shared memory
 mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
               const int64_t* __restrict__ idx, double* __restrict__ partial)
@@ -74,8 +75,9 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
     extern __shared__ __align__(16) unsigned char smraw[];
     Cx<T>* tile = reinterpret_cast<Cx<T>*>(smraw);                       // [m1][W + 1]
     Cx<T>* tw = tile + (size_t)p.m1 * K1_LD;                             // [m1]  W_m1^e
-    double* colacc = reinterpret_cast<double*>(tw + p.m1);               // [2][s]
-    Cx<T>* dstep = reinterpret_cast<Cx<T>*>(colacc + 2 * p.s);           // [s]  (cos, sin) of 2 pi k_i / m   (dtab only)
+    constexpr int NACC = REIM ? 4 : 2;                                    // Re a, Re b (, Im a, Im b)
+    double* colacc = reinterpret_cast<double*>(tw + p.m1);               // [NACC][s]
+    Cx<T>* dstep = reinterpret_cast<Cx<T>*>(colacc + NACC * p.s);           // [s]  (cos, sin) of 2 pi k_i / m   (dtab only)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tcol = lane % W, sub = lane / W;
     const int pair = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
@@ -88,7 +90,7 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
         sincospi(-2.0 * (double)e / (double)m1, &sn, &cs);
         tw[e] = Cx<T>{(T)cs, (T)sn};
     }
-    for (int e = tid; e < 2 * p.s; e += K1_NT) colacc[e] = 0.0;
+    for (int e = tid; e < NACC * p.s; e += K1_NT) colacc[e] = 0.0;
     if (p.dtab)
         for (int i = tid; i < p.s; i += K1_NT) {
             const int64_t k = idx[i];
@@ -193,7 +195,7 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
             if (p.dtab) d1 = dstep[i];
             else sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d1.y, &d1.x);
             d8 = cmul(d1, d1); d8 = cmul(d8, d8); d8 = cmul(d8, d8);           // three squarings: a few ulp in T
-            T va = (T)0, vb = (T)0;
+            T va = (T)0, vb = (T)0, ia = (T)0, ib = (T)0;
 #pragma unroll 1
             for (int j8 = 0; j8 < K1_W; j8 += 8) {
                 Cx<T> w = w0;
@@ -203,17 +205,22 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
                     // 2 Z_a = P + conj Qn, 2 Z_b = -i (P - conj Qn);  Re(e^{-i th} Z) = cos*Zr + sin*Zi
                     va = fma(w.x, P.x + Qn.x, va); va = fma(w.y, P.y - Qn.y, va);
                     vb = fma(w.x, P.y + Qn.y, vb); vb = fma(w.y, Qn.x - P.x, vb);
+                    if (REIM) {                                 // Im(e^{-i th} Z) = cos*Zi - sin*Zr
+                        ia = fma(w.x, P.y - Qn.y, ia); ia = fma(-w.y, P.x + Qn.x, ia);
+                        ib = fma(w.x, Qn.x - P.x, ib); ib = fma(-w.y, P.y + Qn.y, ib);
+                    }
                     w = cmul(w, d1);
                 }
                 w0 = cmul(w0, d8);
             }
             colacc[i] += 0.5 * (double)va;
             colacc[p.s + i] += 0.5 * (double)vb;
+            if (REIM) { colacc[2 * p.s + i] += 0.5 * (double)ia; colacc[3 * p.s + i] += 0.5 * (double)ib; }
         }
     }
     __syncthreads();
-    double* out = partial + ((size_t)pair * p.chunks + chunk) * 2 * p.s;
-    for (int e = tid; e < 2 * p.s; e += K1_NT) out[e] = colacc[e];
+    double* out = partial + ((size_t)pair * p.chunks + chunk) * NACC * p.s;
+    for (int e = tid; e < NACC * p.s; e += K1_NT) out[e] = colacc[e];
 }
 
 // A_s[i, j] = fl_p( sqrt(s/m) * sum_chunks partial ), chunks added in ascending order.
@@ -221,11 +228,13 @@ template <int PREC>
 __global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial, double* __restrict__ As, Status* st)
 {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= p.s * p.n) return;
-    const int i = e % p.s, j = e / p.s;
-    const double* src = partial + ((size_t)(j >> 1) * p.chunks) * 2 * p.s + (size_t)(j & 1) * p.s + i;
+    const int rows = p.reim ? 2 * p.s : p.s, nacc = p.reim ? 4 : 2;
+    if (e >= rows * p.n) return;
+    const int r = e % rows, j = e / rows;
+    const int i = r % p.s, part = (j & 1) + 2 * (r / p.s);           // Re a, Re b, Im a, Im b
+    const double* src = partial + ((size_t)(j >> 1) * p.chunks) * nacc * p.s + (size_t)part * p.s + i;
     double acc = 0.0;
-    for (int c = 0; c < p.chunks; ++c) acc += src[(size_t)c * 2 * p.s];
+    for (int c = 0; c < p.chunks; ++c) acc += src[(size_t)c * nacc * p.s];
     double v = acc * sqrt((double)p.s / (double)p.m);
     if (PREC == 16) v = (double)__half2float(__double2half(v));
     else if (PREC == 32) v = (double)__double2float_rn(v);
@@ -237,17 +246,18 @@ __global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial
 // s >= 512: C3 3.40 -> 3.30 ms, n = 512 9.8 -> 9.0 ms; 64-byte row segments).  16 is taken for FP64, and for
 // FP16/FP32 sketches with s >= 1024 where stage 2 dominates, when the matrix is long enough for whole sign words
 // per tile row (m2 % 32 == 0)
-static int k1_tile_w(int64_t m, int prec, int s)
+static int k1_tile_w(int64_t m, int prec, int s, int reim)
 {
+    if (reim) return 32;                               // the variant is built for the 32-wide tile only
     if (prec == 64) return (s >= 512 && m >= 512 * 32) ? 8 : (m >= 256 * 32 ? 16 : 32);
     return (s >= 1024 && m >= 512 * 32) ? 16 : 32;     // measured: s = 256 slower (0.50 -> 0.58 ms at C2), 512 equal, 1024 6.9 -> 6.0 ms
 }
 
-static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec)
+static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec, int reim)
 {
     K1Params p;
-    p.m = m; p.lda = lda; p.n = n; p.s = s;
-    const int K1_W = k1_tile_w(m, prec, s);
+    p.m = m; p.lda = lda; p.n = n; p.s = s; p.reim = reim;
+    const int K1_W = k1_tile_w(m, prec, s, reim);
     const int m1max = ((prec == 64) ? 128 : 256) * (32 / K1_W);    // 68 KB tile (W = 8: 74 KB)
     int64_t m1 = m / K1_W;
     if (m1 > m1max) m1 = m1max;
@@ -266,39 +276,52 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec)
 
 size_t k1_workspace_bytes(int64_t m, int n, int s, int prec)
 {
-    K1Params p = k1_params(m, n, m, s, prec);
-    const size_t fft = (size_t)((n + 1) / 2) * p.chunks * 2 * (size_t)s * sizeof(double);
+    size_t fft = 0;
+    for (int reim = 0; reim < 2; ++reim) {             // either variant may run in this workspace
+        K1Params p = k1_params(m, n, m, s, prec, reim);
+        const size_t b = (size_t)((n + 1) / 2) * p.chunks * (reim ? 4 : 2) * (size_t)s * sizeof(double);
+        if (b > fft) fft = b;
+    }
     const size_t tc = k1_tc_workspace_bytes();
     return fft > tc ? fft : tc;
 }
 
-template <typename T, int PREC, int W>
+template <typename T, int PREC, int W, bool REIM = false>
 static void k1_launch_t(const K1Params& p_in, const double* A, const uint64_t* signs, const int64_t* idx,
                         double* partial, double* As, Status* st, cudaStream_t stream)
 {
     K1Params p = p_in;
-    size_t smem = (size_t)p.m1 * (W + 1) * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + 2 * (size_t)p.s * sizeof(double);
+    size_t smem = (size_t)p.m1 * (W + 1) * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + (REIM ? 4 : 2) * (size_t)p.s * sizeof(double);
     p.dtab = smem + (size_t)p.s * sizeof(Cx<T>) <= 200 * 1024;
     if (p.dtab) smem += (size_t)p.s * sizeof(Cx<T>);
-    auto k = mrcqr_k1_srtt<T, PREC, W>;
+    auto k = mrcqr_k1_srtt<T, PREC, W, REIM>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int grid = ((p.n + 1) / 2) * p.chunks;
     k<<<grid, K1_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
-    mrcqr_k1_finalize<PREC><<<(p.s * p.n + 255) / 256, 256, 0, stream>>>(p, partial, As, st);
+    mrcqr_k1_finalize<PREC><<<((REIM ? 2 : 1) * p.s * p.n + 255) / 256, 256, 0, stream>>>(p, partial, As, st);
 }
 
 int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int s,
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
-                   Status* st, cudaStream_t stream)
+                   Status* st, cudaStream_t stream, int reim)
 {
+    if (reim) {                                        // Re+Im variant: FFT form, 32-wide tiles
+        K1Params p = k1_params(m, n, lda, s, prec, 1);
+        p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
+        double* partial = reinterpret_cast<double*>(k1_work);
+        if (prec == 16) k1_launch_t<float, 16, 32, true>(p, A, signs, idx, partial, As, st, stream);
+        else if (prec == 32) k1_launch_t<float, 32, 32, true>(p, A, signs, idx, partial, As, st, stream);
+        else k1_launch_t<double, 64, 32, true>(p, A, signs, idx, partial, As, st, stream);
+        return 2;
+    }
     if (k1_tc_usable(m, n, lda, A, prec, s)) {
         const int k = launch_k1_tc(m, n, lda, A, s, signs, idx, k1_work, As, st, stream);
         if (k > 0) return k;                          // < 0: the tensor map could not be encoded -> FFT form
     }
-    K1Params p = k1_params(m, n, lda, s, prec);
+    K1Params p = k1_params(m, n, lda, s, prec, 0);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
     double* partial = reinterpret_cast<double*>(k1_work);
-    const int tw_ = k1_tile_w(m, prec, s);
+    const int tw_ = k1_tile_w(m, prec, s, 0);
     const bool w16 = tw_ == 16;
     if (prec == 16) { if (w16) k1_launch_t<float, 16, 16>(p, A, signs, idx, partial, As, st, stream);
                       else k1_launch_t<float, 16, 32>(p, A, signs, idx, partial, As, st, stream); }

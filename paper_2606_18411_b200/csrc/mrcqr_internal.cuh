@@ -108,7 +108,7 @@ __device__ __forceinline__ void k2_prepare(const double* Rs, int n, double* RsPr
 size_t k1_workspace_bytes(int64_t m, int n, int s, int prec);
 int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int s,
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
-                   Status* st, cudaStream_t stream);
+                   Status* st, cudaStream_t stream, int reim = 0);      // reim: 2s rows, Im X[S] below Re X[S]
 
 // K1, tensor-core form for the FP16 sketch with s <= 128 (k1_tc.cu)
 bool k1_tc_usable(int64_t m, int n, int64_t lda, const double* A, int prec, int s);

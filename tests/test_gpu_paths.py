@@ -280,3 +280,49 @@ def test_graph_replay_gives_the_same_bits(orc, m, n, prec):
         assert rc in (0, 2)
     finally:
         B.mrcqr_set_graph(False)
+
+
+@pytest.mark.parametrize("m,n,s,prec,tol", [
+    (1 << 13, 6, 20, 64, 1e-12),       # FP64, single chunk
+    (1 << 14, 33, 100, 32, 5e-5),      # FP32, odd n (last column pair half empty), 2s = 200 sketch rows
+    (1 << 15, 64, 128, 16, 1e-2),      # the C1 geometry at small m: FP16, 2s = 256 rows (the FFT form, not the tensor-core one)
+    (1 << 12, 150, 300, 32, 5e-5),     # n > 64: blocked sketch QR on 600 rows, store-Y stage 2
+])
+def test_reim_sketch_variant(orc, m, n, s, prec, tol):
+    """mrcqr_set_sketch_reim: the 2s x n sketch [Re X[S]; Im X[S]] against the oracle's, then the
+    whole factorization with that sketch: same invariants, and R equal to the oracle's stages run on the oracle's
+    Re+Im sketch (Q, R are unique given diag(R) > 0, so the sketch only enters through rounding)."""
+    AT = inputs.make_A(m, n, 4, 600 + n, 601 + n, "cuda")
+    A = np.asfortranarray(to_np(AT))
+    seed = 1200 + n
+    signs, idx = orc.draw(m, s, seed)
+    As_o = orc.sketch_reim(A, signs, idx)
+    dsigns, didx = draw_to_dev(signs, idx)
+    p = {16: B.FP16, 32: B.FP32, 64: B.FP64}[prec]
+    B.mrcqr_set_sketch_reim(True)
+    try:
+        Rs, As = B.mrcqr_sketch(AT, p, dsigns, didx, want_As=True)
+        Asg = to_np(As)
+        assert Asg.shape == (2 * s, n)
+        assert relf(Asg, As_o) <= tol
+        assert relf(Asg[s:], As_o[s:]) <= 2 * tol          # the imaginary rows on their own
+        if prec == 16:
+            assert np.array_equal(Asg, Asg.astype(np.float16).astype(np.float64))
+        # R_s is the R factor of the GPU's own sketch: R_s^T R_s = A_s^T A_s, upper triangular, diag > 0
+        Rsn = to_np(Rs)
+        assert np.all(np.diag(Rsn) > 0) and np.array_equal(np.tril(Rsn, -1), np.zeros((n, n)))
+        assert relf(Rsn.T @ Rsn, Asg.T @ Asg) <= 1e-12
+        QT, R = B.mrcqr_factor(AT, p, s, seed)
+    finally:
+        B.mrcqr_set_sketch_reim(False)
+    Q, Rn = to_np(QT), to_np(R)
+    assert orc.orth_error_fro(Q) <= 1e-13
+    assert orc.residual_fro(A, Q, Rn) <= 1e-13
+    assert np.all(np.diag(Rn) > 0)
+    o = orc.factor(A, s, seed)                              # Re-only oracle factorization: same unique (Q, R)
+    kappa = np.linalg.cond(o["R"])
+    assert np.linalg.norm(Rn - o["R"]) <= 10 * kappa * n * U * np.linalg.norm(o["R"])
+    assert np.linalg.norm(Q - o["Q"]) <= 10 * kappa * n * U
+    # and the switch is off again: the default sketch has s rows
+    _, As1 = B.mrcqr_sketch(AT, p, dsigns, didx, want_As=True)
+    assert to_np(As1).shape == (s, n)
