@@ -102,6 +102,9 @@ __device__ __forceinline__ void gram_accumulate(double (&acc)[MAXOWN][2], const 
     }
 }
 
+// Every element of a partial belongs to ONE thread for the whole kernel, so later flushes add with a result-less
+// atomicAdd (RED.ADD.F64: fire and forget, same rounding as DADD, applied in program order for one thread and one
+// address: still deterministic) instead of a load-add-store whose load latency every warp would wait out.
 template <int NB, int NWG, int ROLE, int MAXOWN>
 __device__ __forceinline__ void gram_flush(double (&acc)[MAXOWN][2], double* part, int n16, bool first, int lane)
 {
@@ -114,7 +117,7 @@ __device__ __forceinline__ void gram_flush(double (&acc)[MAXOWN][2], double* par
                 constexpr int slot = gram_slot<NB, NWG>(ROLE, I, J);
                 double* dst = part + (size_t)(8 * J + 2 * t) * n16 + 8 * I + g;
                 if (first) { dst[0] = acc[slot][0]; dst[n16] = acc[slot][1]; }
-                else { dst[0] += acc[slot][0]; dst[n16] += acc[slot][1]; }
+                else { atomicAdd(dst, acc[slot][0]); atomicAdd(dst + n16, acc[slot][1]); }
                 acc[slot][0] = acc[slot][1] = 0.0;
             }
         });

@@ -142,7 +142,7 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
                         const int I = 2 * pp[u] + (b >> 1), J = 2 * qq[u] + (b & 1);
                         double* dst = part + (size_t)(8 * J + 2 * t) * n16 + 8 * I + g;
                         if (first_tile) { dst[0] = acc[u][b][0]; dst[n16] = acc[u][b][1]; }
-                        else { dst[0] += acc[u][b][0]; dst[n16] += acc[u][b][1]; }
+                        else { atomicAdd(dst, acc[u][b][0]); atomicAdd(dst + n16, acc[u][b][1]); }    // RED: see gram_flush
                     }
                 }
             }

@@ -177,7 +177,7 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
             for (int b = 0; b < 8; ++b) {
                 double* dst = part + (size_t)(64 * wj + 8 * b + 2 * t) * SY_B + 32 * wi + 8 * a + g;
                 if (first) { dst[0] = acc[a][b][0]; dst[SY_B] = acc[a][b][1]; }
-                else { dst[0] += acc[a][b][0]; dst[SY_B] += acc[a][b][1]; }
+                else { atomicAdd(dst, acc[a][b][0]); atomicAdd(dst + SY_B, acc[a][b][1]); }   // RED: see gram_flush
                 acc[a][b][0] = acc[a][b][1] = 0.0;
             }
         first = false;
