@@ -90,7 +90,10 @@ class ClockSampler:
 
 def workload(name):
     from paper_2606_18411_b200 import inputs
-    cfg = dict(inputs.CONFIGS[name])
+    if name.startswith("C4n"):          # a point of the column sweep (configs[4]), FP16 sketch: "C4n16", "C4n32", ...
+        cfg = inputs.sweep_config(int(name[3:]), 16)
+    else:
+        cfg = dict(inputs.CONFIGS[name])
     cfg["name"] = name
     return cfg
 
@@ -382,7 +385,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
+    ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3", "C4n16", "C4n32", "C4n64", "C4n128", "C4n256", "C4n512"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--stability", action="store_true", help="orthogonality / residual vs kappa on the paper's eq.(3) matrices")
     ap.add_argument("--sweep", action="store_true", help="per-stage table over BASELINE.json configs 0-4 instead of the JSON line")

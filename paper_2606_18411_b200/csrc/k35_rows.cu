@@ -62,8 +62,14 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
 
     if (NB > 0) {
         constexpr int NBc = NB > 0 ? NB : 2;
-        constexpr int MAXOWN = gram_maxown<NBc, NW>();
-        constexpr int FLUSH_TILES = GRAM_CHAIN * 4 / TM;
+        // WP (n16 <= 32): the Gram of so few blocks is not worth a CTA-wide split (it kept 1-2 of the 4 warps busy
+        // between two CTA barriers per tile): every warp accumulates all blocks over ITS OWN slab, with no CTA
+        // barrier in the tile loop; the NW accumulator sets are summed in a fixed order (warp 0, through the
+        // slabs) only when a chain is flushed.
+        constexpr bool WP = (NB == 2 || NB == 4);
+        constexpr int NWG = WP ? 1 : NW;
+        constexpr int MAXOWN = gram_maxown<NBc, NWG>();
+        constexpr int FLUSH_TILES = WP ? GRAM_CHAIN * 4 / SR : GRAM_CHAIN * 4 / TM;
         double acc[MAXOWN][2];
 #pragma unroll
         for (int b = 0; b < MAXOWN; ++b) acc[b][0] = acc[b][1] = 0.0;
@@ -77,18 +83,46 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
             solve_slab<RG, 0, NBc>(slab, fragS, nB, lane);
             if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); }
             if (Ystore) { __syncwarp(); store_slab<SR, VEC>(slab, Ystore, ldys, m, n, row0, lane); }   // store-Y variant
-            __syncthreads();
+            const bool flush = (++since >= FLUSH_TILES) || (tile + gridDim.x >= ntiles);
+            if constexpr (WP) {
+                __syncwarp();
+                gram_accumulate<NBc, 1, 0, SR, 1, MAXOWN>(acc, slab, slab_stride, lane);
+                __syncwarp();
+                if (flush) {
+#pragma unroll
+                    for (int b = 0; b < MAXOWN; ++b) { slab[(2 * b) * 32 + lane] = acc[b][0]; slab[(2 * b + 1) * 32 + lane] = acc[b][1]; }
+                    __syncthreads();
+                    if (warp == 0) {
+#pragma unroll
+                        for (int b = 0; b < MAXOWN; ++b)
+#pragma unroll
+                            for (int w = 1; w < NW; ++w) {
+                                acc[b][0] += Ysm[(size_t)w * slab_stride + (2 * b) * 32 + lane];
+                                acc[b][1] += Ysm[(size_t)w * slab_stride + (2 * b + 1) * 32 + lane];
+                            }
+                        gram_flush<NBc, 1, 0, MAXOWN>(acc, part, n16, first, lane);
+                    } else {
+#pragma unroll
+                        for (int b = 0; b < MAXOWN; ++b) acc[b][0] = acc[b][1] = 0.0;
+                    }
+                    __syncthreads();
+                    zero_pad_columns<SR>(slab, n, n16, lane);        // the scratch use above ran over the padding columns
+                    __syncwarp();
+                    first = false; since = 0;
+                }
+            } else {
+                __syncthreads();
 #define GRAM_ACC(R_) gram_accumulate<NBc, NW, R_, SR, NW, MAXOWN>(acc, Ysm, slab_stride, lane);
-            MRCQR_ROLE_SWITCH(GRAM_ACC)
+                MRCQR_ROLE_SWITCH(GRAM_ACC)
 #undef GRAM_ACC
-            ++since;
-            if (since >= FLUSH_TILES || tile + gridDim.x >= ntiles) {
+                if (flush) {
 #define GRAM_FLUSH(R_) gram_flush<NBc, NW, R_, MAXOWN>(acc, part, n16, first, lane);
-                MRCQR_ROLE_SWITCH(GRAM_FLUSH)
+                    MRCQR_ROLE_SWITCH(GRAM_FLUSH)
 #undef GRAM_FLUSH
-                first = false; since = 0;
+                    first = false; since = 0;
+                }
+                __syncthreads();
             }
-            __syncthreads();
         }
         return;
     }
