@@ -27,8 +27,8 @@ sys.path.insert(0, ROOT)
 METRIC = "MRCQR FP64 thin-QR ms per factorization"
 FP64_DMMA_PEAK_TFLOPS = 37.2      # measured on this pool's B200 (profiles/r01_peaks.md), DMMA.8x8x4 issue peak
 # DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the ncu --set full capture of
-# config C1 summarised in profiles/r01_ncu_full_v7.md; only valid for that workload
-NCU_TRAFFIC_C1 = {"k5_form_q": 536.97e6 + 486.98e6, "k3_gram": 554.86e6 + 22.85e6}
+# config C1 summarised in profiles/r01_ncu_full_final.md; only valid for that workload
+NCU_TRAFFIC_C1 = {"k5_form_q": 537.0e6 + 480.4e6, "k3_gram": 556.2e6 + 23.2e6}    # profiles/r01_ncu_full_final.md
 HBM_FALLBACK_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
 
 

@@ -66,7 +66,7 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
         // between two CTA barriers per tile): every warp accumulates all blocks over ITS OWN slab, with no CTA
         // barrier in the tile loop; the NW accumulator sets are summed in a fixed order (warp 0, through the
         // slabs) only when a chain is flushed.
-        constexpr bool WP = (NB == 2 || NB == 4);
+        constexpr bool WP = (NB == 2 || NB == 4 || NB == 6);
         constexpr int NWG = WP ? 1 : NW;
         constexpr int MAXOWN = gram_maxown<NBc, NWG>();
         constexpr int FLUSH_TILES = WP ? GRAM_CHAIN * 4 / SR : GRAM_CHAIN * 4 / TM;
