@@ -129,6 +129,24 @@ def test_stage2_ragged_rows(orc, m):
     assert relf(to_np(R), orc.triu_mul(Rco, Rs)) <= 1e-14
 
 
+@pytest.mark.parametrize("m,n", [((1 << 22) + 100, 16), ((1 << 22) + 100, 24), ((1 << 21) + 100, 40), (5000, 40)])
+def test_warp_private_gram_flushes_mid_run(orc, m, n):
+    # K3 at n16 <= 48 keeps one Gram accumulator set per warp and sums the four sets of a CTA (fixed order) every
+    # 32 tiles and at the end.  The large m values give every CTA more than 32 tiles, so that the first flush
+    # (plain store) AND the later ones (ordered adds) run; 5000 rows: a single flush, ragged last tile, n16 = 48.
+    AT = inputs.gaussian_colmajor(m, n, 900 + n, "cuda")
+    A = to_np(AT)
+    rng = np.random.default_rng(n)
+    Rs = np.triu(rng.standard_normal((n, n))) + 6 * np.eye(n)
+    Rc, G = B.mrcqr_precondition_gram(AT, colmajor_to_dev(Rs), want_G=True)
+    Go = orc.gram(orc.row_solve(A, Rs))
+    assert relf(to_np(G), Go) <= 1e-13
+    Rc2, G2 = B.mrcqr_precondition_gram(AT, colmajor_to_dev(Rs), want_G=True)
+    assert torch.equal(G, G2) and torch.equal(Rc, Rc2)          # deterministic split-m reduction
+    Rco, info = orc.cholesky_upper(Go)
+    assert info == 0 and relf(to_np(Rc), Rco) <= 1e-12
+
+
 def test_lda_padding_and_unaligned_base(orc):
     # lda > m and a base pointer that is only 8-byte aligned (scalar load path)
     m, n, lda = 2048, 16, 2048 + 6
