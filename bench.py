@@ -159,6 +159,18 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(value, device="cpu"):
+    """The multi-GPU timing rule: every rank contributes its device-measured time, the MAX is the job's.
+    No-op for a single process.  (Replicas only: this and the barrier are the only collectives bench.py uses.)"""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -210,10 +222,7 @@ def run_ours(args):
             stage_sum[k] += v
     B.mrcqr_set_timing(False)
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, "cuda")
     ms = total_ms / args.steps
     stages = {k: v / args.steps for k, v in stage_sum.items()}
 
@@ -245,10 +254,7 @@ def run_ours(args):
         B.mrcqr_factor_host(A_host, prec, s, seed, Q_host, R_host)
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, "cuda")
 
     if rank == 0:
         hbm_peak, how = measured_peaks()
