@@ -41,17 +41,54 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    """SM clock and throttle reasons sampled DURING the timed region.  The timed region of one bench run is
+    tens of milliseconds, so the sampler polls NVML in-process every 4 ms (pynvml, the same counters nvidia-smi
+    prints); if NVML cannot be opened it falls back to an `nvidia-smi -lms 200` child process."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    REASONS = (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4))
 
     def __init__(self, gpu_index):
-        self.idx, self.proc = gpu_index, None
-        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.idx, self.proc, self.thread, self.rows = gpu_index, None, None, []
+        self.tmp = None
+
+    def _physical_index(self):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+        ids = [v.strip() for v in vis.split(",") if v.strip()]
+        if ids and self.idx < len(ids) and ids[self.idx].isdigit():
+            return int(ids[self.idx])
+        return self.idx
+
+    def _poll(self):
+        nv, h = self.nv
+        while True:
+            try:
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                self.rows.append((float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)),
+                                  float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)), int(mask)))
+            except Exception:
+                pass
+            if self.halt.wait(0.004):
+                return
 
     def start(self):
         try:
+            import threading
+            import pynvml as nv
+            nv.nvmlInit()
+            self.nv = (nv, nv.nvmlDeviceGetHandleByIndex(self._physical_index()))
+            self.halt = threading.Event()
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.thread = None
+        try:
+            self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
                                           "--format=csv,noheader,nounits", "-lms", "200"],
                                          stdout=self.tmp, stderr=subprocess.DEVNULL)
@@ -59,27 +96,36 @@ class ClockSampler:
             self.proc = None
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
-        if self.proc is None:
-            return out
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except Exception:
-            self.proc.kill()
-        self.tmp.flush()
-        rows = [l.strip().split(",") for l in open(self.tmp.name) if l.strip()]
-        os.unlink(self.tmp.name)
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         sm, reasons = [], set()
-        for r in rows:
-            try:
-                r = [x.strip() for x in r]
-                sm.append(float(r[1])); out["sm_max_mhz"] = float(r[2])
-                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
-                    if v.lower().startswith("active"):
+        if self.thread is not None:
+            self.halt.set()
+            self.thread.join(timeout=2)
+            for clk, mx, mask in self.rows:
+                sm.append(clk); out["sm_max_mhz"] = mx
+                for name, bit in self.REASONS:
+                    if mask & bit:
                         reasons.add(name)
+            out["source"] = "nvml, 4 ms"
+        elif self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
             except Exception:
-                pass
+                self.proc.kill()
+            self.tmp.flush()
+            rows = [l.strip().split(",") for l in open(self.tmp.name) if l.strip()]
+            os.unlink(self.tmp.name)
+            for r in rows:
+                try:
+                    r = [x.strip() for x in r]
+                    sm.append(float(r[1])); out["sm_max_mhz"] = float(r[2])
+                    for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                        if v.lower().startswith("active"):
+                            reasons.add(name)
+                except Exception:
+                    pass
+            out["source"] = "nvidia-smi -lms 200"
         if sm:
             sm.sort()
             out["sm_mhz"] = sm[len(sm) // 2]
