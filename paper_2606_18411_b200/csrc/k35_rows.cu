@@ -45,7 +45,7 @@ __device__ __forceinline__ void sb_to_pq(int sb, int& p, int& q)
 // NB > 0: n16 = 8*NB <= 128, compile-time Gram ownership, accumulators live in registers across tiles.
 // NB = 0: n16 > 128, 16x16 super-blocks in sweeps, flushed to the L2-resident partial every tile.
 template <int RG, int NW, int NB, bool VEC>
-__global__ void __launch_bounds__(NW * 32, (RG == 4 && NW == 4) ? (NB == 2 ? 5 : (NB == 4 ? 4 : 3)) : 1)
+__global__ void __launch_bounds__(NW * 32, (RG == 4 && NW == 4) ? (NB == 2 ? 5 : 3) : 1)
 mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__ A,
               const double2* __restrict__ fragS, double* __restrict__ partials,
               int64_t ntiles, double* __restrict__ Ydump, double* __restrict__ Ystore, int64_t ldys)
