@@ -190,7 +190,7 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
 // mode 3: both solves (y = a Rs^-1, q = y Rc^-1); mode 1: only the first (store-Y form of stage 2a for
 // n16 > 128, Y goes to the Q buffer); mode 2: only the second, in place on the stored Y.
 // warps per CTA by panel size: small panels need few registers, and a 4 KB slab needs many warps in flight
-constexpr int k5_max_warps(int nbt) { return nbt == 2 ? 20 : (nbt == 4 ? 16 : 12); }
+constexpr int k5_max_warps(int nbt) { return nbt == 2 ? 32 : (nbt == 4 ? 16 : 12); }
 
 template <int RG, int NBT, bool VEC>
 __global__ void __launch_bounds__(32 * k5_max_warps(NBT), 1)
