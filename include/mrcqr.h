@@ -56,6 +56,14 @@ enum {
 int mrcqr_draw(int64_t m, int s, uint64_t seed, uint64_t* signs_host, int64_t* idx_host);
 
 /*
+ * The same draw (Algorithm 2 step 1) exactly as mrcqr_factor performs it, into DEVICE buffers: the
+ * ceil(m/64) sign words by the device kernel of the library, the s bins drawn on the host and copied.  The words
+ * and bins are bit-identical to mrcqr_draw's (and the oracle's); the GPU tests pin that.  signs / idx: device.
+ * Synchronises the stream.  Returns as mrcqr_draw, or 4.
+ */
+int mrcqr_draw_device(int64_t m, int s, uint64_t seed, uint64_t* signs, int64_t* idx, void* stream);
+
+/*
  * Stage 1, Algorithm 2 steps 2-6: the subsampled randomized trigonometric
  * transform and the sketch QR.
  *   x~ = fl_p(D a_j) (sign-bit flip + round to p), X = DFT_m(x~) down each column,
@@ -104,8 +112,9 @@ int mrcqr_factor(int64_t m, int n, int64_t lda, const double* A, double* Q, doub
                  mrcqr_prec_t sketch_prec, int s, uint64_t seed, void* stream);
 
 /*
- * mrcqr_factor with HOST buffers: copies A to the device (library-owned buffers), factors,
- * copies Q and R back; synchronous.  This is the end-to-end path bench.py times as `e2e`.
+ * mrcqr_factor with HOST buffers: copies the m x n part of A (lda >= m; the padding rows m..lda-1 of a column are
+ * neither read nor written) to library-owned device buffers on a stream of the library's own, factors, copies Q
+ * (same lda) and R back; synchronous.  This is the end-to-end path bench.py times as `e2e`.
  */
 int mrcqr_factor_host(int64_t m, int n, int64_t lda, const double* A_host, double* Q_host,
                       double* R_host, mrcqr_prec_t sketch_prec, int s, uint64_t seed);
@@ -194,9 +203,13 @@ int mrcqr_set_sketch_reim(int on);
  * kernels, copies and the status read-back of mrcqr_factor are captured ONCE into a CUDA graph per (m, n, lda, A, Q, R,
  * precision, s) and replayed by later calls with the same arguments; the seed and the drawn bins are data of the graph
  * (read from pinned host memory at replay), so they may change from call to call.  Same results bit for bit.  Per-kernel
- * timing (mrcqr_set_timing) takes the ordinary path.  Returns 0.
+ * timing (mrcqr_set_timing) takes the ordinary path.  Stream capture is not permitted on the legacy default stream
+ * (stream = NULL): such calls take the ordinary path; mrcqr_last_used_graph() tells which one ran.  Returns 0.
  */
 int mrcqr_set_graph(int on);
+
+/* 1 if the last mrcqr_factor / mrcqr_factor_host call replayed (or captured and replayed) a CUDA graph, else 0. */
+int mrcqr_last_used_graph(void);
 
 /*
  * Test hook for the "bit-identical Y" requirement: runs the stage-2a and the stage-2b

@@ -39,6 +39,7 @@ def lib():
         L = C.CDLL(path)
         i64, u64, vp, ci = C.c_int64, C.c_uint64, C.c_void_p, C.c_int
         L.mrcqr_draw.argtypes = [i64, ci, u64, vp, vp]
+        L.mrcqr_draw_device.argtypes = [i64, ci, u64, vp, vp, vp]
         L.mrcqr_sketch.argtypes = [i64, ci, i64, vp, ci, ci, vp, vp, vp, vp, vp]
         L.mrcqr_precondition_gram.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
         L.mrcqr_form_q.argtypes = [i64, ci, i64, vp, vp, vp, i64, vp, vp, vp]
@@ -57,7 +58,7 @@ def lib():
         L.mrcqr_set_sketch_reim.argtypes = [ci]
         L.mrcqr_set_graph.argtypes = [ci]
         L.mrcqr_last_timing.argtypes = [vp]
-        for f in ("mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
+        for f in ("mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
                   "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
                   "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"):
             getattr(L, f).restype = ci
@@ -65,7 +66,7 @@ def lib():
     return _lib
 
 
-EXPORTS = ["mrcqr_draw", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
+EXPORTS = ["mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
            "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"]
 
@@ -99,6 +100,21 @@ def mrcqr_draw(m, s, seed):
     return signs, idx[:s].clone()
 
 
+def mrcqr_draw_device(m, s, seed, stream=None):
+    """The draw as mrcqr_factor performs it (device kernel for the sign words): (signs int64 tensor, idx int64 tensor) on the GPU."""
+    signs = torch.zeros((m + 63) // 64, dtype=torch.int64, device="cuda")
+    idx = torch.zeros(max(s, 1), dtype=torch.int64, device="cuda")
+    _chk(lib().mrcqr_draw_device(m, s, seed, signs.data_ptr(), idx.data_ptr(), _stream(stream)))
+    return signs, idx[:s].clone()
+
+
+def _out(QT, AT):
+    """A caller-supplied Q must have A's shape and leading dimension (the C ABI gives mrcqr_factor one lda)."""
+    assert QT.is_cuda and QT.dtype == torch.float64 and QT.device == AT.device
+    assert QT.shape == AT.shape and QT.stride(1) == 1 and QT.stride(0) == AT.stride(0), "Q must share A's shape and lda"
+    return QT
+
+
 def mrcqr_sketch(AT, prec, signs, idx, want_As=False, stream=None):
     """Stage 1.  signs/idx: device tensors.  Returns (Rs (n,n) col-major, As (n,s) col-major or None)."""
     m, n, lda, pA = _mat(AT)
@@ -127,6 +143,7 @@ def mrcqr_form_q(AT, Rs, Rc, QT=None, stream=None):
     m, n, lda, pA = _mat(AT)
     if QT is None:
         QT = torch.empty((n, m), dtype=torch.float64, device=AT.device)
+    assert QT.is_cuda and QT.dtype == torch.float64 and QT.shape == AT.shape and QT.stride(1) == 1 and QT.stride(0) >= m
     R = torch.empty((n, n), dtype=torch.float64, device=AT.device)
     rc = lib().mrcqr_form_q(m, n, lda, pA, Rs.data_ptr(), Rc.data_ptr(), QT.stride(0), QT.data_ptr(),
                             R.data_ptr(), _stream(stream))
@@ -141,6 +158,7 @@ def mrcqr_factor(AT, prec, s, seed, QT=None, R=None, stream=None, check=True):
         QT = torch.empty_strided((n, m), (lda, 1), dtype=torch.float64, device=AT.device)
     if R is None:
         R = torch.empty((n, n), dtype=torch.float64, device=AT.device)
+    _out(QT, AT)
     rc = lib().mrcqr_factor(m, n, lda, pA, QT.data_ptr(), R.data_ptr(), prec, s, seed, _stream(stream))
     if not check:
         return rc
@@ -153,7 +171,9 @@ def mrcqr_factor_host(AT_host, prec, s, seed, QT_host=None, R_host=None):
     assert (not AT_host.is_cuda) and AT_host.dtype == torch.float64 and AT_host.stride(1) == 1
     n, m = AT_host.shape
     if QT_host is None:
-        QT_host = torch.empty((n, m), dtype=torch.float64, pin_memory=True)
+        QT_host = torch.empty((n, AT_host.stride(0)), dtype=torch.float64, pin_memory=True)[:, :m]
+    assert (not QT_host.is_cuda) and QT_host.shape == AT_host.shape and QT_host.stride(1) == 1 \
+        and QT_host.stride(0) == AT_host.stride(0), "Q_host must share A_host's shape and lda"
     if R_host is None:
         R_host = torch.empty((n, n), dtype=torch.float64, pin_memory=True)
     rc = lib().mrcqr_factor_host(m, n, AT_host.stride(0), AT_host.data_ptr(), QT_host.data_ptr(),
@@ -203,6 +223,7 @@ def mrcqr_factor_auto(AT, first_prec, s, seed, tol=0.0, QT=None, R=None, stream=
     if R is None:
         R = torch.empty((n, n), dtype=torch.float64, device=AT.device)
     used, orth = C.c_int(0), C.c_double(0.0)
+    _out(QT, AT)
     rc = lib().mrcqr_factor_auto(m, n, lda, pA, QT.data_ptr(), R.data_ptr(), first_prec, s, seed, float(tol),
                                  C.byref(used), C.byref(orth), _stream(stream))
     if not check:
@@ -218,6 +239,7 @@ def mrcqr_cholqr(AT, passes=1, QT=None, R=None, stream=None, check=True):
         QT = torch.empty_strided((n, m), (lda, 1), dtype=torch.float64, device=AT.device)
     if R is None:
         R = torch.empty((n, n), dtype=torch.float64, device=AT.device)
+    _out(QT, AT)
     rc = lib().mrcqr_cholqr(m, n, lda, pA, QT.data_ptr(), R.data_ptr(), passes, _stream(stream))
     if not check:
         return rc
@@ -238,6 +260,10 @@ def mrcqr_kappa_probe(AT, stream=None):
 def mrcqr_set_graph(on):
     """Repeated-call mode: mrcqr_factor replays a CUDA graph captured per (shape, buffers)."""
     lib().mrcqr_set_graph(1 if on else 0)
+
+
+def mrcqr_last_used_graph():
+    return bool(lib().mrcqr_last_used_graph())
 
 
 _reim = False

@@ -52,7 +52,7 @@ static void draw_bins_host(int64_t m, int s, uint64_t seed, int64_t* idx)
 
 // ---- workspace -----------------------------------------------------------------------------------
 struct Layout {
-    size_t status, signs, idx, As, Rs, RsPrep, RcPrep, G16, Rc, betas, k1, k3, total;
+    size_t status, signs, idx, As, Rs, RsPrep, RcPrep, G16, Rc, Rtmp, betas, k1, k3, total;
 };
 
 static size_t al(size_t x) { return (x + 255) / 256 * 256; }
@@ -71,9 +71,10 @@ static Layout make_layout(int64_t m, int n, int s, int prec)
     L.RcPrep = o; o += al(n16 * n16 * 8);
     L.G16 = o;    o += al(n16 * n16 * 8);
     L.Rc = o;     o += al((size_t)n * n * 8);
+    L.Rtmp = o;   o += al((size_t)2 * n * n * 8);                        // CholQR2: R1, R2
     L.betas = o;  o += al((size_t)n * 8);
     L.k1 = o;     o += al(s > 0 ? k1_workspace_bytes(m, n, s, prec) : 0);
-    L.k3 = o;     o += al(std::max(k3_partials_bytes(n), syrk_partials_bytes(n)));
+    L.k3 = o;     o += al(std::max(k3_partials_bytes(n), syrk_partials_bytes(n)));   // Gram partials of either stage-2 form
     L.total = o;
     return L;
 }
@@ -84,6 +85,8 @@ struct Ctx {
     int64_t* h_idx = nullptr; size_t h_idx_cap = 0;   // pinned staging of the bins
     double* hA = nullptr; double* hQ = nullptr; double* hR = nullptr; size_t hA_bytes = 0, hR_bytes = 0; // host-path device buffers
     int last_info = 0, last_launches = 0;
+    bool last_graph = false;                 // the last mrcqr_factor call replayed a CUDA graph
+    cudaStream_t host_stream = nullptr;      // mrcqr_factor_host: a non-blocking stream of the library's own
     bool timing = false; cudaEvent_t ev[8] = {}; bool ev_ok = false; float stage_ms[8] = {};
     bool have_device = false, probed = false;
     bool store_y = false;                    // mrcqr_set_store_y: store-Y variant also for n16 <= 128
@@ -135,6 +138,7 @@ static bool ensure_hidx(size_t count)
 static int finish(const Layout& L, cudaStream_t st, int launches)
 {
     g.last_launches = launches;
+    g.last_graph = false;
     cudaMemcpyAsync(g.h_status, g.ws + L.status, 8, cudaMemcpyDeviceToHost, st);
     if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) return MRCQR_ERR_CUDA;
     g.last_info = g.h_status[1];
@@ -214,6 +218,27 @@ extern "C" int mrcqr_draw(int64_t m, int s, uint64_t seed, uint64_t* signs_host,
     return 0;
 }
 
+// The draw exactly as mrcqr_factor performs it: sign words by the device kernel, bins on the host and copied.
+extern "C" int mrcqr_draw_device(int64_t m, int s, uint64_t seed, uint64_t* signs, int64_t* idx, void* stream)
+{
+    if (m < 1) return -1;
+    if (s < 0 || (int64_t)s > m / 2 + 1) return -2;
+    if (!signs) return -4;
+    if (!idx && s > 0) return -5;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    if (!ensure_hidx((size_t)std::max(s, 1))) return MRCQR_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t nw = (m + 63) / 64;
+    mrcqr_draw_signs<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed, nw, signs, nullptr);
+    if (s > 0) {
+        draw_bins_host(m, s, seed, g.h_idx);
+        cudaMemcpyAsync(idx, g.h_idx, sizeof(int64_t) * (size_t)s, cudaMemcpyHostToDevice, st);
+    }
+    g.last_launches = 1; g.last_graph = false;
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) return MRCQR_ERR_CUDA;
+    return 0;
+}
+
 extern "C" size_t mrcqr_workspace_bytes(int64_t m, int n, int s, mrcqr_prec_t prec)
 {
     if (m < 1 || n < 1 || n > N_MAX || !prec_ok((int)prec) || !device_ok()) return 0;
@@ -223,6 +248,7 @@ extern "C" size_t mrcqr_workspace_bytes(int64_t m, int n, int s, mrcqr_prec_t pr
 
 extern "C" int mrcqr_last_info(void) { return g.last_info; }
 extern "C" int mrcqr_last_launch_count(void) { return g.last_launches; }
+extern "C" int mrcqr_last_used_graph(void) { return g.last_graph ? 1 : 0; }
 
 extern "C" void mrcqr_shutdown(void)
 {
@@ -237,6 +263,7 @@ extern "C" void mrcqr_shutdown(void)
     if (g.hA) cudaFree(g.hA);
     if (g.hQ) cudaFree(g.hQ);
     if (g.hR) cudaFree(g.hR);
+    if (g.host_stream) cudaStreamDestroy(g.host_stream);
     g = Ctx();
 }
 
@@ -315,15 +342,8 @@ extern "C" int mrcqr_debug_dump_y(int64_t m, int n, int64_t lda, const double* A
     mrcqr_reset_status<<<1, 1, 0, st>>>(reinterpret_cast<Status*>(g.ws + L.status));
     double* Rc = reinterpret_cast<double*>(g.ws + L.Rc);
     int k = 1 + enqueue_gram(L, m, n, lda, A, Rs, nullptr, Rc, Y_stage2a, st);
-    // stage 2b writes its Q over the dump afterwards, so dump into 2b and form Q into 2a's twin: use
-    // Y_stage2b as the dump target and a scratch Q = Y_stage2b is not possible; Q goes to workspace-free
-    // path: reuse Y_stage2b for the dump and discard Q by writing it to Y_stage2b's rows AFTER the dump
-    // would destroy it -- so Q is written to a separate temporary.
-    double* Qtmp = nullptr;
-    if (cudaMalloc(&Qtmp, sizeof(double) * (size_t)m * n) != cudaSuccess) { cudaGetLastError(); return MRCQR_ERR_CUDA; }
-    k += enqueue_formq(L, m, n, lda, A, Rs, Rc, false, false, m, Qtmp, nullptr, Y_stage2b, st);
+    k += enqueue_formq(L, m, n, lda, A, Rs, Rc, false, false, m, nullptr, nullptr, Y_stage2b, st);   // Q = nullptr: not stored
     int rc = finish(L, st, k);
-    cudaFree(Qtmp);
     return rc;
 }
 
@@ -448,6 +468,7 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
         if (g.gexec) {
             *g.h_seed = seed;
             g.last_launches = g.glaunches;
+            g.last_graph = true;
             if (cudaGraphLaunch(g.gexec, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess ||
                 cudaGetLastError() != cudaSuccess) return MRCQR_ERR_CUDA;
             g.last_info = g.h_status[1];
@@ -571,17 +592,16 @@ extern "C" int mrcqr_cholqr(int64_t m, int n, int64_t lda, const double* A, doub
     cudaStream_t st = (cudaStream_t)stream;
     int rc = cholqr_device(m, n, lda, A, lda, Q, R, st);
     if (rc != 0 || passes == 1) return rc;
-    // CholQR2: Algorithm 1 again on Q (in place), R = R2 R1
-    double *R1 = nullptr, *R2 = nullptr;
-    if (cudaMalloc(&R1, sizeof(double) * 2 * (size_t)n * n) != cudaSuccess) { cudaGetLastError(); return MRCQR_ERR_CUDA; }
-    R2 = R1 + (size_t)n * n;
+    // CholQR2: Algorithm 1 again on Q (in place), R = R2 R1; R1, R2 live in the workspace
+    Layout L = make_layout(m, n, 0, 64);
+    double* R1 = reinterpret_cast<double*>(g.ws + L.Rtmp);
+    double* R2 = R1 + (size_t)n * n;
     cudaMemcpyAsync(R1, R, sizeof(double) * (size_t)n * n, cudaMemcpyDeviceToDevice, st);
     rc = cholqr_device(m, n, lda, Q, lda, Q, R2, st);
     if (rc == 0) {
         launch_triu_mul(R2, R1, n, R, st);
         if (cudaStreamSynchronize(st) != cudaSuccess) rc = MRCQR_ERR_CUDA;
     }
-    cudaFree(R1);
     return rc;
 }
 
@@ -618,7 +638,8 @@ extern "C" int mrcqr_factor_host(int64_t m, int n, int64_t lda, const double* A_
     if (s <= 0) s = 3 * n;
     if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX || (g.reim && 2 * s > S_MAX)) return -8;
     if (!device_ok()) return MRCQR_ERR_CUDA;
-    const size_t bytes = sizeof(double) * (size_t)lda * n, rbytes = sizeof(double) * (size_t)n * n;
+    // device copies are packed (ld = m): only the m x n part of a host matrix with lda > m is touched
+    const size_t bytes = sizeof(double) * (size_t)m * n, rbytes = sizeof(double) * (size_t)n * n;
     if (bytes > g.hA_bytes) {
         if (g.hA) cudaFree(g.hA);
         if (g.hQ) cudaFree(g.hQ);
@@ -632,11 +653,15 @@ extern "C" int mrcqr_factor_host(int64_t m, int n, int64_t lda, const double* A_
         if (cudaMalloc(&g.hR, rbytes) != cudaSuccess) { cudaGetLastError(); return MRCQR_ERR_CUDA; }
         g.hR_bytes = rbytes;
     }
-    cudaStream_t st = 0;
-    if (cudaMemcpyAsync(g.hA, A_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return MRCQR_ERR_CUDA;
-    int rc = factor_device(m, n, lda, g.hA, lda, g.hQ, g.hR, (int)sketch_prec, s, seed, st);
+    if (!g.host_stream && cudaStreamCreateWithFlags(&g.host_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError(); g.host_stream = nullptr; return MRCQR_ERR_CUDA;
+    }
+    cudaStream_t st = g.host_stream;
+    const size_t row = sizeof(double) * (size_t)m, hpitch = sizeof(double) * (size_t)lda;
+    if (cudaMemcpy2DAsync(g.hA, row, A_host, hpitch, row, (size_t)n, cudaMemcpyHostToDevice, st) != cudaSuccess) return MRCQR_ERR_CUDA;
+    int rc = factor_device(m, n, m, g.hA, m, g.hQ, g.hR, (int)sketch_prec, s, seed, st);
     if (rc != 0) return rc;
-    cudaMemcpyAsync(Q_host, g.hQ, bytes, cudaMemcpyDeviceToHost, st);
+    cudaMemcpy2DAsync(Q_host, hpitch, g.hQ, row, row, (size_t)n, cudaMemcpyDeviceToHost, st);
     cudaMemcpyAsync(R_host, g.hR, rbytes, cudaMemcpyDeviceToHost, st);
     if (cudaStreamSynchronize(st) != cudaSuccess) return MRCQR_ERR_CUDA;
     return 0;

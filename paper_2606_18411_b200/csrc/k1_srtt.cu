@@ -8,12 +8,17 @@
 //   stage 1  a CTA stages an m1 x W tile (W = 32 or 16 consecutive t2, all t1; 256- or 128-byte coalesced
 //            row segments of the column-major A), applying the sign bit and the cast to p on the way
 //            in (DiagMult), and runs the 32 length-m1 FFTs in shared memory with
-//            radix-4 decimation-in-frequency passes (output left in bit-reversed order).  Two real
-//            columns ride in one complex transform (re = column 2c, im = column 2c+1).
-//   stage 2  for each sampled bin k_i only the residue k1 = k_i mod m1 is needed; the CTA multiplies
-//            Z[k1, t2] by W_m^{k_i t2}, takes the real part, and sums over its t2 (warp shuffle +
-//            a per-CTA accumulator); a finalize kernel adds the per-chunk partials in a fixed order,
-//            scales by sqrt(s/m) and rounds to p.
+//            radix-4 decimation-in-frequency passes (output left in bit-reversed order).  The input is
+//            real, so two ADJACENT t2 of the SAME column ride in one complex transform
+//            (z[t1][u] = x~[t1, 2u] + i x~[t1, 2u+1]: exactly the 16-byte pairs the loads fetch): a tile
+//            of W complex columns covers 2W consecutive t2 of one column of A, and a column's sketch
+//            depends on that column only ("column-wise": a zero column gives an exactly zero
+//            sketch column, a column scaled by 2^e an exactly scaled one).
+//   stage 2  for each sampled bin k_i only the residue k1 = k_i mod m1 is needed: with P = Z[k1] and
+//            Qn = Z[m1 - k1] of the packed transform, the even / odd t2 have E = (P + conj Qn) / 2 and
+//            O = -i (P - conj Qn) / 2; the thread that owns the bin multiplies them by W_m^{k_i t2},
+//            takes the real part and sums over the tile's t2 into a per-CTA accumulator; a finalize
+//            kernel adds the per-chunk partials in a fixed order, scales by sqrt(s/m) and rounds to p.
 // Same mathematical result as FFT-then-gather; pass 1 reads A exactly once in every precision.
 // T = float serves p = FP16 (inputs and outputs rounded to FP16, FP32 arithmetic) and p = FP32;
 // T = double serves p = FP64.  No fast-math intrinsics: twiddles come from sincospi.
@@ -22,9 +27,10 @@
 
 namespace mrcqr {
 
-// W = t2 values per tile (32: a warp instruction covers one tile row; 16: two rows, used for FP64 so that m1 = 256
-// fits the same 68 KB and the per-bin work of stage 2, which scales with s * m / m1, halves); the row stride of the
-// tile is W + 1 complex elements (odd: the per-bin gathers of stage 2 spread over the banks)
+// W = complex elements per tile row = 2W consecutive t2 of one column (32: a warp instruction covers one tile row;
+// 16: two rows, used for FP64 so that m1 = 256 fits the same 68 KB and the per-bin work of stage 2, which scales with
+// s * m / m1, halves); the row stride of the tile is W + 1 complex elements (odd: the per-bin gathers of stage 2
+// spread over the banks)
 constexpr int K1_NT = 256;
 constexpr int K1_NWARP = K1_NT / 32;
 
@@ -75,15 +81,14 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
     extern __shared__ __align__(16) unsigned char smraw[];
     Cx<T>* tile = reinterpret_cast<Cx<T>*>(smraw);                       // [m1][W + 1]
     Cx<T>* tw = tile + (size_t)p.m1 * K1_LD;                             // [m1]  W_m1^e
-    constexpr int NACC = REIM ? 4 : 2;                                    // Re a, Re b (, Im a, Im b)
+    constexpr int NACC = REIM ? 2 : 1;                                    // Re (, Im)
     double* colacc = reinterpret_cast<double*>(tw + p.m1);               // [NACC][s]
     Cx<T>* dstep = reinterpret_cast<Cx<T>*>(colacc + NACC * p.s);           // [s]  (cos, sin) of 2 pi k_i / m   (dtab only)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tcol = lane % W, sub = lane / W;
-    const int pair = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
-    const int ja = 2 * pair, jb = 2 * pair + 1;
-    const bool has_b = jb < p.n;
+    const int col = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
     const int m1 = p.m1;
+    const double* colA = A + (size_t)col * (size_t)p.lda;
 
     for (int e = tid; e < m1; e += K1_NT) {
         double sn, cs;
@@ -102,56 +107,48 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
     const int tile_lo = chunk * p.tiles_per_chunk;
     const int tile_hi = min(p.tiles_per_col, tile_lo + p.tiles_per_chunk);
     for (int tl = tile_lo; tl < tile_hi; ++tl) {
-        const int64_t t2_0 = (int64_t)tl * K1_W;
+        const int64_t t2_0 = (int64_t)tl * (2 * K1_W);
         __syncthreads();
-        // ---- load + DiagMult: 16-byte loads, a warp covers two 256-byte rows per instruction, eight
-        //      row pairs (16 loads per thread) in flight before the first conversion ------------------
+        // ---- load + DiagMult: lane (row, u) fetches the 16-byte pair x[t1, 2u], x[t1, 2u+1] = one complex element;
+        //      eight rows per thread (8 loads + 8 sign words) in flight before the first conversion -------------
         if (p.vec) {
-            constexpr int PRL = W / 2, RPI = 32 / PRL;            // lanes per row (double2 each), rows per instruction
-            const int half = lane / PRL, pr = lane % PRL;         // row within the group, double2 index
-            const double2* colA = reinterpret_cast<const double2*>(A + (size_t)ja * (size_t)p.lda + t2_0) + pr;
-            const double2* colB = reinterpret_cast<const double2*>(A + (size_t)(has_b ? jb : ja) * (size_t)p.lda + t2_0) + pr;
+            const double2* src = reinterpret_cast<const double2*>(colA + t2_0) + tcol;
             const int64_t m2h = p.m2 >> 1;                          // row stride in double2
-            for (int t1b = RPI * warp; t1b < m1; t1b += RPI * K1_NWARP * 8) {
-                double2 va[8], vb[8];
+            for (int t1b = warp * SUB + sub; t1b < m1; t1b += K1_NWARP * SUB * 8) {
+                double2 va[8];
                 unsigned sg[8];
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
-                    const int t1 = t1b + u * RPI * K1_NWARP + half;
-                    va[u] = make_double2(0.0, 0.0); vb[u] = va[u]; sg[u] = 0;
+                    const int t1 = t1b + u * K1_NWARP * SUB;
+                    va[u] = make_double2(0.0, 0.0); sg[u] = 0;
                     if (t1 < m1) {
-                        const int64_t off = (int64_t)t1 * m2h;
-                        va[u] = __ldcs(colA + off);
-                        if (has_b) vb[u] = __ldcs(colB + off);
-                        sg[u] = signs32[((int64_t)t1 * p.m2 + t2_0) >> 5] >> ((int)(t2_0 & 31) + 2 * pr);
+                        va[u] = __ldcs(src + (int64_t)t1 * m2h);
+                        const int64_t tb = (int64_t)t1 * p.m2 + t2_0 + 2 * tcol;       // even: the pair shares a sign word
+                        sg[u] = signs32[tb >> 5] >> (int)(tb & 31);
                     }
                 }
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
-                    const int t1 = t1b + u * RPI * K1_NWARP + half;
-                    if (t1 < m1) {
-                        Cx<T> e0{diag_cast<T, PREC>(va[u].x, sg[u] & 1u), diag_cast<T, PREC>(vb[u].x, sg[u] & 1u)};
-                        Cx<T> e1{diag_cast<T, PREC>(va[u].y, (sg[u] >> 1) & 1u), diag_cast<T, PREC>(vb[u].y, (sg[u] >> 1) & 1u)};
-                        Cx<T>* dst = tile + (size_t)t1 * K1_LD + 2 * pr;
-                        dst[0] = e0; dst[1] = e1;
-                    }
+                    const int t1 = t1b + u * K1_NWARP * SUB;
+                    if (t1 < m1)
+                        tile[(size_t)t1 * K1_LD + tcol] = Cx<T>{diag_cast<T, PREC>(va[u].x, sg[u] & 1u),
+                                                                diag_cast<T, PREC>(va[u].y, (sg[u] >> 1) & 1u)};
                 }
             }
         }
         else {                                                    // unaligned A: 8-byte loads
-            const double* colA = A + (size_t)ja * (size_t)p.lda + t2_0 + tcol;
-            const double* colB = A + (size_t)(has_b ? jb : ja) * (size_t)p.lda + t2_0 + tcol;
+            const double* src = colA + t2_0 + 2 * tcol;
 #pragma unroll 4
             for (int t1 = warp * SUB + sub; t1 < m1; t1 += K1_NWARP * SUB) {
                 const int64_t off = (int64_t)t1 * p.m2;
-                const unsigned neg = (signs32[(off + t2_0) >> 5] >> ((int)(t2_0 & 31) + tcol)) & 1u;
-                const double a = __ldcs(colA + off);
-                const double b = has_b ? __ldcs(colB + off) : 0.0;
-                tile[t1 * K1_LD + tcol] = Cx<T>{diag_cast<T, PREC>(a, neg), diag_cast<T, PREC>(b, neg)};
+                const int64_t tb = off + t2_0 + 2 * tcol;
+                const unsigned sg = signs32[tb >> 5] >> (int)(tb & 31);
+                const double a = __ldcs(src + off), b = __ldcs(src + off + 1);
+                tile[t1 * K1_LD + tcol] = Cx<T>{diag_cast<T, PREC>(a, sg & 1u), diag_cast<T, PREC>(b, (sg >> 1) & 1u)};
             }
         }
         __syncthreads();
-        // ---- stage 1: m1-point DIF FFT down t1 for each of the 32 lanes ---------------------------
+        // ---- stage 1: m1-point DIF FFT down t1 for each of the W complex lanes ---------------------
         int nb = m1;                                   // current block size
         while (nb >= 4) {
             const int q = nb >> 2, tstride = m1 / nb;
@@ -179,9 +176,10 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
             }
             __syncthreads();
         }
-        // ---- stage 2: sampled bins.  Thread (bin i) walks the 32 t2 values of the tile with the twiddle
-        //      recurrence w <- w * W_m^k, re-seeded every 8 steps from w0 * (W_m^{8k})^j (a few ulp in T);
-        //      one sincospi per bin and tile; no shuffles: a bin's partial sum belongs to one thread.
+        // ---- stage 2: sampled bins.  Thread (bin i) walks the W complex columns (2W values of t2) of the tile with the
+        //      twiddle recurrence we <- we * W_m^{2k} for the even t2 (the odd one is we * W_m^k), re-seeded every 8 steps
+        //      from w0 * (W_m^{16k})^j (a few ulp in T); one sincospi per bin and tile; no shuffles: a bin's partial sum
+        //      belongs to one thread.
         for (int i = tid; i < p.s; i += K1_NT) {
             const int64_t k = idx[i];
             const int k1 = (int)(k & (m1 - 1));
@@ -190,36 +188,38 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
             const int brn = p.log_m1 ? (int)(__brev((unsigned)k1n) >> (32 - p.log_m1)) : 0;
             const Cx<T>* rowP = tile + (size_t)br * K1_LD;
             const Cx<T>* rowQ = tile + (size_t)brn * K1_LD;
-            Cx<T> w0, d1, d8;                                  // (cos, sin) of 2 pi k t2_0 / m, 2 pi k / m, 2 pi 8k / m
+            Cx<T> w0, d1, d2, d16;                             // (cos, sin) of 2 pi k t2_0 / m, 2 pi k / m, 2 pi 2k / m, 2 pi 16k / m
             sincospi_t((T)(2.0 * (double)((k * t2_0) & (p.m - 1)) / (double)p.m), &w0.y, &w0.x);
             if (p.dtab) d1 = dstep[i];
             else sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d1.y, &d1.x);
-            d8 = cmul(d1, d1); d8 = cmul(d8, d8); d8 = cmul(d8, d8);           // three squarings: a few ulp in T
-            T va = (T)0, vb = (T)0, ia = (T)0, ib = (T)0;
+            d2 = cmul(d1, d1);
+            d16 = cmul(d2, d2); d16 = cmul(d16, d16); d16 = cmul(d16, d16);    // four squarings of d1: a few ulp in T
+            T va = (T)0, ia = (T)0;
+            constexpr int STEP = K1_W < 8 ? K1_W : 8;
 #pragma unroll 1
-            for (int j8 = 0; j8 < K1_W; j8 += 8) {
-                Cx<T> w = w0;
+            for (int j8 = 0; j8 < K1_W; j8 += STEP) {
+                Cx<T> we = w0;
 #pragma unroll
-                for (int u = 0; u < 8; ++u) {
+                for (int u = 0; u < STEP; ++u) {
                     const Cx<T> P = rowP[j8 + u], Qn = rowQ[j8 + u];
-                    // 2 Z_a = P + conj Qn, 2 Z_b = -i (P - conj Qn);  Re(e^{-i th} Z) = cos*Zr + sin*Zi
-                    va = fma(w.x, P.x + Qn.x, va); va = fma(w.y, P.y - Qn.y, va);
-                    vb = fma(w.x, P.y + Qn.y, vb); vb = fma(w.y, Qn.x - P.x, vb);
+                    const Cx<T> wo = cmul(we, d1);
+                    // 2 E = P + conj Qn (t2 even), 2 O = -i (P - conj Qn) (t2 odd);  Re(e^{-i th} Z) = cos*Zr + sin*Zi
+                    va = fma(we.x, P.x + Qn.x, va); va = fma(we.y, P.y - Qn.y, va);
+                    va = fma(wo.x, P.y + Qn.y, va); va = fma(wo.y, Qn.x - P.x, va);
                     if (REIM) {                                 // Im(e^{-i th} Z) = cos*Zi - sin*Zr
-                        ia = fma(w.x, P.y - Qn.y, ia); ia = fma(-w.y, P.x + Qn.x, ia);
-                        ib = fma(w.x, Qn.x - P.x, ib); ib = fma(-w.y, P.y + Qn.y, ib);
+                        ia = fma(we.x, P.y - Qn.y, ia); ia = fma(-we.y, P.x + Qn.x, ia);
+                        ia = fma(wo.x, Qn.x - P.x, ia); ia = fma(-wo.y, P.y + Qn.y, ia);
                     }
-                    w = cmul(w, d1);
+                    we = cmul(we, d2);
                 }
-                w0 = cmul(w0, d8);
+                w0 = cmul(w0, d16);
             }
             colacc[i] += 0.5 * (double)va;
-            colacc[p.s + i] += 0.5 * (double)vb;
-            if (REIM) { colacc[2 * p.s + i] += 0.5 * (double)ia; colacc[3 * p.s + i] += 0.5 * (double)ib; }
+            if (REIM) colacc[p.s + i] += 0.5 * (double)ia;
         }
     }
     __syncthreads();
-    double* out = partial + ((size_t)pair * p.chunks + chunk) * NACC * p.s;
+    double* out = partial + ((size_t)col * p.chunks + chunk) * NACC * p.s;
     for (int e = tid; e < NACC * p.s; e += K1_NT) out[e] = colacc[e];
 }
 
@@ -228,11 +228,11 @@ template <int PREC>
 __global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial, double* __restrict__ As, Status* st)
 {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    const int rows = p.reim ? 2 * p.s : p.s, nacc = p.reim ? 4 : 2;
+    const int rows = p.reim ? 2 * p.s : p.s, nacc = p.reim ? 2 : 1;
     if (e >= rows * p.n) return;
     const int r = e % rows, j = e / rows;
-    const int i = r % p.s, part = (j & 1) + 2 * (r / p.s);           // Re a, Re b, Im a, Im b
-    const double* src = partial + ((size_t)(j >> 1) * p.chunks) * nacc * p.s + (size_t)part * p.s + i;
+    const int i = r % p.s, part = r / p.s;                               // Re, Im
+    const double* src = partial + ((size_t)j * p.chunks) * nacc * p.s + (size_t)part * p.s + i;
     double acc = 0.0;
     for (int c = 0; c < p.chunks; ++c) acc += src[(size_t)c * nacc * p.s];
     double v = acc * sqrt((double)p.s / (double)p.m);
@@ -242,15 +242,19 @@ __global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial
     As[e] = v;
 }
 
-// tile width: 16 doubles m1 at the same tile size (FP64: 256, FP32 arithmetic: 512), 8 doubles it again (FP64 with
-// s >= 512: C3 3.40 -> 3.30 ms, n = 512 9.8 -> 9.0 ms; 64-byte row segments).  16 is taken for FP64, and for
-// FP16/FP32 sketches with s >= 1024 where stage 2 dominates, when the matrix is long enough for whole sign words
-// per tile row (m2 % 32 == 0)
+// tile width W (complex elements = 2W consecutive t2 of one column): halving W doubles m1 at the same tile size (FP64:
+// 256 at W = 16, FP32 arithmetic: 512), W = 8 doubles it again (FP64 with s >= 512: C3 3.40 -> 3.30 ms, n = 512
+// 9.8 -> 9.0 ms).  16 is taken for FP64, and for FP16/FP32 sketches with s >= 1024 where stage 2 dominates; short
+// columns (m < 64 W) take the widest tile that still leaves m1 >= 2.
 static int k1_tile_w(int64_t m, int prec, int s, int reim)
 {
-    if (reim) return 32;                               // the variant is built for the 32-wide tile only
-    if (prec == 64) return (s >= 512 && m >= 512 * 32) ? 8 : (m >= 256 * 32 ? 16 : 32);
-    return (s >= 1024 && m >= 512 * 32) ? 16 : 32;     // measured: s = 256 slower (0.50 -> 0.58 ms at C2), 512 equal, 1024 6.9 -> 6.0 ms
+    int w = 32;
+    if (!reim) {                                       // the Re+Im variant is built for the 32-wide tile only
+        if (prec == 64) w = (s >= 512 && m >= 512 * 32) ? 8 : (m >= 256 * 32 ? 16 : 32);
+        else w = (s >= 1024 && m >= 512 * 32) ? 16 : 32;   // measured: s = 256 slower (0.50 -> 0.58 ms at C2), 512 equal, 1024 6.9 -> 6.0 ms
+    }
+    while (w > 8 && 4 * (int64_t)w > m) w >>= 1;       // m >= 32: 2W <= m / 2
+    return w;
 }
 
 static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec, int reim)
@@ -259,14 +263,13 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec, int re
     p.m = m; p.lda = lda; p.n = n; p.s = s; p.reim = reim;
     const int K1_W = k1_tile_w(m, prec, s, reim);
     const int m1max = ((prec == 64) ? 128 : 256) * (32 / K1_W);    // 68 KB tile (W = 8: 74 KB)
-    int64_t m1 = m / K1_W;
+    int64_t m1 = m / (2 * K1_W);
     if (m1 > m1max) m1 = m1max;
     if (m1 < 1) m1 = 1;
     p.m1 = (int)m1; p.m2 = m / m1;
     p.log_m1 = 0; while ((1 << p.log_m1) < p.m1) ++p.log_m1;
-    p.tiles_per_col = (int)(p.m2 / K1_W);
-    const int npairs = (n + 1) / 2;
-    int chunks = (12 * num_sms() + npairs - 1) / npairs;
+    p.tiles_per_col = (int)(p.m2 / (2 * K1_W));
+    int chunks = (12 * num_sms() + n - 1) / n;
     if (chunks > p.tiles_per_col) chunks = p.tiles_per_col;
     if (chunks < 1) chunks = 1;
     p.tiles_per_chunk = (p.tiles_per_col + chunks - 1) / chunks;
@@ -279,7 +282,7 @@ size_t k1_workspace_bytes(int64_t m, int n, int s, int prec)
     size_t fft = 0;
     for (int reim = 0; reim < 2; ++reim) {             // either variant may run in this workspace
         K1Params p = k1_params(m, n, m, s, prec, reim);
-        const size_t b = (size_t)((n + 1) / 2) * p.chunks * (reim ? 4 : 2) * (size_t)s * sizeof(double);
+        const size_t b = (size_t)n * p.chunks * (reim ? 2 : 1) * (size_t)s * sizeof(double);
         if (b > fft) fft = b;
     }
     const size_t tc = k1_tc_workspace_bytes();
@@ -291,12 +294,12 @@ static void k1_launch_t(const K1Params& p_in, const double* A, const uint64_t* s
                         double* partial, double* As, Status* st, cudaStream_t stream)
 {
     K1Params p = p_in;
-    size_t smem = (size_t)p.m1 * (W + 1) * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + (REIM ? 4 : 2) * (size_t)p.s * sizeof(double);
+    size_t smem = (size_t)p.m1 * (W + 1) * sizeof(Cx<T>) + (size_t)p.m1 * sizeof(Cx<T>) + (REIM ? 2 : 1) * (size_t)p.s * sizeof(double);
     p.dtab = smem + (size_t)p.s * sizeof(Cx<T>) <= 200 * 1024;
     if (p.dtab) smem += (size_t)p.s * sizeof(Cx<T>);
     auto k = mrcqr_k1_srtt<T, PREC, W, REIM>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    const int grid = ((p.n + 1) / 2) * p.chunks;
+    const int grid = p.n * p.chunks;
     k<<<grid, K1_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
     mrcqr_k1_finalize<PREC><<<((REIM ? 2 : 1) * p.s * p.n + 255) / 256, 256, 0, stream>>>(p, partial, As, st);
 }
@@ -305,31 +308,22 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
                    Status* st, cudaStream_t stream, int reim)
 {
-    if (reim) {                                        // Re+Im variant: FFT form, 32-wide tiles
-        K1Params p = k1_params(m, n, lda, s, prec, 1);
-        p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
-        double* partial = reinterpret_cast<double*>(k1_work);
-        if (prec == 16) k1_launch_t<float, 16, 32, true>(p, A, signs, idx, partial, As, st, stream);
-        else if (prec == 32) k1_launch_t<float, 32, 32, true>(p, A, signs, idx, partial, As, st, stream);
-        else k1_launch_t<double, 64, 32, true>(p, A, signs, idx, partial, As, st, stream);
-        return 2;
-    }
-    if (k1_tc_usable(m, n, lda, A, prec, s)) {
+    double* partial = reinterpret_cast<double*>(k1_work);
+    if (!reim && k1_tc_usable(m, n, lda, A, prec, s)) {
         const int k = launch_k1_tc(m, n, lda, A, s, signs, idx, k1_work, As, st, stream);
         if (k > 0) return k;                          // < 0: the tensor map could not be encoded -> FFT form
     }
-    K1Params p = k1_params(m, n, lda, s, prec, 0);
+    K1Params p = k1_params(m, n, lda, s, prec, reim);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
-    double* partial = reinterpret_cast<double*>(k1_work);
-    const int tw_ = k1_tile_w(m, prec, s, 0);
-    const bool w16 = tw_ == 16;
-    if (prec == 16) { if (w16) k1_launch_t<float, 16, 16>(p, A, signs, idx, partial, As, st, stream);
-                      else k1_launch_t<float, 16, 32>(p, A, signs, idx, partial, As, st, stream); }
-    else if (prec == 32) { if (w16) k1_launch_t<float, 32, 16>(p, A, signs, idx, partial, As, st, stream);
-                           else k1_launch_t<float, 32, 32>(p, A, signs, idx, partial, As, st, stream); }
-    else { if (tw_ == 8) k1_launch_t<double, 64, 8>(p, A, signs, idx, partial, As, st, stream);
-           else if (w16) k1_launch_t<double, 64, 16>(p, A, signs, idx, partial, As, st, stream);
-           else k1_launch_t<double, 64, 32>(p, A, signs, idx, partial, As, st, stream); }
+    const int w = k1_tile_w(m, prec, s, reim);
+#define K1_GO(T_, P_, W_) { if (reim) k1_launch_t<T_, P_, W_, true>(p, A, signs, idx, partial, As, st, stream); \
+                            else k1_launch_t<T_, P_, W_, false>(p, A, signs, idx, partial, As, st, stream); }
+#define K1_W_SWITCH(T_, P_) { if (w == 8) K1_GO(T_, P_, 8) else if (w == 16) K1_GO(T_, P_, 16) else K1_GO(T_, P_, 32) }
+    if (prec == 16) K1_W_SWITCH(float, 16)
+    else if (prec == 32) K1_W_SWITCH(float, 32)
+    else K1_W_SWITCH(double, 64)
+#undef K1_W_SWITCH
+#undef K1_GO
     return 2;
 }
 

@@ -432,7 +432,6 @@ int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double*
 {
     size_t need = ((size_t)9 * n16 + 2 + (size_t)n16 * (n16 + 1)) * sizeof(double);
     const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
-    const size_t smem = use_smem ? need : (size_t)9 * n16 * sizeof(double);
     if (use_smem) {
         const size_t sm2 = ((size_t)2 * n16 + 2 + (size_t)n16 * (n16 + 1)) * sizeof(double);
 #define K4_GO(JM_) { cudaFuncSetAttribute(mrcqr_k4_cholesky_sm<JM_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2); \
@@ -442,10 +441,6 @@ int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double*
         return 1;
     }
     return launch_k4_coop(const_cast<double*>(G16), n, n16, G_out, Rc, RcPrep, Rs, R, st, s);
-    const int threads = n16 <= 64 ? 256 : (n16 <= 128 ? 512 : SMALL_NT);
-    cudaFuncSetAttribute(mrcqr_k4_cholesky, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    mrcqr_k4_cholesky<<<1, threads, smem, s>>>(const_cast<double*>(G16), n, n16, use_smem, G_out, Rc, RcPrep, Rs, R, st);
-    return 1;
 }
 
 int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* Rs, double* RsPrep, int n16,

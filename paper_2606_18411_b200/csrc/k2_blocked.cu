@@ -175,13 +175,6 @@ mrcqr_k2_blocked(double* __restrict__ As, int s, int n, double* __restrict__ bet
                     for (int i = 0; i < j; ++i) S[j][i] = tot[i];
                 }
         }
-        if (blockIdx.x == 0) {                       // R entries of the panel (rows <= pivot) back to the sketch
-#pragma unroll
-            for (int q = 0; q < RPT; ++q)
-#pragma unroll
-                for (int c = 0; c < KB_B; ++c)
-                    if (c < bw && rel[q] >= -j0 && rel[q] <= c) As[(size_t)(j0 + c) * s + tid + KB_NT * q] = P[c][q];
-        }
         // ---- apply H_{bw-1} ... H_0 to the trailing columns this CTA owns
         int c0 = j0 + bw;
         c0 += ((int)blockIdx.x - c0 % G + G) % G;
@@ -210,8 +203,18 @@ mrcqr_k2_blocked(double* __restrict__ As, int s, int n, double* __restrict__ bet
 #undef KB_RECUR
         __threadfence();
         grid.sync();
+        // only now may the R entries of the panel (rows <= pivot) replace the unfactored panel in the sketch: every CTA
+        // loaded it at the top of this iteration, and nothing orders those loads before this point except the barrier
+        if (blockIdx.x == 0) {
+#pragma unroll
+            for (int q = 0; q < RPT; ++q)
+#pragma unroll
+                for (int c = 0; c < KB_B; ++c)
+                    if (c < bw && rel[q] >= -j0 && rel[q] <= c) As[(size_t)(j0 + c) * s + tid + KB_NT * q] = P[c][q];
+        }
     }
     if (blockIdx.x == 0) {
+        __syncthreads();                             // the last panel's write-back above, by other threads of this CTA
         for (int e = tid; e < n * n; e += KB_NT) {
             const int i = e % n, j = e / n;
             double v = 0.0;

@@ -176,7 +176,7 @@ mrcqr_k3_gram(int64_t m, int n, int n16, int64_t lda, const double* __restrict__
                         const int I = 2 * pp[u] + (b >> 1), J = 2 * qq[u] + (b & 1);
                         double* dst = part + (size_t)(8 * J + 2 * t) * n16 + 8 * I + g;
                         if (first_tile) { dst[0] = acc[u][b][0]; dst[n16] = acc[u][b][1]; }
-                        else { atomicAdd(dst, acc[u][b][0]); atomicAdd(dst + n16, acc[u][b][1]); }    // RED: see gram_flush
+                        else { atomicAdd(dst, acc[u][b][0]); atomicAdd(dst + n16, acc[u][b][1]); }    // RED.ADD.F64 by the element's ONE owner thread, in program order: deterministic (gram_roles.cuh, gram_flush)
                     }
                 }
             }
@@ -215,7 +215,7 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
         if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); __syncwarp(); }
         if (mode & 2) solve_slab<RG, 1, NBT>(slab, fragC, nB, lane);        // q = y Rc^-1
         __syncwarp();
-        store_slab<SR, VEC>(slab, Q, ldq, m, n, row0, lane);
+        if (Q) store_slab<SR, VEC>(slab, Q, ldq, m, n, row0, lane);          // Q = nullptr: the debug dump wants only Y
     }
 }
 
@@ -365,8 +365,10 @@ int num_sms()
 size_t k3_partials_bytes(int n)
 {
     RowCfg c = row_config(n);
-    // at most 4 (8 for n16 <= 32) resident CTAs per SM are ever launched
-    return (size_t)num_sms() * (c.n16 <= 32 ? 8 : 4) * (size_t)c.n16 * c.n16 * sizeof(double);
+    // one partial per CTA: at most 8 (n16 <= 32) / 4 (n16 <= 128) resident CTAs per SM are launched (grid_for's cap);
+    // the n16 > 128 kernel holds a whole SM's shared memory: 1 CTA per SM
+    const int per_sm = c.n16 <= 32 ? 8 : (c.n16 <= 128 ? 4 : 1);
+    return (size_t)num_sms() * per_sm * (size_t)c.n16 * c.n16 * sizeof(double);
 }
 
 int upload_diag(const double* prep, int n16, int fac, cudaStream_t s)
@@ -401,7 +403,7 @@ int launch_k3_gram(int64_t m, int n, int64_t lda, const double* A, const double*
     const double2* frag = reinterpret_cast<const double2*>(RsPrep);
 #define K3_GO(RG_, NW_, NB_, V_)                                                                    \
     { auto k = mrcqr_k3_gram<RG_, NW_, NB_, V_>;                                                    \
-      int grid = grid_for(k, NW_ * 32, c.smem_bytes, ntiles, c.n16 <= 32 ? 8 : 4); *n_partials_out = grid;               \
+      int grid = grid_for(k, NW_ * 32, c.smem_bytes, ntiles, c.n16 <= 32 ? 8 : (c.n16 <= 128 ? 4 : 1)); *n_partials_out = grid; \
       k<<<grid, NW_ * 32, c.smem_bytes, s>>>(m, n, c.n16, lda, A, frag, partials, ntiles, Ydump, Ystore, ldys); }
 #define K3_CALL(RG_, NW_, NB_) { if (vec) K3_GO(RG_, NW_, NB_, true) else K3_GO(RG_, NW_, NB_, false) }
     switch (c.n16) {
@@ -431,7 +433,7 @@ int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double
     const int64_t nslabs = (m + SR - 1) / SR;
     int64_t grid = (nslabs + nw - 1) / nw;
     if (grid > num_sms()) grid = num_sms();
-    const bool vec = vec_ok(A, lda) && vec_ok(Q, ldq);
+    const bool vec = vec_ok(A, lda) && (!Q || vec_ok(Q, ldq));
     const double2* fS = reinterpret_cast<const double2*>(RsPrep);
     const double2* fC = reinterpret_cast<const double2*>(RcPrep);
 #define K5_GO(RG_, NB_, V_)                                                                         \

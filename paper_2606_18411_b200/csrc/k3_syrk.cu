@@ -11,7 +11,10 @@
 // triple-buffered shared-memory tile (cp.async, one barrier per chunk) and accumulates on DMMA: 8 warps as 4 x 2, each
 // 32 x 64 of the block (4 x 8 accumulators, 12 fragment loads per 32 DMMA).  Accumulator chains are
 // flushed to the CTA's partial every 1024 rows (reading R7); a reduction kernel adds the
-// partials of a block in a fixed order.  No atomics: bit-reproducible.
+// partials of a block in a fixed order.  Bit-reproducible: every element of a CTA's partial has ONE owner
+// thread for the whole kernel; its later flushes are result-less atomic adds (RED.ADD.F64: same rounding as DADD,
+// applied in program order for one thread and one address, see gram_flush in gram_roles.cuh), so the order of the
+// additions is fixed although the instruction is an atomic.
 #include "mrcqr_internal.cuh"
 #include "gram_roles.cuh"
 
@@ -177,7 +180,7 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
             for (int b = 0; b < 8; ++b) {
                 double* dst = part + (size_t)(64 * wj + 8 * b + 2 * t) * SY_B + 32 * wi + 8 * a + g;
                 if (first) { dst[0] = acc[a][b][0]; dst[SY_B] = acc[a][b][1]; }
-                else { atomicAdd(dst, acc[a][b][0]); atomicAdd(dst + SY_B, acc[a][b][1]); }   // RED: see gram_flush
+                else { atomicAdd(dst, acc[a][b][0]); atomicAdd(dst + SY_B, acc[a][b][1]); }   // single-owner RED.ADD.F64: order fixed (header comment)
                 acc[a][b][0] = acc[a][b][1] = 0.0;
             }
         first = false;

@@ -79,12 +79,42 @@ def test_config3_invariants_and_sampled_rows(orc):
     assert sv[0] / sv[-1] < 50
 
 
-@pytest.mark.parametrize("n,prec", [(16, 16), (32, 32), (64, 64), (128, 16), (256, 32), (512, 64),
-                                    (64, 16), (256, 64), (512, 16)])
-def test_column_sweep_invariants(n, prec):
+@pytest.mark.parametrize("n", [16, 32, 64, 128, 256, 512])
+@pytest.mark.parametrize("prec", [16, 32, 64])
+def test_column_sweep_invariants(orc, n, prec):
+    """Every (n, precision) point of BASELINE.json configs[4] (m = 2^21, s = 2n, kappa ~ 1e4): the invariants, and the
+    sketch of four columns against the oracle's transform of those columns at full length."""
     cfg = inputs.sweep_config(n, prec)
     AT = inputs.make_config(cfg, "cuda")
-    QT, R = B.mrcqr_factor(AT, prec, cfg["s"], cfg["seed_draw"])
+    m, s = cfg["m"], cfg["s"]
+    QT, R = B.mrcqr_factor(AT, prec, s, cfg["seed_draw"])
     check_invariants(AT, QT, R)
+    del QT
+    signs, idx = orc.draw(m, s, cfg["seed_draw"])
+    dsigns, didx = draw_to_dev(signs, idx)
+    _, As = B.mrcqr_sketch(AT, prec, dsigns, didx, want_As=True)
+    cols = [0, 1, n // 2, n - 1]
+    As_o = orc.sketch(np.asfortranarray(to_np(AT[cols])), signs, idx)
+    assert np.linalg.norm(to_np(As)[:, cols] - As_o) / np.linalg.norm(As_o) <= SKETCH_TOL[prec]
+    del AT
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("n", [16, 32, 64, 128])
+def test_column_sweep_elementwise(orc, n):
+    """The FP16-sketch sweep points the oracle finishes in seconds to a minute (n <= 128 at m = 2^21, kappa ~ 1e4, where
+    10 kappa n u is a meaningful bound): every element of Q and R against the oracle's factorization."""
+    cfg = inputs.sweep_config(n, 16)
+    AT = inputs.make_config(cfg, "cuda")
+    A = to_np(AT)
+    o = orc.factor(A, cfg["s"], cfg["seed_draw"])
+    assert o["rc"] == 0
+    QT, R = B.mrcqr_factor(AT, 16, cfg["s"], cfg["seed_draw"])
+    check_invariants(AT, QT, R)
+    Q = to_np(QT)
+    kappa = np.linalg.cond(o["R"])
+    assert np.linalg.norm(Q - o["Q"]) <= 10 * kappa * n * U
+    assert np.linalg.norm(to_np(R) - o["R"]) <= 10 * kappa * n * U * np.linalg.norm(o["R"])
     del AT, QT
     torch.cuda.empty_cache()

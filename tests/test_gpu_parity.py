@@ -197,13 +197,19 @@ def test_power_of_two_scaling_is_exact(orc):
 def test_breakdown_and_errors_are_reported(orc):
     m, n = 4096, 8
     rng = np.random.default_rng(0)
-    # rank deficient by an exact zero column.  It is the unpaired last column (n odd) so that no
-    # rounding noise of a neighbouring column leaks into it through the two-columns-per-complex-FFT
-    # packing: its sketch is exactly zero and R_s[6,6] = 0.
+    # rank deficient by an exact zero column: the transform is column-wise, so the sketch of a zero
+    # column is exactly zero whatever its neighbours hold, and R_s[5,5] = 0 (PAPER.md:31 assumes rank n).  All three
+    # sketch precisions, an interior column of an even n (the round-1 kernel packed column pairs and failed this)
+    A8 = np.asfortranarray(rng.standard_normal((m, n)))
+    A8[:, 5] = 0.0
+    for prec in (64, 32, 16):
+        rc = B.mrcqr_factor(colmajor_to_dev(A8), prec, 16, 1, check=False)
+        assert rc == 2 and B.mrcqr_last_info() == 5
+    # ... and the last column of an odd n
     A7 = np.asfortranarray(rng.standard_normal((m, 7)))
     A7[:, 6] = 0.0
     rc = B.mrcqr_factor(colmajor_to_dev(A7), 64, 14, 1, check=False)
-    assert rc == 2 and B.mrcqr_last_info() == 6               # PAPER.md:31 assumes rank n
+    assert rc == 2 and B.mrcqr_last_info() == 6
     A = np.zeros((m, n), order="F")
     A[:, :] = rng.standard_normal((m, n))
     A[:, 5] = 2.0 * A[:, 2]                                   # numerically dependent column
@@ -245,3 +251,100 @@ def test_fp16_degrades_beyond_its_range_never_silently(orc):
         assert orc.orth_error_fro(to_np(QT16)) > 1e-13          # degraded, detectably
     else:
         assert rc in (2, 3)
+
+
+@pytest.mark.parametrize("prec,m,n,s", [(64, 1 << 13, 6, 24), (32, 1 << 14, 7, 40), (64, 1 << 15, 4, 520), (32, 1 << 15, 5, 1030),
+                                        (32, 64, 4, 16), (64, 32, 3, 9), (16, 1 << 14, 6, 200)])
+def test_sketch_is_column_wise(orc, prec, m, n, s):
+    """the transform runs down each column on its own.  Scaling column j of A by 2^-30 scales column j of
+    the sketch by 2^-30 BIT FOR BIT and leaves every other column untouched, for even and odd j, in every tile width
+    of the FFT form of K1 (the FP16 sketch would underflow: checked with 2^-3)."""
+    AT = inputs.make_A(m, n, 2, 700 + n, 701 + n, "cuda")
+    signs, idx = orc.draw(m, s, 31 + n)
+    dsigns, didx = draw_to_dev(signs, idx)
+    _, As0 = B.mrcqr_sketch(AT, prec, dsigns, didx, want_As=True) if s >= n else (None, None)
+    f = 2.0 ** (-3 if prec == 16 else -30)
+    for j in (0, 1, n - 1, n - 2):
+        AT2 = AT.clone()
+        AT2[j] *= f
+        _, As1 = B.mrcqr_sketch(AT2, prec, dsigns, didx, want_As=True)
+        want = As0.clone()
+        want[j] *= f
+        if prec == 16:                                   # FP16 rounding of the scaled input is not an exact scaling near the subnormals
+            assert torch.equal(As1[torch.arange(n) != j], want[torch.arange(n) != j])
+            assert relf(to_np(As1[j]), to_np(want[j])) <= 2e-3
+        else:
+            assert torch.equal(As1, want)
+    # the sketch of one column alone equals that column of the whole sketch
+    _, As_one = B.mrcqr_sketch(AT[1:2].contiguous(), prec, dsigns, didx, want_As=True) if s >= 1 else (None, None)
+    assert torch.equal(As_one[0], As0[1])
+
+
+@pytest.mark.parametrize("m,s,seed", [(32, 4, 5), (64, 33, 6), (1 << 15, 100, 7), (1 << 20, 128, 12), (1 << 21, 512, 32)])
+def test_device_draw_is_bit_exact(orc, m, s, seed):
+    """a0 (north_star: bit-exact for integer work): the sign words mrcqr_factor draws with its DEVICE
+    kernel and the bins it copies are the oracle's, word for word (m = 2^15: 512 words, two CTAs of the draw kernel)."""
+    osigns, oidx = orc.draw(m, s, seed)
+    dsigns, didx = B.mrcqr_draw_device(m, s, seed)
+    assert np.array_equal(dsigns.cpu().numpy().view(np.uint64), osigns)
+    assert np.array_equal(didx.cpu().numpy(), oidx)
+
+
+@pytest.mark.parametrize("m,n,s,prec", [(32, 4, 8, 64), (1 << 15, 24, 48, 32), (1 << 15, 64, 128, 16), (1 << 14, 100, 200, 64)])
+def test_factor_equals_its_stages_on_the_oracle_draw(orc, m, n, s, prec):
+    """mrcqr_factor(seed) is bit for bit the composition sketch(oracle.draw) -> precondition_gram -> form_q: every
+    kernel is deterministic, so equality holds iff the device-drawn sign words and bins equal the oracle's."""
+    AT = inputs.make_A(m, n, 3, 800 + n, 801 + n, "cuda")
+    QT, R = B.mrcqr_factor(AT, prec, s, 77)
+    signs, idx = orc.draw(m, s, 77)
+    dsigns, didx = draw_to_dev(signs, idx)
+    Rs, _ = B.mrcqr_sketch(AT, prec, dsigns, didx)
+    Rc, _ = B.mrcqr_precondition_gram(AT, Rs)
+    Q2, R2 = B.mrcqr_form_q(AT, Rs, Rc)
+    assert torch.equal(QT, Q2) and torch.equal(R, R2)
+
+
+def test_default_s_is_3n(orc):
+    """c = 3n by default.  s <= 0 in mrcqr_factor is exactly s = 3n."""
+    m, n = 1 << 13, 20
+    AT = inputs.make_A(m, n, 4, 5, 6, "cuda")
+    Q0, R0 = B.mrcqr_factor(AT, 32, 0, 9)
+    Q1, R1 = B.mrcqr_factor(AT, 32, 3 * n, 9)
+    assert torch.equal(Q0, Q1) and torch.equal(R0, R1)
+    Q2, R2 = B.mrcqr_factor(AT, 32, 2 * n, 9)
+    assert not torch.equal(R0, R2)                        # a different sketch: same QR only to rounding
+    factor_parity(orc, AT, 3 * n, 9, 32)
+    Qa, Ra, used, orth = B.mrcqr_factor_auto(AT, 32, -1, 9)
+    assert torch.equal(Qa, Q1) and used == 32
+
+
+@pytest.mark.parametrize("name,m,n,s,prec,expo,pad", [("C0", 4096, 16, 32, 32, 6, 0), ("wide", 1 << 12, 136, 272, 64, 5, 0),
+                                                      ("lda", 1 << 12, 24, 48, 64, 3, 10)])
+def test_factor_host_matches_oracle(orc, name, m, n, s, prec, expo, pad):
+    """mrcqr_factor_host (the path bench.py times as e2e) against the oracle, element by element; with lda > m the
+    padding rows of A_host are not read (NaN there) and those of Q_host are not written (sentinels survive)."""
+    if name == "C0":
+        cfg = inputs.CONFIGS["C0"]
+        AT = inputs.make_config(cfg, "cpu")
+        seed = cfg["seed_draw"]
+    else:
+        AT = inputs.make_A(m, n, expo, 900 + n, 901 + n, "cpu")
+        seed = 5
+    lda = m + pad
+    A_host = torch.full((n, lda), float("nan"), dtype=torch.float64).pin_memory()
+    A_host[:, :m] = AT
+    Q_host = torch.full((n, lda), -7.0, dtype=torch.float64).pin_memory()
+    R_host = torch.empty((n, n), dtype=torch.float64).pin_memory()
+    B.mrcqr_factor_host(A_host[:, :m], prec, s, seed, Q_host[:, :m], R_host)
+    A = to_np(AT)
+    Q, Rn = Q_host[:, :m].numpy().T, R_host.numpy().T
+    assert np.all(Q_host[:, m:].numpy() == -7.0)
+    o = orc.factor(A, s, seed)
+    assert o["rc"] == 0
+    assert orc.orth_error_fro(Q) <= 1e-13 and orc.residual_fro(A, Q, Rn) <= 1e-13
+    kappa = np.linalg.cond(o["R"])
+    assert np.linalg.norm(Q - o["Q"]) <= 10 * kappa * n * U
+    assert np.linalg.norm(Rn - o["R"]) <= 10 * kappa * n * U * np.linalg.norm(o["R"])
+    # same bits as the device-buffer call
+    QT, R = B.mrcqr_factor(AT.cuda(), prec, s, seed)
+    assert torch.equal(QT.cpu(), Q_host[:, :m]) and torch.equal(R.cpu(), R_host)

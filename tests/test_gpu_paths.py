@@ -101,7 +101,8 @@ def test_store_y_path_is_deterministic_and_handles_strides(orc):
     big = torch.zeros((n, m + 6), dtype=torch.float64, device="cuda")
     big[:, :m] = AT
     Q3, R3 = B.mrcqr_factor(big[:, :m], B.FP64, 2 * n, 3)
-    assert torch.equal(Q3[:, :m] if Q3.shape[1] != m else Q3, Q1) and torch.equal(R3, R1)
+    assert Q3.shape == (n, m) and Q3.stride(0) == m + 6                # Q takes A's leading dimension
+    assert torch.equal(Q3, Q1) and torch.equal(R3, R1)
     # columns that start on an odd element (8-byte aligned only): the fall-back kernels run; same Q to rounding
     odd = torch.zeros((n, m + 7), dtype=torch.float64, device="cuda")
     odd[:, 1:m + 1] = AT
@@ -259,25 +260,38 @@ def test_cholqr_cholqr2_and_the_kappa_probe(orc):
     assert B.mrcqr_orth_error(Q3) <= 1e-13 and orc.residual_fro(to_np(AT3), to_np(Q3), to_np(R3)) <= 1e-13
 
 
-@pytest.mark.parametrize("m,n,prec", [(4096, 16, 32), (1 << 14, 64, 16), (1 << 12, 200, 64)])
+@pytest.mark.parametrize("m,n,prec", [(4096, 16, 32), (1 << 14, 64, 16), (1 << 12, 200, 64), (1 << 12, 131, 64)])
 def test_graph_replay_gives_the_same_bits(orc, m, n, prec):
     """mrcqr_set_graph(1): the captured pipeline replays with new seeds (seed and bins are graph data) and returns
-    exactly what the ordinary path returns, positive codes included."""
+    exactly what the ordinary path returns, positive codes included.  Capture is illegal on the legacy default stream,
+    so the replays run on a stream of their own and mrcqr_last_used_graph() must say that a graph ran (n = 16: the
+    register QR, n = 64: the tensor-core sketch with its TMA descriptor, n > 128: the cooperative K2 / K4 launches
+    and the panel passes)."""
     AT = inputs.make_A(m, n, 3, 300 + n, 301 + n, "cuda")
     QT = torch.empty_like(AT); R = torch.empty((n, n), dtype=torch.float64, device="cuda")
     ref = {}
     for seed in (1, 2, 3):
         B.mrcqr_factor(AT, prec, 2 * n, seed, QT, R)
         ref[seed] = (QT.clone(), R.clone())
+    assert not B.mrcqr_last_used_graph()
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
     B.mrcqr_set_graph(True)
     try:
-        for seed in (1, 2, 3, 1):
-            B.mrcqr_factor(AT, prec, 2 * n, seed, QT, R)
-            assert torch.equal(QT, ref[seed][0]) and torch.equal(R, ref[seed][1])
-        assert B.mrcqr_last_launch_count() > 0
-        bad = AT.clone(); bad[n - 1, :] = 0.0                    # exact zero last column -> code 2 from the replayed graph too
-        rc = B.mrcqr_factor(bad, 64, 2 * n, 1, check=False) if n % 2 == 1 else 0
-        assert rc in (0, 2)
+        # the legacy default stream cannot be captured: the ordinary path runs, same bits
+        B.mrcqr_factor(AT, prec, 2 * n, 2, QT, R, stream=torch.cuda.default_stream())
+        assert not B.mrcqr_last_used_graph() and torch.equal(QT, ref[2][0])
+        with torch.cuda.stream(side):
+            for seed in (1, 2, 3, 1):
+                B.mrcqr_factor(AT, prec, 2 * n, seed, QT, R, stream=side)
+                assert B.mrcqr_last_used_graph()
+                assert torch.equal(QT, ref[seed][0]) and torch.equal(R, ref[seed][1])
+            assert B.mrcqr_last_launch_count() > 0
+            bad = AT.clone(); bad[n - 1, :] = 0.0                # exact zero last column -> code 2 from a replayed graph too
+            Qb = torch.empty_like(bad)
+            for _ in range(2):
+                rc = B.mrcqr_factor(bad, prec, 2 * n, 1, Qb, R, stream=side, check=False)
+                assert rc == 2 and B.mrcqr_last_info() == n - 1 and B.mrcqr_last_used_graph()
     finally:
         B.mrcqr_set_graph(False)
 
