@@ -1,19 +1,22 @@
-#!/usr/bin/env python
 """bench.py -- MRCQR FP64 thin-QR benchmark (BASELINE.json metric: ms per factorization at m x n,
 achieved HBM GB/s and FP64 TFLOP/s against the B200's measured peaks).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C1|C0|C2|C3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C3|C0|C1|C2|C4n<n>]
 
-A "step" is one pass of the whole hot path (mrcqr_factor: draw, K1..K5) over the synthetic
-matrix of BASELINE.json configs[1] (C1: m = 2^20, n = 64, FP16 sketch, s = 128), already resident
-in HBM.  `e2e` is the same factorization through mrcqr_factor_host with pinned HOST buffers
-(H2D of A, D2H of Q and R inside the timed region).  The path does not shard (SURVEY.md 8(e):
-"replicas only"): with N > 1 every rank factors its own replica; the value stays ms per
+A "step" is one pass of the whole hot path (mrcqr_factor: draw, K1..K5) over one synthetic matrix already
+resident in HBM.  The headline workload is BASELINE.json configs[3] (C3: m = 2^21, n = 256, FP64 sketch, s = 512):
+north_star quotes its target at m = 2^21, n <= 256, and C3 is the largest fixed configuration.  The same JSON line
+carries, under "points", C1, C2 and the six FP16-sketch points of the column sweep configs[4] (per point: ms,
+per-stage ms, both floors, both fractions, the clocks seen).  `e2e` is the headline factorization through
+mrcqr_factor_host with pinned HOST buffers (H2D of A, D2H of Q and R inside the timed region).  The path does not
+shard ("replicas only"): with N > 1 every rank factors its own replica; the value stays ms per
 factorization of the slowest rank and `factorizations_per_s` aggregates the ranks.
 --impl reference times the CPU oracle (oracle/) on the host cores, rank 0 only.
 Prints ONE JSON line on rank 0.
 """
 import argparse
+import glob
+import hashlib
 import json
 import os
 import subprocess
@@ -25,11 +28,61 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "MRCQR FP64 thin-QR ms per factorization"
-FP64_DMMA_PEAK_TFLOPS = 37.2      # measured on this pool's B200 (profiles/r01_peaks.md), DMMA.8x8x4 issue peak
-# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the ncu --set full capture of
-# config C1 summarised in profiles/r01_ncu_full_final.md; only valid for that workload
-NCU_TRAFFIC_C1 = {"k5_form_q": 537.0e6 + 480.4e6, "k3_gram": 556.2e6 + 23.2e6}    # profiles/r01_ncu_full_final.md
+# FP64 peak: nominal 148 SMs x 64 FMA/clk x 2 x 1.965 GHz = 37.2 TFLOP/s, confirmed by a DMMA.8x8x4 issue probe on this
+# pool (profiles/r01_peaks.md); MEASURED_PEAKS.json has no FP64 figure, and the guide's bf16-scaled rule
+# (1608.8 x 40 / 2250 = 28.6) would flatter every fraction by 1.3x
+FP64_DMMA_PEAK_TFLOPS = 37.2
 HBM_FALLBACK_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")
+POINTS = ["C1", "C2", "C4n16", "C4n32", "C4n64", "C4n128", "C4n256", "C4n512"]
+
+
+def source_sha16():
+    """Identity of the kernels being timed: sha256 over csrc/*.cu, *.cuh (the GPU box has no .git)."""
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2606_18411_b200", "csrc", "*.cu*"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(config, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the ncu --set full capture recorded in
+    profiles/r02_traffic.json (written by --traffic-from), or None when the capture is of other sources / configs."""
+    try:
+        d = json.load(open(TRAFFIC_FILE))
+        if d.get("src_sha16") != source_sha16():
+            return None
+        return d["configs"][config][kernel]["dram_bytes_per_launch"]
+    except Exception:
+        return None
+
+
+def write_traffic(csv_path, config):
+    """--traffic-from: reads `ncu -i <rep> --page raw --csv` output and records, per kernel name, the mean
+    dram__bytes_read.sum + dram__bytes_write.sum per launch, keyed by config and the sha of the kernel sources."""
+    import csv
+    rows = list(csv.reader(open(csv_path)))
+    hdr = rows[0]
+    units = rows[1]
+    kn, rd, wr = hdr.index("Kernel Name"), hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    acc = {}
+    for r in rows[2:]:
+        if len(r) <= max(kn, rd, wr):
+            continue
+        name = r[kn].split("(")[0].replace("void ", "").replace("mrcqr::", "").strip()
+        b = float(r[rd].replace(",", "")) * scale[units[rd]] + float(r[wr].replace(",", "")) * scale[units[wr]]
+        acc.setdefault(name, []).append(b)
+    try:
+        d = json.load(open(TRAFFIC_FILE))
+    except Exception:
+        d = {}
+    if d.get("src_sha16") != source_sha16():
+        d = {"src_sha16": source_sha16(), "configs": {}}
+    d["configs"][config] = {k: {"dram_bytes_per_launch": sum(v) / len(v), "launches": len(v)} for k, v in acc.items()}
+    json.dump(d, open(TRAFFIC_FILE, "w"), indent=1, sort_keys=True)
+    print("wrote", TRAFFIC_FILE, "for", config, "sources", d["src_sha16"])
 
 
 def measured_peaks():
@@ -217,6 +270,100 @@ def max_over_ranks(value, device="cpu"):
     return float(t.item())
 
 
+def floors(m, n, hbm_peak):
+    """Algorithmic work of one factorization (SURVEY.md 8(d)): 32 m n bytes (3 reads of A + 1 write of Q) for every n;
+    4 m n^2 flops in the recompute form (n <= 128), 3 m n^2 in the store-Y form (n > 128: its extra write + read of Y is
+    traffic, not algorithm).  Returns (bytes, flops, hbm floor ms, fp64 floor ms)."""
+    alg_bytes = 32.0 * m * n
+    flops = (3.0 if n > 128 else 4.0) * m * n * n
+    return alg_bytes, flops, alg_bytes / (hbm_peak * 1e9) * 1e3, flops / (FP64_DMMA_PEAK_TFLOPS * 1e12) * 1e3
+
+
+def time_point(B, AT, QT, R, cfg, steps, warmup, stream, sampler=None, barrier=None):
+    """warmup + steps factorizations timed with CUDA events on `stream`; then the same loop again with the library's
+    per-kernel events (kept out of the first loop: the extra event records cost a few % of a 1 ms step).
+    Returns (total ms of the K steps, launches, {stage: ms per step})."""
+    import torch
+    prec, s, seed = cfg["prec"], cfg["s"], cfg["seed_draw"]
+    for _ in range(warmup):
+        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
+    launches = 0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if barrier:
+        barrier()
+    else:
+        torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    e0.record(stream)
+    for _ in range(steps):
+        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
+        launches += B.mrcqr_last_launch_count()
+    e1.record(stream)
+    if barrier:
+        barrier()
+    else:
+        torch.cuda.synchronize()
+    total_ms = e0.elapsed_time(e1)
+    B.mrcqr_set_timing(True)
+    stage_sum = {k: 0.0 for k in B.STAGES}
+    for _ in range(steps):
+        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
+        for k, v in B.mrcqr_last_timing().items():
+            stage_sum[k] += v
+    B.mrcqr_set_timing(False)
+    return total_ms, launches, {k: v / steps for k, v in stage_sum.items()}
+
+
+def dominant_kernel(cfg, stages, hbm_peak, how):
+    """The kernel with the largest share of the step and its roofline (DESIGN.md section 5 states the per-row figures).
+    n <= 128: K3 (8n bytes, 2n^2 flops per row) or K5 (16n bytes, 2n^2 flops per row), one launch = all m rows.
+    n > 128: one triangular solve = ceil(n/64) panel-pass launches (n^2 flops, 16n bytes per row over those launches) or
+    the SYRK launch (n^2 flops, 8n bytes per row); `kernel_ms` is the duration of those launches together."""
+    m, n = cfg["m"], cfg["n"]
+    if n <= 128:
+        cand = {"k3_gram": ("mrcqr_k3_gram", 8.0 * m * n, 2.0 * m * n * n),
+                "k5_form_q": ("mrcqr_k5_formq", 16.0 * m * n, 2.0 * m * n * n)}
+    else:
+        cand = {"k3_gram": ("mrcqr_panel_pass<0> (solve with R_s, %d launches)" % ((n + 63) // 64), 16.0 * m * n, 1.0 * m * n * n),
+                "gram_reduce": ("mrcqr_syrk", 8.0 * m * n, 1.0 * m * n * n),
+                "k5_form_q": ("mrcqr_panel_pass<1> (solve with R_c, %d launches)" % ((n + 63) // 64), 16.0 * m * n, 1.0 * m * n * n)}
+    stage = max(cand, key=lambda k: stages[k])
+    kname, dom_bytes, dom_flops = cand[stage]
+    dom_ms = stages[stage]
+    t_hbm, t_f64 = dom_bytes / (hbm_peak * 1e9), dom_flops / (FP64_DMMA_PEAK_TFLOPS * 1e12)
+    if t_f64 >= t_hbm:
+        ach = dom_flops / (dom_ms * 1e-3) / 1e12
+        roof = {"bound": "tensor", "achieved": ach, "peak": FP64_DMMA_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": ach / FP64_DMMA_PEAK_TFLOPS,
+                "peak_source": "FP64 DMMA (mma.sync m8n8k4 f64) peak: nominal 148 x 64 x 2 x 1.965 GHz, confirmed by probe "
+                               "(profiles/r01_peaks.md); MEASURED_PEAKS.json has no FP64 figure"}
+    else:
+        ach = dom_bytes / (dom_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % how}
+    tkey = {"mrcqr_k3_gram": "mrcqr_k3_gram", "mrcqr_k5_formq": "mrcqr_k5_formq", "mrcqr_syrk": "mrcqr_syrk"}.get(kname, "mrcqr_panel_pass")
+    traffic = ncu_traffic(cfg["name"], tkey)
+    if traffic is not None and tkey == "mrcqr_panel_pass":
+        traffic *= (n + 63) // 64                       # the capture holds the mean per launch; the solve is that many launches
+    roof.update({"traffic": traffic, "kernel": kname, "stage": stage, "kernel_ms": dom_ms, "algorithmic_bytes": dom_bytes,
+                 "algorithmic_flops": dom_flops, "hbm_gbs_achieved": dom_bytes / (dom_ms * 1e-3) / 1e9,
+                 "traffic_source": "profiles/r02_traffic.json (ncu --set full of these kernel sources)" if traffic is not None
+                 else "no ncu capture of these kernel sources / this config on file"})
+    return roof
+
+
+def point_json(cfg, ms, stages, hbm_peak, clocks=None):
+    alg_bytes, flops, t_hbm, t_f64 = floors(cfg["m"], cfg["n"], hbm_peak)
+    out = {"config": "%s: m=%d n=%d s=%d fp%d" % (cfg["name"], cfg["m"], cfg["n"], cfg["s"], cfg["prec"]),
+           "ms": ms, "stage_ms": stages, "hbm_floor_ms": t_hbm, "fp64_floor_ms": t_f64,
+           "hbm_frac": t_hbm / ms, "fp64_frac": t_f64 / ms, "binding_frac": max(t_hbm, t_f64) / ms,
+           "hbm_gbs": alg_bytes / (ms * 1e-3) / 1e9, "fp64_tflops": flops / (ms * 1e-3) / 1e12}
+    if clocks is not None:
+        out["clocks"] = clocks
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -244,50 +391,30 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
     sampler = ClockSampler(local)
-    launches = 0
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    sampler.start()
-    e0.record(stream)
-    for _ in range(args.steps):
-        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
-        launches += B.mrcqr_last_launch_count()
-    e1.record(stream)
-    barrier()
-    total_ms = e0.elapsed_time(e1)
-    # per-kernel times: a second loop of the same K steps with the library's CUDA events between its kernels
-    # (kept out of the loop above: the 8 extra event records per step cost ~4 % of a 1 ms step)
-    B.mrcqr_set_timing(True)
-    stage_sum = {k: 0.0 for k in B.STAGES}
-    for _ in range(args.steps):
-        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
-        for k, v in B.mrcqr_last_timing().items():
-            stage_sum[k] += v
-    B.mrcqr_set_timing(False)
+    total_ms, launches, stages = time_point(B, AT, QT, R, cfg, args.steps, args.warmup, stream, sampler, barrier)
     clocks = sampler.stop()
     total_ms = max_over_ranks(total_ms, "cuda")
     ms = total_ms / args.steps
-    stages = {k: v / args.steps for k, v in stage_sum.items()}
 
-    # ---- variant: store-Y form of stage 2, same metric, reported beside the default ----
-    B.mrcqr_set_timing(False)
-    B.mrcqr_set_store_y(True)
-    for _ in range(3):
-        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
-    v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    v0.record(stream)
-    for _ in range(args.steps):
-        B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
-    v1.record(stream)
-    torch.cuda.synchronize()
-    store_y_ms = v0.elapsed_time(v1) / args.steps
-    B.mrcqr_set_store_y(False)
+    # ---- variant: store-Y form of stage 2 for n <= 128 (n > 128 always stores Y) ----
+    variants = None
+    if n <= 128:
+        B.mrcqr_set_store_y(True)
+        for _ in range(3):
+            B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
+        v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        v0.record(stream)
+        for _ in range(args.steps):
+            B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
+        v1.record(stream)
+        torch.cuda.synchronize()
+        B.mrcqr_set_store_y(False)
+        variants = {"store_y_ms": v0.elapsed_time(v1) / args.steps,
+                    "note": "mrcqr_set_store_y(1): Y = A Rs^-1 written to Q's buffer by stage 2a, solved in place by stage 2b "
+                            "(5 passes, 3 m n^2 flops) instead of kept on chip and recomputed (4 passes, 4 m n^2)"}
 
     # ---- end to end: HOST buffers through mrcqr_factor_host (H2D + D2H inside the timed region) ----
-    B.mrcqr_set_timing(False)
     A_host = torch.empty((n, m), dtype=torch.float64, pin_memory=True)
     A_host.copy_(AT)
     Q_host = torch.empty((n, m), dtype=torch.float64, pin_memory=True)
@@ -301,58 +428,52 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
     e2e_ms = max_over_ranks(e2e_ms, "cuda")
+    del A_host, Q_host
+
+    hbm_peak, how = measured_peaks()
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        _, cpu = time_oracle(cfg, AT.cpu().numpy().T, 1, 0)
+
+    # ---- the other configurations of BASELINE.json, same protocol, carried in the same line ----
+    points = []
+    if rank == 0 and world == 1 and not args.no_points:
+        del AT, QT
+        torch.cuda.empty_cache()
+        for name in POINTS:
+            if name == cfg["name"]:
+                continue
+            pc = workload(name)
+            PA = inputs.make_config(pc, "cuda")
+            PQ = torch.empty_like(PA)
+            PR = torch.empty((pc["n"], pc["n"]), dtype=torch.float64, device="cuda")
+            psamp = ClockSampler(local)
+            psteps = max(1, min(args.steps, 10))
+            ptot, _, pstages = time_point(B, PA, PQ, PR, pc, psteps, 3, stream, psamp)
+            points.append(point_json(pc, ptot / psteps, pstages, hbm_peak, psamp.stop()))
+            del PA, PQ
+            torch.cuda.empty_cache()
 
     if rank == 0:
-        hbm_peak, how = measured_peaks()
-        panels = n > 128                               # store-Y panel passes + SYRK (n16 > 128)
-        if not panels:
-            alg_bytes = 32.0 * m * n                   # 3 reads of A + 1 write of Q (north_star)
-            flops = 4.0 * m * n * n                    # 2 solves in K5, 1 solve + Gram in K3
-            # dominant kernel = the slower of K3 / K5; its algorithmic work
-            dom = "k5_form_q" if stages["k5_form_q"] >= stages["k3_gram"] else "k3_gram"
-            dom_flops = 2.0 * m * n * n
-            dom_bytes = (16.0 if dom == "k5_form_q" else 8.0) * m * n
-        else:
-            alg_bytes = 40.0 * m * n                   # A read twice (K1, solve 1), Y written, read by SYRK, solved in place (r+w)
-            flops = 3.0 * m * n * n                    # two triangular solves + the symmetric Gram, m n^2 each
-            dom = "k5_form_q" if stages["k5_form_q"] >= stages["k3_gram"] else "k3_gram"   # one panel solve each here
-            dom_flops = 1.0 * m * n * n
-            dom_bytes = 16.0 * m * n
-        dom_ms = stages[dom]
-        t_hbm, t_f64 = dom_bytes / (hbm_peak * 1e9), dom_flops / (FP64_DMMA_PEAK_TFLOPS * 1e12)
-        if t_f64 >= t_hbm:
-            ach = dom_flops / (dom_ms * 1e-3) / 1e12
-            roof = {"bound": "tensor", "achieved": ach, "peak": FP64_DMMA_PEAK_TFLOPS, "unit": "TFLOP/s",
-                    "frac": ach / FP64_DMMA_PEAK_TFLOPS, "traffic": None,
-                    "peak_source": "FP64 DMMA peak measured on this pool (profiles/r01_peaks.md); "
-                                   "MEASURED_PEAKS.json has no FP64 figure"}
-        else:
-            ach = dom_bytes / (dom_ms * 1e-3) / 1e9
-            roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
-                    "traffic": None, "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % how}
-        if cfg["name"] == "C1":
-            roof["traffic"] = NCU_TRAFFIC_C1.get(dom)
-        roof.update({"kernel": dom, "kernel_ms": dom_ms, "algorithmic_bytes": dom_bytes, "algorithmic_flops": dom_flops,
-                     "hbm_gbs_achieved": dom_bytes / (dom_ms * 1e-3) / 1e9})
-        cpu = None
-        if world == 1 and not args.no_cpu_baseline:
-            _, cpu = time_oracle(cfg, AT.cpu().numpy().T, 1, 0)
+        alg_bytes, flops, t_hbm, t_f64 = floors(m, n, hbm_peak)
+        roof = dominant_kernel(cfg, stages, hbm_peak, how)
         line = {"metric": METRIC, "value": ms, "unit": "ms", "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_json(cfg),
                 "factorizations_per_s": world * 1e3 / ms,
-                "pipeline": {"hbm_gbs": alg_bytes / (ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_peak,
+                "pipeline": {"algorithmic_bytes": alg_bytes, "algorithmic_flops": flops,
+                             "hbm_gbs": alg_bytes / (ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_peak,
                              "hbm_frac": alg_bytes / (ms * 1e-3) / 1e9 / hbm_peak,
                              "fp64_tflops": flops / (ms * 1e-3) / 1e12, "fp64_peak_tflops": FP64_DMMA_PEAK_TFLOPS,
                              "fp64_frac": flops / (ms * 1e-3) / 1e12 / FP64_DMMA_PEAK_TFLOPS,
-                             "stage_ms": stages},
-                "variants": {"store_y_ms": store_y_ms,
-                             "note": "mrcqr_set_store_y(1): Y = A Rs^-1 written to Q's buffer by stage 2a, solved in place by "
-                                     "stage 2b (5 passes, 3 m n^2 flops) instead of kept on chip and recomputed (4 passes, 4 m n^2)"},
-                "roofline": roof, "cpu_baseline": cpu,
+                             "hbm_floor_ms": t_hbm, "fp64_floor_ms": t_f64, "binding_frac": max(t_hbm, t_f64) / ms,
+                             "stage_ms": stages,
+                             "extra_traffic": "store-Y form (n > 128): +16 m n bytes (Y written by solve 1, read by the SYRK) "
+                                              "beyond the 32 m n algorithmic bytes" if n > 128 else None},
+                "variants": variants, "roofline": roof, "cpu_baseline": cpu,
                 "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": 8 * m * n,
                         "d2h_bytes_per_step": 8 * m * n + 8 * n * n, "steps": e2e_steps},
-                "gpu_launches": launches, "clocks": clocks}
+                "gpu_launches": launches, "clocks": clocks, "points": points, "src_sha16": source_sha16()}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -396,7 +517,7 @@ def run_sweep(args):
         tot = e0.elapsed_time(e1) / args.steps
         flop = (3.0 if n > 128 else 4.0) * m * n * n
         print("| %s | %d | %d | fp%d | %.3f | %.3f | %.3f | %.3f | %.3f | %.3f | %.3f | %.3f | %.1e | %.1e |" % (
-            name, m, n, cfg["prec"], tot, acc["k1_srtt"], acc["k2_sketch_qr"], acc["k3_gram"], acc["reduce_k4_chol"],
+            name, m, n, cfg["prec"], tot, acc["k1_srtt"], acc["k2_sketch_qr"], acc["k3_gram"], acc["gram_reduce"] + acc["k4_chol"],
             acc["k5_form_q"], 32.0 * m * n / (hbm_peak * 1e9) * 1e3, flop / (FP64_DMMA_PEAK_TFLOPS * 1e12) * 1e3,
             gpu_orth_error_fro(QT), gpu_residual_fro(AT, QT, R)), flush=True)
         del AT, QT
@@ -437,11 +558,15 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3", "C4n16", "C4n32", "C4n64", "C4n128", "C4n256", "C4n512"])
+    ap.add_argument("--config", default="C3", choices=["C0", "C1", "C2", "C3", "C4n16", "C4n32", "C4n64", "C4n128", "C4n256", "C4n512"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-points", action="store_true", help="skip the other configurations carried under \"points\"")
+    ap.add_argument("--traffic-from", default=None, help="ncu --page raw --csv file: record per-kernel DRAM bytes of --config in profiles/r02_traffic.json")
     ap.add_argument("--stability", action="store_true", help="orthogonality / residual vs kappa on the paper's eq.(3) matrices")
     ap.add_argument("--sweep", action="store_true", help="per-stage table over BASELINE.json configs 0-4 instead of the JSON line")
     args = ap.parse_args()
+    if args.traffic_from:
+        return write_traffic(args.traffic_from, args.config)
     if args.stability:
         return run_stability(args)
     if args.sweep:

@@ -132,8 +132,10 @@ int mrcqr_last_launch_count(void);
  * Per-kernel device timing of mrcqr_factor (CUDA events recorded on the call's stream between the
  * kernels; off by default).  mrcqr_last_timing fills 7 floats, milliseconds of the last
  * mrcqr_factor / mrcqr_factor_host call:  [0] K1 sampled transform (Alg.2 steps 2-4),  [1] K2 sketch QR
- * (steps 5-6),  [2] R_s preparation,  [3] K3 precondition + Gram (step 7, Alg.1 step 1),  [4] partial
- * reduction + K4 Cholesky (Alg.1 step 2),  [5] K5 form Q (Alg.1 step 3),  [6] R = Rc Rs (step 9).
+ * (steps 5-6),  [2] upload of the prepared R_s,  [3] K3 precondition + Gram (step 7, Alg.1 step 1; n > 128: the
+ * first triangular solve, Y = A R_s^-1 into Q's buffer),  [4] reduction of the Gram partials (n > 128: the SYRK
+ * G = Y^T Y and its reduction),  [5] K4 Cholesky + R = Rc Rs (Alg.1 step 2, Alg.2 step 9),  [6] K5 form Q
+ * (Alg.1 step 3; n > 128: the second triangular solve, in place).
  */
 int mrcqr_set_timing(int on);
 int mrcqr_last_timing(float* ms_out_host);

@@ -70,7 +70,7 @@ EXPORTS = ["mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_sk
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
            "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"]
 
-STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "reduce_k4_chol", "k5_form_q", "r_mul"]
+STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "gram_reduce", "k4_chol", "k5_form_q"]
 
 
 def _stream(stream):

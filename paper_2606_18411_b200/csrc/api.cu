@@ -397,14 +397,15 @@ static int enqueue_stage23(const Layout& L, int64_t m, int n, int64_t lda, const
             if (tm) cudaEventRecord(g.ev[4], st);
             k += launch_reduce_partials(part, np, n, n16, G16, st);
         }
+        if (tm) cudaEventRecord(g.ev[5], st);
         k += launch_k4_cholesky(G16, n, n16, nullptr, Rc, RcPrep, Rs, R, stat, st);     // + step 9: R = Rc Rs
         k += upload_diag(RcPrep, n16, 1, st);
-        if (tm) cudaEventRecord(g.ev[5], st);
+        if (tm) cudaEventRecord(g.ev[6], st);
         if (panels) k += launch_panel_solve(m, n, 1, Q, ldq, RcPrep, Q, ldq, st);                // q = y Rc^-1 in place
         else if (store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);
         else if (g.store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);  // variant: stored Y
         else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 3, st);        // Alg.1 step 3
-        if (tm) { cudaEventRecord(g.ev[6], st); cudaEventRecord(g.ev[7], st); }
+        if (tm) cudaEventRecord(g.ev[7], st);
     }
     return k;
 }
