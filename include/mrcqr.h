@@ -112,6 +112,23 @@ int mrcqr_factor(int64_t m, int n, int64_t lda, const double* A, double* Q, doub
                  mrcqr_prec_t sketch_prec, int s, uint64_t seed, void* stream);
 
 /*
+ * Algorithm 2 for a BATCH of independent problems of one shape: the repeated-call regime the paper motivates (block
+ * Arnoldi, randomized-SVD power iterations, time stepping), where one small factorization is a chain of
+ * dependent kernels whose latency no loop or graph can hide.  Problem b (0 <= b < batch) is
+ *     A_b = A + b * strideA  (m x n, column-major, leading dimension lda),   Q_b = Q + b * strideQ (same lda),
+ *     R_b = R + b * n * n,   drawn with seed + b: its result is that of mrcqr_factor(..., seed + b, ...).
+ * Shapes with n <= 32, s <= 128, m <= 2^16 run as ONE kernel, one CTA per problem, out of shared memory and L2 (the sketch
+ * is the defining cosine sum evaluated directly in the arithmetic of p; everything else as in mrcqr_factor); other shapes
+ * are factored one after the other by the ordinary path.  Strides count doubles; strideA, strideQ >= (n-1) lda + m.
+ * codes_host (nullable, HOST, batch ints): the code of every problem (0, 1, 2, 3).  Returns 0 if every problem succeeded,
+ * else the code of the first failing problem (its index detail via mrcqr_last_info()); a negative argument index:
+ * -1 batch, -2 m, -3 n, -4 lda, -5 strideA, -6 A, -7 strideQ, -8 Q, -9 R, -10 prec, -11 s; or 4.
+ */
+int mrcqr_factor_batched(int batch, int64_t m, int n, int64_t lda, int64_t strideA, const double* A,
+                         int64_t strideQ, double* Q, double* R, mrcqr_prec_t sketch_prec, int s,
+                         uint64_t seed, int* codes_host, void* stream);
+
+/*
  * mrcqr_factor with HOST buffers: copies the m x n part of A (lda >= m; the padding rows m..lda-1 of a column are
  * neither read nor written) to library-owned device buffers on a stream of the library's own, factors, copies Q
  * (same lda) and R back; synchronous.  This is the end-to-end path bench.py times as `e2e`.

@@ -44,6 +44,7 @@ def lib():
         L.mrcqr_precondition_gram.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
         L.mrcqr_form_q.argtypes = [i64, ci, i64, vp, vp, vp, i64, vp, vp, vp]
         L.mrcqr_factor.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64, vp]
+        L.mrcqr_factor_batched.argtypes = [ci, i64, ci, i64, i64, vp, i64, vp, vp, ci, ci, u64, vp, vp]
         L.mrcqr_factor_host.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64]
         L.mrcqr_workspace_bytes.restype = C.c_size_t
         L.mrcqr_workspace_bytes.argtypes = [i64, ci, ci, ci]
@@ -58,7 +59,7 @@ def lib():
         L.mrcqr_set_sketch_reim.argtypes = [ci]
         L.mrcqr_set_graph.argtypes = [ci]
         L.mrcqr_last_timing.argtypes = [vp]
-        for f in ("mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
+        for f in ("mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
                   "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
                   "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"):
             getattr(L, f).restype = ci
@@ -66,7 +67,7 @@ def lib():
     return _lib
 
 
-EXPORTS = ["mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
+EXPORTS = ["mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
            "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"]
 
@@ -164,6 +165,25 @@ def mrcqr_factor(AT, prec, s, seed, QT=None, R=None, stream=None, check=True):
         return rc
     _chk(rc)
     return QT, R
+
+
+def mrcqr_factor_batched(AB, prec, s, seed, QB=None, RB=None, stream=None, check=True):
+    """Batch of problems: AB is a (batch, n, m) float64 CUDA tensor (problem b = AB[b], column-major m x n).  Problem b is
+    drawn with seed + b.  Returns (QB (batch, n, m), RB (batch, n, n), codes list) -- raises on the first failing problem
+    unless check=False."""
+    assert AB.is_cuda and AB.dtype == torch.float64 and AB.dim() == 3 and AB.stride(2) == 1
+    batch, n, m = AB.shape
+    if QB is None:
+        QB = torch.empty_strided((batch, n, m), AB.stride(), dtype=torch.float64, device=AB.device)
+    if RB is None:
+        RB = torch.empty((batch, n, n), dtype=torch.float64, device=AB.device)
+    assert QB.shape == AB.shape and QB.stride(2) == 1 and QB.stride(1) == AB.stride(1) and RB.is_contiguous()
+    codes = (C.c_int * batch)()
+    rc = lib().mrcqr_factor_batched(batch, m, n, AB.stride(1), AB.stride(0), AB.data_ptr(), QB.stride(0), QB.data_ptr(),
+                                    RB.data_ptr(), prec, s, seed, codes, _stream(stream))
+    if check:
+        _chk(rc)
+    return QB, RB, list(codes)
 
 
 def mrcqr_factor_host(AT_host, prec, s, seed, QT_host=None, R_host=None):

@@ -8,15 +8,6 @@
 
 namespace mrcqr {
 
-// ---- splitmix64, counter form: X(k) = mix(seed + (k+1) * gamma) ----------------------------------
-__host__ __device__ __forceinline__ uint64_t splitmix64_at(uint64_t seed, uint64_t k)
-{
-    uint64_t z = seed + (k + 1ull) * 0x9E3779B97F4A7C15ull;
-    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
-    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
-    return z ^ (z >> 31);
-}
-
 // device side of the draw: sign words, plus reset of the status block (first kernel of a call)
 __global__ void mrcqr_draw_signs(uint64_t seed, int64_t nwords, uint64_t* __restrict__ signs, Status* st)
 {
@@ -87,6 +78,7 @@ struct Ctx {
     int last_info = 0, last_launches = 0;
     bool last_graph = false;                 // the last mrcqr_factor call replayed a CUDA graph
     cudaStream_t host_stream = nullptr;      // mrcqr_factor_host: a non-blocking stream of the library's own
+    int* bcodes = nullptr; int* h_bcodes = nullptr; size_t bcodes_cap = 0;   // mrcqr_factor_batched: (code, info) per problem, device + pinned
     bool timing = false; cudaEvent_t ev[8] = {}; bool ev_ok = false; float stage_ms[8] = {};
     bool have_device = false, probed = false;
     bool store_y = false;                    // mrcqr_set_store_y: store-Y variant also for n16 <= 128
@@ -264,6 +256,8 @@ extern "C" void mrcqr_shutdown(void)
     if (g.hQ) cudaFree(g.hQ);
     if (g.hR) cudaFree(g.hR);
     if (g.host_stream) cudaStreamDestroy(g.host_stream);
+    if (g.bcodes) cudaFree(g.bcodes);
+    if (g.h_bcodes) cudaFreeHost(g.h_bcodes);
     g = Ctx();
 }
 
@@ -624,6 +618,60 @@ extern "C" int mrcqr_kappa_probe(int64_t m, int n, int64_t lda, const double* A,
     *kappa_lb_host = lb;
     if (prec_host) *prec_host = lb < 1e4 ? 16 : (lb < 1e8 ? 32 : 64);
     return 0;
+}
+
+// Algorithm 2 for `batch` independent problems of one shape (the repeated-call regime).
+extern "C" int mrcqr_factor_batched(int batch, int64_t m, int n, int64_t lda, int64_t strideA, const double* A,
+                                    int64_t strideQ, double* Q, double* R, mrcqr_prec_t sketch_prec, int s,
+                                    uint64_t seed, int* codes_host, void* stream)
+{
+    if (batch < 1) return -1;
+    if (!is_pow2(m) || m < n || m < 32) return -2;
+    if (n < 1 || n > N_MAX) return -3;
+    if (lda < m) return -4;
+    if (batch > 1 && strideA < (int64_t)(n - 1) * lda + m) return -5;
+    if (!A) return -6;
+    if (batch > 1 && strideQ < (int64_t)(n - 1) * lda + m) return -7;
+    if (!Q) return -8;
+    if (!R) return -9;
+    if (!prec_ok((int)sketch_prec)) return -10;
+    if (s <= 0) s = 3 * n;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX || (g.reim && 2 * s > S_MAX)) return -11;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    int first = 0;
+    if (!g.reim && batched_fused_usable(m, n, s)) {
+        if ((size_t)batch > g.bcodes_cap) {
+            if (g.bcodes) cudaFree(g.bcodes);
+            if (g.h_bcodes) cudaFreeHost(g.h_bcodes);
+            g.bcodes = g.h_bcodes = nullptr; g.bcodes_cap = 0;
+            if (cudaMalloc(&g.bcodes, sizeof(int) * 2 * (size_t)batch) != cudaSuccess ||
+                cudaMallocHost(&g.h_bcodes, sizeof(int) * 2 * (size_t)batch) != cudaSuccess) { cudaGetLastError(); return MRCQR_ERR_CUDA; }
+            g.bcodes_cap = (size_t)batch;
+        }
+        const int k = launch_factor_batched(batch, m, n, lda, strideA, A, lda, strideQ, Q, R, (int)sketch_prec, s, seed, g.bcodes, st);
+        g.last_launches = k; g.last_graph = false;
+        cudaMemcpyAsync(g.h_bcodes, g.bcodes, sizeof(int) * 2 * (size_t)batch, cudaMemcpyDeviceToHost, st);
+        if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) return MRCQR_ERR_CUDA;
+        for (int b = 0; b < batch; ++b) {
+            if (codes_host) codes_host[b] = g.h_bcodes[2 * b];
+            if (!first && g.h_bcodes[2 * b]) { first = g.h_bcodes[2 * b]; g.last_info = g.h_bcodes[2 * b + 1]; }
+        }
+        return first;
+    }
+    // shapes beyond one CTA's reach: the problems are large enough for the ordinary path, one after the other
+    int launches = 0, info = 0;
+    for (int b = 0; b < batch; ++b) {
+        const int rc = factor_device(m, n, lda, A + (size_t)b * (size_t)strideA, lda, Q + (size_t)b * (size_t)strideQ,
+                                     R + (size_t)b * (size_t)n * n, (int)sketch_prec, s, seed + (uint64_t)b, st);
+        if (rc < 0 || rc == MRCQR_ERR_CUDA) return rc;
+        launches += g.last_launches;
+        if (codes_host) codes_host[b] = rc;
+        if (!first && rc) { first = rc; info = g.last_info; }
+    }
+    g.last_launches = launches;
+    if (first) g.last_info = info;
+    return first;
 }
 
 extern "C" int mrcqr_factor_host(int64_t m, int n, int64_t lda, const double* A_host, double* Q_host,

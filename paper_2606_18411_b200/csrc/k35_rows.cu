@@ -315,7 +315,7 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
             }
         }
         if (active) {
-            panel_core<RG, FAC, PB>(acc, SlabXpose<RG>(slab - (size_t)(8 * P0) * LDS_, lane), frag, P0, lane, NoSink());
+            panel_core<RG, PB>(acc, SlabXpose<RG>(slab - (size_t)(8 * P0) * LDS_, lane), ConstFactor<FAC>{frag}, P0, lane, NoSink());
             __syncwarp();
             store_slab<SR, true>(slab, dst, ldd, m, ncols, row0, lane);
         }

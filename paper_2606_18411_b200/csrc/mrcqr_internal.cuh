@@ -16,6 +16,15 @@ __device__ __forceinline__ void report(Status* st, int code, int info)
 
 inline int round_up(int x, int q) { return (x + q - 1) / q * q; }
 
+// splitmix64, counter form: X(k) = mix(seed + (k+1) * gamma), the stream of the draw (reading R1)
+__host__ __device__ __forceinline__ uint64_t splitmix64_at(uint64_t seed, uint64_t k)
+{
+    uint64_t z = seed + (k + 1ull) * 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
 // ---- slab geometry of the row-streaming kernels (K3 / K5), chosen from n only -----------------
 // n16 = n padded to a multiple of 16 (8-wide DMMA blocks in pairs).  A warp owns a slab of 8*RG rows,
 // a CTA NW slabs; slab = n16 x (8*RG + 4) doubles of shared memory.
@@ -115,6 +124,12 @@ bool k1_tc_usable(int64_t m, int n, int64_t lda, const double* A, int prec, int 
 size_t k1_tc_workspace_bytes();
 int launch_k1_tc(int64_t m, int n, int64_t lda, const double* A, int s, const uint64_t* signs,
                  const int64_t* idx, void* work, double* As, Status* st, cudaStream_t stream);
+
+// batched small problems, one CTA per problem (k_batched.cu); codes_dev: batch x 2 ints (code, info)
+bool batched_fused_usable(int64_t m, int n, int s);
+int launch_factor_batched(int batch, int64_t m, int n, int64_t lda, int64_t strideA, const double* A, int64_t ldq,
+                          int64_t strideQ, double* Q, double* R, int prec, int s, uint64_t seed, int* codes_dev,
+                          cudaStream_t st);
 
 size_t k3_partials_bytes(int n);
 int num_sms();

@@ -26,7 +26,9 @@ namespace mrcqr {
 // Diagonal 8x8 blocks of the two prepared factors (FAC 0: R_s, FAC 1: R_c), 36 doubles per block:
 // [0..8) 1/R[j,j], then -R[j,jj] for j < jj, j-major.  Constant memory: the thread-per-row
 // substitution reads them with warp-uniform addresses, off the shared-memory pipe.
+#ifndef MRCQR_NO_CONST_DIAG
 __constant__ double c_diag[2][PREP_MAX_NB * PREP_DIAG];
+#endif
 
 __host__ __device__ constexpr int diag_off(int j, int jj) { return 8 + j * 7 - j * (j - 1) / 2 + (jj - j - 1); }
 
@@ -133,6 +135,25 @@ __device__ __forceinline__ const double2* fragpair(const double2* __restrict__ f
     return frag + ((size_t)(Jg * (Jg - 1) / 2 + Kg) * 32 + lane);
 }
 
+// ---- where the prepared factor of a solve lives ---------------------------------------------------------
+// ConstFactor: off-diagonal fragment pairs in global memory (read-only path, L1 / L2 resident), the diagonal blocks of
+// factor FAC in constant memory.  SmemFactor: the whole prepared factor (layout of mrcqr_internal.cuh) in shared memory
+// (the batched one-CTA-per-problem kernel, where every problem has factors of its own).  Same arithmetic either way.
+#ifndef MRCQR_NO_CONST_DIAG
+template <int FAC>
+struct ConstFactor {
+    const double2* __restrict__ frag;
+    __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const { return __ldg(fragpair(frag, Kg, Jg, lane)); }
+    __device__ __forceinline__ const double* diag(int Kg) const { return &c_diag[FAC][Kg * PREP_DIAG]; }
+};
+#endif
+struct SmemFactor {
+    const double* prep; int nB;
+    __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const
+    { return *reinterpret_cast<const double2*>(prep + 2 * ((size_t)(Jg * (Jg - 1) / 2 + Kg) * 32 + lane)); }
+    __device__ __forceinline__ const double* diag(int Kg) const { return prep + prep_diag_offset(nB) + Kg * PREP_DIAG; }
+};
+
 // ---- where a block goes between its DMMA (accumulator) form and its one-thread-per-row form -------
 // SlabXpose: through the block's own columns of the slab (leading dimension SR + 4); the solved block
 // stays there (in-place solve).
@@ -156,8 +177,8 @@ struct NoSink { __device__ __forceinline__ void operator()(int, const double (&)
 // with) the dependent fma chain of that step's substitution; only J = K+1 is updated at once.
 // sink(Kg, y) sees every solved block in row form (lane = row of the slab).
 // This is the ONLY place the solve's arithmetic lives: K3 and K5 both run it.
-template <int RG, int FAC, int PB, typename X, typename SINK>
-__device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp, const double2* __restrict__ frag,
+template <int RG, int PB, typename X, typename F, typename SINK>
+__device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp, const F& fac,
                                            int P0, int lane, const SINK& sink)
 {
     double ap0[RG], ap1[RG];                                  // A fragments of block K-1
@@ -174,7 +195,7 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
         if (K > 0) {
 #pragma unroll
             for (int J = K + 1; J < PB; ++J) {
-                const double2 b = __ldg(fragpair(frag, P0 + K - 1, P0 + J, lane));
+                const double2 b = fac.pair(P0 + K - 1, P0 + J, lane);
 #pragma unroll
                 for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], ap0[rg], b.x);
 #pragma unroll
@@ -182,7 +203,7 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
             }
         }
         if (xp.row_active()) {
-            diag_substitute(y, &c_diag[FAC][(P0 + K) * PREP_DIAG]);
+            diag_substitute(y, fac.diag(P0 + K));
 #pragma unroll
             for (int j = 0; j < 8; ++j) *xp.rowp(P0 + K, j) = y[j];
             sink(P0 + K, y);
@@ -195,7 +216,7 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
             for (int rg = 0; rg < RG; ++rg) { acc[rg][K][0] = ap0[rg]; acc[rg][K][1] = ap1[rg]; }
         }
         if (K + 1 < PB) {
-            const double2 b = __ldg(fragpair(frag, P0 + K, P0 + K + 1, lane));
+            const double2 b = fac.pair(P0 + K, P0 + K + 1, lane);
 #pragma unroll
             for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][K + 1], ap0[rg], b.x);
 #pragma unroll
@@ -206,8 +227,8 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
 }
 
 // One panel of PB column blocks starting at global block P0 of an in-place slab solve.
-template <int RG, int FAC, int PB>
-__device__ __forceinline__ void solve_panel(double* slab, const double2* __restrict__ frag, int P0, int lane)
+template <int RG, int PB, typename F>
+__device__ __forceinline__ void solve_panel(double* slab, const F& fac, int P0, int lane)
 {
     constexpr int SR = 8 * RG, LDS_ = SR + 4;
     const int g = lane >> 2, t = lane & 3;
@@ -230,36 +251,45 @@ __device__ __forceinline__ void solve_panel(double* slab, const double2* __restr
         }
 #pragma unroll
         for (int J = 0; J < PB; ++J) {
-            const double2 b = __ldg(fragpair(frag, Kg, P0 + J, lane));
+            const double2 b = fac.pair(Kg, P0 + J, lane);
 #pragma unroll
             for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a0[rg], b.x);
 #pragma unroll
             for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a1[rg], b.y);
         }
     }
-    panel_core<RG, FAC, PB>(acc, SlabXpose<RG>(slab, lane), frag, P0, lane, NoSink());
+    panel_core<RG, PB>(acc, SlabXpose<RG>(slab, lane), fac, P0, lane, NoSink());
 }
 
-// In-place Y <- Y * R^-1 on this warp's slab (8*RG rows x 8*nB columns).  frag: prepared factor in
-// fragment order; FAC selects its diagonal blocks in constant memory.  NBT > 0: nB known at compile time
-// (only the panel shapes that occur are instantiated); the arithmetic is the same either way.
-template <int RG, int FAC, int NBT = 0>
-__device__ __forceinline__ void solve_slab(double* slab, const double2* __restrict__ frag, int nB, int lane)
+// In-place Y <- Y * R^-1 on this warp's slab (8*RG rows x 8*nB columns) against the prepared factor `fac`.
+// NBT > 0: nB known at compile time (only the panel shapes that occur are instantiated); the arithmetic is the same
+// either way.
+template <int RG, int NBT, typename F>
+__device__ __forceinline__ void solve_slab_f(double* slab, const F& fac, int nB, int lane)
 {
     if (NBT > 0) {
         constexpr int FULL = NBT / 8, REST = NBT % 8;
 #pragma unroll
-        for (int p = 0; p < FULL; ++p) solve_panel<RG, FAC, 8>(slab, frag, 8 * p, lane);
-        if (REST > 0) solve_panel<RG, FAC, (REST > 0 ? REST : 2)>(slab, frag, 8 * FULL, lane);
+        for (int p = 0; p < FULL; ++p) solve_panel<RG, 8>(slab, fac, 8 * p, lane);
+        if (REST > 0) solve_panel<RG, (REST > 0 ? REST : 2)>(slab, fac, 8 * FULL, lane);
         return;
     }
     for (int P0 = 0; P0 < nB; P0 += 8) {
         const int pb = nB - P0;
-        if (pb >= 8)      solve_panel<RG, FAC, 8>(slab, frag, P0, lane);
-        else if (pb == 6) solve_panel<RG, FAC, 6>(slab, frag, P0, lane);
-        else if (pb == 4) solve_panel<RG, FAC, 4>(slab, frag, P0, lane);
-        else              solve_panel<RG, FAC, 2>(slab, frag, P0, lane);
+        if (pb >= 8)      solve_panel<RG, 8>(slab, fac, P0, lane);
+        else if (pb == 6) solve_panel<RG, 6>(slab, fac, P0, lane);
+        else if (pb == 4) solve_panel<RG, 4>(slab, fac, P0, lane);
+        else              solve_panel<RG, 2>(slab, fac, P0, lane);
     }
 }
+
+#ifndef MRCQR_NO_CONST_DIAG
+// The form K3 / K5 use: frag = prepared factor in fragment order (global), FAC selects its diagonal blocks in constant memory.
+template <int RG, int FAC, int NBT = 0>
+__device__ __forceinline__ void solve_slab(double* slab, const double2* __restrict__ frag, int nB, int lane)
+{
+    solve_slab_f<RG, NBT>(slab, ConstFactor<FAC>{frag}, nB, lane);
+}
+#endif
 
 } // namespace mrcqr

@@ -67,6 +67,22 @@ def test_argument_errors_before_any_device_work():
     assert L.mrcqr_sketch(1024, 8, 1024, p, 32, 16, None, p, None, p, None) == -7
 
 
+def test_batched_argument_errors():
+    L = B.lib()
+    p = C.c_void_p(16)            # never dereferenced
+    assert L.mrcqr_factor_batched(0, 1024, 8, 1024, 8192, p, 8192, p, p, 32, 16, 0, None, None) == -1
+    assert L.mrcqr_factor_batched(2, 1000, 8, 1000, 8000, p, 8000, p, p, 32, 16, 0, None, None) == -2
+    assert L.mrcqr_factor_batched(2, 1024, 0, 1024, 8192, p, 8192, p, p, 32, 16, 0, None, None) == -3
+    assert L.mrcqr_factor_batched(2, 1024, 8, 1000, 8192, p, 8192, p, p, 32, 16, 0, None, None) == -4
+    assert L.mrcqr_factor_batched(2, 1024, 8, 1024, 100, p, 8192, p, p, 32, 16, 0, None, None) == -5
+    assert L.mrcqr_factor_batched(2, 1024, 8, 1024, 8192, None, 8192, p, p, 32, 16, 0, None, None) == -6
+    assert L.mrcqr_factor_batched(2, 1024, 8, 1024, 8192, p, 100, p, p, 32, 16, 0, None, None) == -7
+    assert L.mrcqr_factor_batched(2, 1024, 8, 1024, 8192, p, 8192, None, p, 32, 16, 0, None, None) == -8
+    assert L.mrcqr_factor_batched(2, 1024, 8, 1024, 8192, p, 8192, p, None, 32, 16, 0, None, None) == -9
+    assert L.mrcqr_factor_batched(2, 1024, 8, 1024, 8192, p, 8192, p, p, 8, 16, 0, None, None) == -10
+    assert L.mrcqr_factor_batched(2, 1024, 8, 1024, 8192, p, 8192, p, p, 32, 4, 0, None, None) == -11
+
+
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-device behaviour")
 def test_no_cpu_fallback_without_device():
     L = B.lib()

@@ -340,3 +340,80 @@ def test_reim_sketch_variant(orc, m, n, s, prec, tol):
     # and the switch is off again: the default sketch has s rows
     _, As1 = B.mrcqr_sketch(AT, p, dsigns, didx, want_As=True)
     assert to_np(As1).shape == (s, n)
+
+
+def _guarded(shape_elems, margin=4096, fill=-1234.5):
+    """A float64 CUDA buffer of `shape_elems` elements with `margin` sentinel elements on both sides (16-byte aligned)."""
+    buf = torch.full((shape_elems + 2 * margin,), fill, dtype=torch.float64, device="cuda")
+    return buf, buf[margin:margin + shape_elems]
+
+
+def _margins_intact(buf, inner_elems, margin=4096, fill=-1234.5):
+    return bool((buf[:margin] == fill).all()) and bool((buf[margin + inner_elems:] == fill).all())
+
+
+@pytest.mark.parametrize("m,n,s,prec,pad", [
+    (4096, 16, 32, 32, 0),       # register K2, K3 / K5 at n16 = 16, single-CTA Cholesky
+    (1 << 14, 64, 128, 16, 0),   # tensor-core K1 (TMA), n16 = 64
+    (1 << 13, 50, 150, 64, 6),   # ragged n, lda > m: the padding rows of Q must stay untouched
+    (1 << 13, 100, 200, 32, 0),  # blocked (cooperative) K2, n16 = 112
+    (1 << 12, 136, 272, 64, 2),  # panel passes + SYRK, cooperative K4... n16 = 144, lda > m
+    (1 << 11, 300, 600, 32, 0),  # n16 > 256
+    (64, 8, 16, 64, 0),          # tiny m
+])
+def test_no_writes_outside_the_outputs(orc, m, n, s, prec, pad):
+    """Stand-in for compute-sanitizer memcheck (closed on this pool, profiles/r02_sanitizer.md): every output lives inside a
+    larger buffer of sentinels; after mrcqr_factor and the three stage calls the sentinels (margins, and the padding rows
+    m..lda-1 of every column of Q) are unchanged and A is bit-identical to its copy."""
+    lda = m + pad
+    A0 = inputs.make_A(m, n, 3, 50 + n, 51 + n, "cuda")
+    abuf, aflat = _guarded(n * lda)
+    AT = aflat.view(n, lda)[:, :m]
+    AT.copy_(A0)
+    a_before = abuf.clone()
+    qbuf, qflat = _guarded(n * lda)
+    QT = qflat.view(n, lda)[:, :m]
+    rbuf, rflat = _guarded(n * n)
+    R = rflat.view(n, n)
+    B.mrcqr_factor(AT, prec, s, 5, QT, R)
+    assert _margins_intact(qbuf, n * lda) and _margins_intact(rbuf, n * n)
+    if pad:
+        assert bool((qflat.view(n, lda)[:, m:] == -1234.5).all())
+    assert torch.equal(abuf, a_before)
+    Qn, Rn = to_np(QT.contiguous()), to_np(R)
+    assert orc.orth_error_fro(Qn) <= 1e-13 and orc.residual_fro(to_np(A0), Qn, Rn) <= 1e-13
+    # stage calls: As, Rs, G, Rc, Q, R inside guards
+    signs, idx = orc.draw(m, s, 5)
+    dsigns, didx = draw_to_dev(signs, idx)
+    L = B.lib()
+    asbuf, asflat = _guarded(s * n)
+    rsbuf, rsflat = _guarded(n * n)
+    st = torch.cuda.current_stream().cuda_stream
+    assert L.mrcqr_sketch(m, n, lda, AT.data_ptr(), prec, s, dsigns.data_ptr(), didx.data_ptr(), asflat.data_ptr(), rsflat.data_ptr(), st) == 0
+    assert _margins_intact(asbuf, s * n) and _margins_intact(rsbuf, n * n)
+    gbuf, gflat = _guarded(n * n)
+    rcbuf, rcflat = _guarded(n * n)
+    assert L.mrcqr_precondition_gram(m, n, lda, AT.data_ptr(), rsflat.data_ptr(), gflat.data_ptr(), rcflat.data_ptr(), st) == 0
+    assert _margins_intact(gbuf, n * n) and _margins_intact(rcbuf, n * n)
+    qbuf.fill_(-1234.5); rbuf.fill_(-1234.5)
+    assert L.mrcqr_form_q(m, n, lda, AT.data_ptr(), rsflat.data_ptr(), rcflat.data_ptr(), lda, QT.data_ptr(), R.data_ptr(), st) == 0
+    assert _margins_intact(qbuf, n * lda) and _margins_intact(rbuf, n * n)
+    if pad:
+        assert bool((qflat.view(n, lda)[:, m:] == -1234.5).all())
+    assert torch.equal(abuf, a_before)
+    # the signs / bins the caller passed are not modified either
+    assert np.array_equal(dsigns.cpu().numpy().view(np.uint64), signs) and np.array_equal(didx.cpu().numpy(), idx)
+
+
+def test_batched_writes_stay_inside(orc):
+    batch, m, n, s = 7, 1024, 12, 30
+    abuf, aflat = _guarded(batch * n * m)
+    AB = aflat.view(batch, n, m)
+    for b in range(batch):
+        AB[b] = inputs.make_A(m, n, 2, 60 + b, 61 + b, "cuda")
+    a_before = abuf.clone()
+    qbuf, qflat = _guarded(batch * n * m)
+    rbuf, rflat = _guarded(batch * n * n)
+    QB, RB, codes = B.mrcqr_factor_batched(AB, 64, s, 1, qflat.view(batch, n, m), rflat.view(batch, n, n))
+    assert codes == [0] * batch
+    assert _margins_intact(qbuf, batch * n * m) and _margins_intact(rbuf, batch * n * n) and torch.equal(abuf, a_before)
