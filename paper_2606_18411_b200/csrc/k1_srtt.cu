@@ -223,6 +223,168 @@ mrcqr_k1_srtt(K1Params p, const double* __restrict__ A, const uint32_t* __restri
     for (int e = tid; e < NACC * p.s; e += K1_NT) out[e] = colacc[e];
 }
 
+// =================================================================================================
+// K1, register radix-16 form (m1 = 256 = 16 x 16, W = 16): the form every long column takes (m >= 8192).
+// The shared-memory radix-4 kernel above moves the tile through shared memory ten times per transform (4 passes read +
+// write, staging, stage 2) and was bound by that (round 1: 0.20-0.33 of the HBM peak).  Here a thread owns one 16-point
+// butterfly per pass IN REGISTERS:
+//   pass 1  thread (b, u) loads x~[t1 = 16 a + b], a = 0..15, of tile column u STRAIGHT FROM GLOBAL MEMORY (a half warp
+//           reads 256 contiguous bytes of one row; the 16 loads of the NEXT tile are issued before this tile's butterflies,
+//           so the HBM latency hides under two passes and stage 2), applies sign and cast, transforms over a, multiplies
+//           by W_256^{b ka} and stores Y[ka][b] to the tile;
+//   pass 2  thread (ka, u) transforms the 16 values b = 0..15 in place: Z[k1 = ka + 16 kb] sits in tile row 16 ka + kb;
+//   stage 2 as above (thread = bin).
+// Three barriers and three shared-memory passes per tile.  ST is the tile's storage type: Cx<T>, or __half2 for the FP16
+// sketch, whose transform keeps its intermediates in half like the paper's cufftXt path (FP32
+// butterflies, R5) and moves half the shared-memory bytes of the FP32 sketch.
+template <typename T> struct K16;
+template <> struct K16<float>  { static constexpr float  C = 0.92387953251128674f, S = 0.38268343236508977f, H = 0.70710678118654752f; };
+template <> struct K16<double> { static constexpr double C = 0.92387953251128674,  S = 0.38268343236508977,  H = 0.70710678118654752; };
+
+// 4-point forward DFT in place
+template <typename T> __device__ __forceinline__ void dft4(Cx<T>& a0, Cx<T>& a1, Cx<T>& a2, Cx<T>& a3)
+{
+    const Cx<T> s02 = cadd(a0, a2), d02 = csub(a0, a2), s13 = cadd(a1, a3), d13 = cmulmi(csub(a1, a3));
+    a0 = cadd(s02, s13); a2 = csub(s02, s13); a1 = cadd(d02, d13); a3 = csub(d02, d13);
+}
+// 16-point forward DFT in registers: input x[n] in natural order, output X[k] at x[4 (k & 3) + (k >> 2)]
+template <typename T> __device__ __forceinline__ void fft16(Cx<T> (&x)[16])
+{
+    constexpr T C = K16<T>::C, S = K16<T>::S, H = K16<T>::H;
+#pragma unroll
+    for (int n2 = 0; n2 < 4; ++n2) dft4(x[n2], x[4 + n2], x[8 + n2], x[12 + n2]);    // x[4 k1 + n2] = sum_n1 x[4 n1 + n2] W4^{n1 k1}
+    Cx<T> v;
+    v = x[5];  x[5]  = Cx<T>{fma(v.x, C, v.y * S), fma(v.y, C, -(v.x * S))};         // W16^1
+    v = x[6];  x[6]  = Cx<T>{(v.x + v.y) * H, (v.y - v.x) * H};                        // W16^2
+    v = x[7];  x[7]  = Cx<T>{fma(v.x, S, v.y * C), fma(v.y, S, -(v.x * C))};         // W16^3
+    v = x[9];  x[9]  = Cx<T>{(v.x + v.y) * H, (v.y - v.x) * H};                        // W16^2
+    v = x[10]; x[10] = Cx<T>{v.y, -v.x};                                               // W16^4 = -i
+    v = x[11]; x[11] = Cx<T>{(v.y - v.x) * H, -((v.x + v.y) * H)};                     // W16^6
+    v = x[13]; x[13] = Cx<T>{fma(v.x, S, v.y * C), fma(v.y, S, -(v.x * C))};         // W16^3
+    v = x[14]; x[14] = Cx<T>{(v.y - v.x) * H, -((v.x + v.y) * H)};                     // W16^6
+    v = x[15]; x[15] = Cx<T>{-fma(v.x, C, v.y * S), fma(v.x, S, -(v.y * C))};        // W16^9 = -W16^1
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) dft4(x[4 * k1], x[4 * k1 + 1], x[4 * k1 + 2], x[4 * k1 + 3]);   // x[4 k1 + k2] = X[k1 + 4 k2]
+}
+__host__ __device__ constexpr int f16pos(int k) { return 4 * (k & 3) + (k >> 2); }
+
+template <typename T> __device__ __forceinline__ void st_tile(Cx<T>* p, Cx<T> v) { *p = v; }
+__device__ __forceinline__ void st_tile(__half2* p, Cx<float> v) { *p = __floats2half2_rn(v.x, v.y); }
+template <typename T> __device__ __forceinline__ Cx<T> ld_tile(const Cx<T>* p) { return *p; }
+__device__ __forceinline__ Cx<float> ld_tile(const __half2* p) { const float2 f = __half22float2(*p); return Cx<float>{f.x, f.y}; }
+
+constexpr int F16_W = 16, F16_NT = 256, F16_M1 = 256, F16_LD = F16_W + 1;
+
+template <typename T, typename ST, int PREC>
+__global__ void __launch_bounds__(F16_NT, sizeof(T) == 8 ? 1 : 2)
+mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
+               const int64_t* __restrict__ idx, double* __restrict__ partial)
+{
+    extern __shared__ __align__(16) unsigned char smraw[];
+    ST* tile = reinterpret_cast<ST*>(smraw);                                        // [256][17]
+    Cx<T>* tw = reinterpret_cast<Cx<T>*>(smraw + (size_t)F16_M1 * F16_LD * sizeof(ST));   // [256]  W_256^e
+    double* colacc = reinterpret_cast<double*>(tw + F16_M1);                        // [s]
+    Cx<T>* dstep = reinterpret_cast<Cx<T>*>(colacc + p.s);                          // [s]  (dtab only)
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int u = tid & (F16_W - 1), b = tid >> 4;                                  // pass 1: b = t1 mod 16; pass 2: b = ka
+    const int col = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
+    const double* colA = A + (size_t)col * (size_t)p.lda;
+
+    for (int e = tid; e < F16_M1; e += F16_NT) {
+        double sn, cs;
+        sincospi(-2.0 * (double)e / (double)F16_M1, &sn, &cs);
+        tw[e] = Cx<T>{(T)cs, (T)sn};
+    }
+    for (int e = tid; e < p.s; e += F16_NT) colacc[e] = 0.0;
+    if (p.dtab)
+        for (int i = tid; i < p.s; i += F16_NT) {
+            const int64_t k = idx[i];
+            Cx<T> d;
+            sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d.y, &d.x);
+            dstep[i] = d;
+        }
+
+    const int tile_lo = chunk * p.tiles_per_chunk;
+    const int tile_hi = min(p.tiles_per_col, tile_lo + p.tiles_per_chunk);
+    double2 v[16];
+    unsigned sw = 0;                                                                // sign word of row a = lane % 16 (this half warp's b)
+    auto fetch = [&](int tl) {
+        const int64_t t2_0 = (int64_t)tl * (2 * F16_W);
+        if (p.vec) {
+            const double2* src = reinterpret_cast<const double2*>(colA + t2_0) + u;
+            const int64_t m2h = p.m2 >> 1;
+#pragma unroll
+            for (int a = 0; a < 16; ++a) v[a] = __ldcs(src + (int64_t)(16 * a + b) * m2h);
+        } else {
+            const double* src = colA + t2_0 + 2 * u;
+#pragma unroll
+            for (int a = 0; a < 16; ++a) {
+                const int64_t off = (int64_t)(16 * a + b) * p.m2;
+                v[a] = make_double2(__ldcs(src + off), __ldcs(src + off + 1));
+            }
+        }
+        sw = __ldg(signs32 + (((int64_t)(16 * (lane & 15) + b) * p.m2 + t2_0) >> 5));   // m2 % 32 == 0: one word per row and tile
+    };
+    if (tile_lo < tile_hi) fetch(tile_lo);
+    for (int tl = tile_lo; tl < tile_hi; ++tl) {
+        const int64_t t2_0 = (int64_t)tl * (2 * F16_W);
+        Cx<T> x[16];
+#pragma unroll
+        for (int a = 0; a < 16; ++a) {                                              // DiagMult + cast
+            const unsigned bits = __shfl_sync(0xffffffffu, sw, (lane & 16) + a) >> (2 * u);
+            x[a] = Cx<T>{diag_cast<T, PREC>(v[a].x, bits & 1u), diag_cast<T, PREC>(v[a].y, (bits >> 1) & 1u)};
+        }
+        if (tl + 1 < tile_hi) fetch(tl + 1);                                        // in flight during both passes and stage 2
+        fft16(x);
+        __syncthreads();                                                            // stage 2 of the previous tile has read the tile
+#pragma unroll
+        for (int ka = 0; ka < 16; ++ka) {
+            Cx<T> y = x[f16pos(ka)];
+            if (ka > 0) y = cmul(y, tw[b * ka]);
+            st_tile(tile + (size_t)(16 * ka + b) * F16_LD + u, y);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int bb = 0; bb < 16; ++bb) x[bb] = ld_tile(tile + (size_t)(16 * b + bb) * F16_LD + u);
+        fft16(x);
+#pragma unroll
+        for (int kb = 0; kb < 16; ++kb) st_tile(tile + (size_t)(16 * b + kb) * F16_LD + u, x[f16pos(kb)]);
+        __syncthreads();
+        // ---- stage 2: thread = bin; Z[k1] sits in row 16 (k1 & 15) + (k1 >> 4)
+        for (int i = tid; i < p.s; i += F16_NT) {
+            const int64_t k = idx[i];
+            const int k1 = (int)(k & (F16_M1 - 1));
+            const int k1n = (F16_M1 - k1) & (F16_M1 - 1);
+            const ST* rowP = tile + (size_t)(16 * (k1 & 15) + (k1 >> 4)) * F16_LD;
+            const ST* rowQ = tile + (size_t)(16 * (k1n & 15) + (k1n >> 4)) * F16_LD;
+            Cx<T> w0, d1, d2, d16;
+            sincospi_t((T)(2.0 * (double)((k * t2_0) & (p.m - 1)) / (double)p.m), &w0.y, &w0.x);
+            if (p.dtab) d1 = dstep[i];
+            else sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d1.y, &d1.x);
+            d2 = cmul(d1, d1);
+            d16 = cmul(d2, d2); d16 = cmul(d16, d16); d16 = cmul(d16, d16);
+            T va = (T)0;
+#pragma unroll
+            for (int j8 = 0; j8 < F16_W; j8 += 8) {
+                Cx<T> we = w0;
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const Cx<T> P = ld_tile(rowP + j8 + q), Qn = ld_tile(rowQ + j8 + q);
+                    const Cx<T> wo = cmul(we, d1);
+                    va = fma(we.x, P.x + Qn.x, va); va = fma(we.y, P.y - Qn.y, va);
+                    va = fma(wo.x, P.y + Qn.y, va); va = fma(wo.y, Qn.x - P.x, va);
+                    we = cmul(we, d2);
+                }
+                w0 = cmul(w0, d16);
+            }
+            colacc[i] += 0.5 * (double)va;
+        }
+    }
+    __syncthreads();
+    double* out = partial + ((size_t)col * p.chunks + chunk) * p.s;
+    for (int e = tid; e < p.s; e += F16_NT) out[e] = colacc[e];
+}
+
 // A_s[i, j] = fl_p( sqrt(s/m) * sum_chunks partial ), chunks added in ascending order.
 template <int PREC>
 __global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial, double* __restrict__ As, Status* st)
@@ -257,12 +419,15 @@ static int k1_tile_w(int64_t m, int prec, int s, int reim)
     return w;
 }
 
+static bool k1_fft16_usable(int64_t m, int reim) { return !reim && m >= (int64_t)F16_M1 * 2 * F16_W; }   // m2 >= 32: whole sign words
+
 static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec, int reim)
 {
     K1Params p;
     p.m = m; p.lda = lda; p.n = n; p.s = s; p.reim = reim;
-    const int K1_W = k1_tile_w(m, prec, s, reim);
-    const int m1max = ((prec == 64) ? 128 : 256) * (32 / K1_W);    // 68 KB tile (W = 8: 74 KB)
+    const bool f16 = k1_fft16_usable(m, reim);
+    const int K1_W = f16 ? F16_W : k1_tile_w(m, prec, s, reim);
+    const int m1max = f16 ? F16_M1 : ((prec == 64) ? 128 : 256) * (32 / K1_W);    // 68 KB tile (W = 8: 74 KB)
     int64_t m1 = m / (2 * K1_W);
     if (m1 > m1max) m1 = m1max;
     if (m1 < 1) m1 = 1;
@@ -304,6 +469,20 @@ static void k1_launch_t(const K1Params& p_in, const double* A, const uint64_t* s
     mrcqr_k1_finalize<PREC><<<((REIM ? 2 : 1) * p.s * p.n + 255) / 256, 256, 0, stream>>>(p, partial, As, st);
 }
 
+template <typename T, typename ST, int PREC>
+static void k1_launch_fft16(const K1Params& p_in, const double* A, const uint64_t* signs, const int64_t* idx,
+                            double* partial, double* As, Status* st, cudaStream_t stream)
+{
+    K1Params p = p_in;
+    size_t smem = (size_t)F16_M1 * F16_LD * sizeof(ST) + (size_t)F16_M1 * sizeof(Cx<T>) + (size_t)p.s * sizeof(double);
+    p.dtab = 1;
+    smem += (size_t)p.s * sizeof(Cx<T>);
+    auto k = mrcqr_k1_fft16<T, ST, PREC>;
+    cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    k<<<p.n * p.chunks, F16_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
+    mrcqr_k1_finalize<PREC><<<(p.s * p.n + 255) / 256, 256, 0, stream>>>(p, partial, As, st);
+}
+
 int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int s,
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
                    Status* st, cudaStream_t stream, int reim)
@@ -315,6 +494,12 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
     }
     K1Params p = k1_params(m, n, lda, s, prec, reim);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
+    if (k1_fft16_usable(m, reim)) {
+        if (prec == 16) k1_launch_fft16<float, __half2, 16>(p, A, signs, idx, partial, As, st, stream);
+        else if (prec == 32) k1_launch_fft16<float, Cx<float>, 32>(p, A, signs, idx, partial, As, st, stream);
+        else k1_launch_fft16<double, Cx<double>, 64>(p, A, signs, idx, partial, As, st, stream);
+        return 2;
+    }
     const int w = k1_tile_w(m, prec, s, reim);
 #define K1_GO(T_, P_, W_) { if (reim) k1_launch_t<T_, P_, W_, true>(p, A, signs, idx, partial, As, st, stream); \
                             else k1_launch_t<T_, P_, W_, false>(p, A, signs, idx, partial, As, st, stream); }

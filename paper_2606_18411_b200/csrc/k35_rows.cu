@@ -224,16 +224,20 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
 // (RG = 4), keeps the panel in accumulator registers, adds the contributions of the already solved
 // panels with a left-looking sweep whose A fragments come straight from global memory (lane (g, t)
 // reads row g of column t: 64 contiguous bytes per column, every sector fully used; one step
-// prefetched ahead), then runs the same in-register panel_core as K3 / K5 and stores the solved panel.
-// Shared memory holds only the panel (18 KB per warp); the row is never resident as a whole, which is what
-// limited the in-place slab solve to 8-row groups beyond n = 128.
-// The -R fragments of the left-looking sweep are shared by the 4 warps of the CTA: chunks of 4 block rows
-// (4 x PB x 512 B) are staged in shared memory by cp.async, double buffered, one barrier per chunk.  A CTA's
-// round is load -> sweep -> solve -> store in lockstep, so two CTAs share an SM (105 KB each) and one's
-// memory phases overlap the other's DMMA phases (8 warps in one CTA: 6.07 ms per solve at C3, this: 5.90).
+// prefetched ahead), then runs the same in-register panel_core as K3 / K5.
+// Memory phases are off the critical path of a warp (round-1 profile of panel 0: 30 % of a warp's time waiting for its
+// slab and its stores, 31 % DMMA): the slab buffer is only the LANDING ZONE of the cp.async load -- once the panel is in
+// accumulator registers the NEXT round's slab is requested into the same buffer and arrives during the solve; the 8x8
+// transposes of panel_core go through a small per-warp scratch block, and every solved block leaves for global memory
+// straight from its row form (lane = row: 256 contiguous bytes per column and warp), so there is no store phase.
+// The panel's diagonal blocks sit at the start of c_pdiag (uploaded per launch): compile-time constant-bank operands.
+// The -R fragments of the left-looking sweep are shared by the 4 warps of the CTA: chunks of PP_KC block rows
+// (PP_KC x PB x 512 B) are staged in shared memory by cp.async, double buffered, one barrier per chunk; the panel's own
+// off-diagonal pairs (14 KB) are staged once per CTA (from L1 / L2 they cost an exposed ~600-cycle load per block step:
+// with 228 KB of shared memory carved out the L1 is 28 KB).  Two CTAs per SM.
 constexpr int PP_NW = 4;              // warps per CTA
-constexpr int PP_KC = 4;              // block rows of R per staged chunk
-constexpr int PP_CTAS = 2;            // CTAs per SM: their load / solve / store phases interleave
+constexpr int PP_KC = 2;              // block rows of R per staged chunk (two chunk buffers + the panel's own pairs fit beside two CTAs' slabs)
+constexpr int PP_CTAS = 2;            // CTAs per SM
 
 template <int FAC, int PB>
 __global__ void __launch_bounds__(PP_NW * 32, PP_CTAS)
@@ -246,11 +250,13 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
     double* slab = Ysm + (size_t)warp * (8 * PB) * LDS_;
-    double2* Bsm = reinterpret_cast<double2*>(Ysm + (size_t)PP_NW * (8 * PB) * LDS_);   // [2][PB][PP_KC][32]
-    zero_pad_columns<SR>(slab, ncols, 8 * PB, lane);
+    double* scr = Ysm + (size_t)PP_NW * (8 * PB) * LDS_ + (size_t)warp * 8 * LDS_;
+    double2* Bsm = reinterpret_cast<double2*>(Ysm + (size_t)PP_NW * (8 * PB + 8) * LDS_);   // [2][PB][PP_KC][32]
+    double2* Own = Bsm + 2 * PB * PP_KC * 32;                                               // [PB (PB-1) / 2][32]: pairs inside the panel
+    zero_pad_columns<SR>(slab, ncols, 8 * PB, lane);       // the loads below never touch the padding columns
     double* yw = slab + t * LDS_ + g;
     const int nchunks = (P0 + PP_KC - 1) / PP_KC;
-    auto stage_chunk = [&](int c) {                  // block rows [8c, 8c+8) x the PB block columns of the panel
+    auto stage_chunk = [&](int c) {                  // block rows [4c, 4c+4) x the PB block columns of the panel
         double2* dstb = Bsm + (size_t)(c & 1) * PB * PP_KC * 32;
         for (int e = tid; e < PB * PP_KC * 32; e += PP_NW * 32) {
             const int J = e / (PP_KC * 32), kl = (e / 32) % PP_KC, ln = e & 31;
@@ -260,13 +266,25 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     const int64_t rounds = (nslabs + (int64_t)gridDim.x * PP_NW - 1) / ((int64_t)gridDim.x * PP_NW);
+    const PanelFactor<FAC, PB> fac{Own, P0};
+    for (int e = tid; e < PB * (PB - 1) / 2 * 32; e += PP_NW * 32) {     // once per CTA: the first round's barrier publishes them
+        int J = 1;
+        while ((J + 1) * J / 2 <= e / 32) ++J;
+        const int K = e / 32 - J * (J - 1) / 2;
+        Own[e] = __ldg(fragpair(frag, P0 + K, P0 + J, e & 31));
+    }
+    {                                                // round 0's slab
+        const int64_t i0 = (int64_t)blockIdx.x * PP_NW + warp;
+        __syncwarp();
+        if (i0 < nslabs) load_slab<SR, true>(slab, own, ld_own, m, ncols, i0 * SR, lane);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
     for (int64_t r = 0; r < rounds; ++r) {
         const int64_t i = (r * gridDim.x + blockIdx.x) * PP_NW + warp;
         const bool active = i < nslabs;
         const int64_t row0 = i * SR;
+        const int64_t inext = ((r + 1) * gridDim.x + blockIdx.x) * PP_NW + warp;
         __syncthreads();                             // previous round done with both chunk buffers
-        if (active) load_slab<SR, true>(slab, own, ld_own, m, ncols, row0, lane);
-        asm volatile("cp.async.commit_group;" ::: "memory");
         if (nchunks > 0) stage_chunk(0);
         const double* yp = Yprev + (size_t)t * (size_t)ldy + row0 + g;
         double a0[RG], a1[RG];
@@ -274,7 +292,7 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
 #pragma unroll
             for (int rg = 0; rg < RG; ++rg) { a0[rg] = yp[8 * rg]; a1[rg] = yp[(size_t)4 * ldy + 8 * rg]; }
         }
-        if (nchunks > 0) asm volatile("cp.async.wait_group 1;" ::: "memory");     // own panel landed
+        if (nchunks > 0) asm volatile("cp.async.wait_group 1;" ::: "memory");     // own panel landed (requested a round ago)
         else asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncwarp();
         double acc[RG][PB][2];
@@ -287,10 +305,17 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
                     acc[rg][J][1] = yw[(8 * J + 4) * LDS_ + 8 * rg];
                 }
         }
+        __syncwarp();                                // every lane has its fragments: the landing zone is free again
+        auto prefetch = [&]() {                      // next round's slab, behind every chunk group of this round
+            if (inext < nslabs) load_slab<SR, true>(slab, own, ld_own, m, ncols, inext * SR, lane);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        if (nchunks == 0) prefetch();
         for (int c = 0; c < nchunks; ++c) {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncthreads();                         // chunk c visible; everyone is done with chunk c-1
             if (c + 1 < nchunks) stage_chunk(c + 1);
+            else prefetch();
             if (active) {
                 const double2* bs = Bsm + (size_t)(c & 1) * PB * PP_KC * 32 + lane;
                 const int kend = (P0 - PP_KC * c < PP_KC) ? P0 - PP_KC * c : PP_KC;
@@ -315,11 +340,18 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
             }
         }
         if (active) {
-            panel_core<RG, PB>(acc, SlabXpose<RG>(slab - (size_t)(8 * P0) * LDS_, lane), ConstFactor<FAC>{frag}, P0, lane, NoSink());
-            __syncwarp();
-            store_slab<SR, true>(slab, dst, ldd, m, ncols, row0, lane);
+            double* out = dst + row0 + lane;         // lane = row of the slab
+            auto sink = [&](int Kg, const double (&y)[8]) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int col = 8 * (Kg - P0) + j;
+                    if (col < ncols) __stcs(out + (size_t)col * (size_t)ldd, y[j]);
+                }
+            };
+            panel_core<RG, PB>(acc, ScratchXpose<RG>(scr, lane), fac, P0, lane, sink);
         }
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
 // G16[i,j] (i <= j) = sum over the CTA partials in a FIXED order (deterministic split-m reduction):
@@ -474,7 +506,9 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
         const int pb = (nB - P0 >= 8) ? 8 : nB - P0;
         int ncols = n - 8 * P0;
         if (ncols > 8 * pb) ncols = 8 * pb;
-        const int smem = nw * (8 * pb) * 36 * 8 + 2 * pb * PP_KC * 512;
+        const int smem = nw * (8 * pb + 8) * 36 * 8 + 2 * pb * PP_KC * 512 + pb * (pb - 1) / 2 * 512;
+        cudaMemcpyToSymbolAsync(c_pdiag, prep + prep_diag_offset(nB) + (size_t)P0 * PREP_DIAG, sizeof(double) * PREP_DIAG * pb,
+                                sizeof(double) * (size_t)fac * 8 * PREP_DIAG, cudaMemcpyDeviceToDevice, s);
         const double* own = src + (size_t)(8 * P0) * (size_t)lds;
         double* out = dstp + (size_t)(8 * P0) * (size_t)ldd;
 #define PP_GO(FAC_, PB_)                                                                            \

@@ -147,6 +147,22 @@ struct ConstFactor {
     __device__ __forceinline__ const double* diag(int Kg) const { return &c_diag[FAC][Kg * PREP_DIAG]; }
 };
 #endif
+#ifndef MRCQR_NO_CONST_DIAG
+// PanelFactor: one 64-column panel starting at block P0 (the panel passes): its off-diagonal pairs staged in shared memory, the
+// panel's own diagonal blocks at the START of c_pdiag[FAC] (uploaded per launch), so that block K of the panel has
+// compile-time constant-bank offsets and the coefficients are instruction operands, not loads.
+__constant__ double c_pdiag[2][8 * PREP_DIAG];
+template <int FAC, int PB>
+struct PanelFactor {
+    const double2* own; int P0;                     // own: the panel's off-diagonal pairs (K < J inside the panel) in shared memory
+    __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const
+    {
+        const int K = Kg - P0, J = Jg - P0;
+        return own[(J * (J - 1) / 2 + K) * 32 + lane];
+    }
+    __device__ __forceinline__ const double* diag(int Kg) const { return &c_pdiag[FAC][(Kg - P0) * PREP_DIAG]; }
+};
+#endif
 struct SmemFactor {
     const double* prep; int nB;
     __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const
@@ -165,6 +181,18 @@ struct SlabXpose {
     __device__ __forceinline__ SlabXpose(double* s, int l) : slab(s), lane(l), g(l >> 2), t(l & 3) {}
     __device__ __forceinline__ double* accp(int Kg, int rg, int e) const { return slab + (8 * Kg + t + 4 * e) * LDS_ + 8 * rg + g; }
     __device__ __forceinline__ double* rowp(int Kg, int j) const { return slab + (8 * Kg + j) * LDS_ + lane; }
+    __device__ __forceinline__ bool row_active() const { return SR >= 32 || lane < SR; }
+};
+// ScratchXpose: through ONE per-warp scratch block (8 columns, leading dimension SR + 4) that every block of the panel
+// reuses; the solved block goes to the sink (e.g. straight to global memory in row form), not to a slab.
+template <int RG>
+struct ScratchXpose {
+    static constexpr int SR = 8 * RG, LDS_ = SR + 4;
+    static constexpr bool REUSE = true;
+    double* scr; int lane, g, t;
+    __device__ __forceinline__ ScratchXpose(double* s, int l) : scr(s), lane(l), g(l >> 2), t(l & 3) {}
+    __device__ __forceinline__ double* accp(int, int rg, int e) const { return scr + (t + 4 * e) * LDS_ + 8 * rg + g; }
+    __device__ __forceinline__ double* rowp(int, int j) const { return scr + j * LDS_ + lane; }
     __device__ __forceinline__ bool row_active() const { return SR >= 32 || lane < SR; }
 };
 struct NoSink { __device__ __forceinline__ void operator()(int, const double (&)[8]) const {} };
