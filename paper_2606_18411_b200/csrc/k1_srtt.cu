@@ -404,18 +404,14 @@ __global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial
     As[e] = v;
 }
 
-// tile width W (complex elements = 2W consecutive t2 of one column): halving W doubles m1 at the same tile size (FP64:
-// 256 at W = 16, FP32 arithmetic: 512), W = 8 doubles it again (FP64 with s >= 512: C3 3.40 -> 3.30 ms, n = 512
-// 9.8 -> 9.0 ms).  16 is taken for FP64, and for FP16/FP32 sketches with s >= 1024 where stage 2 dominates; short
-// columns (m < 64 W) take the widest tile that still leaves m1 >= 2.
+// tile width W of the shared-memory radix-4 form (complex elements = 2W consecutive t2 of one column).  That form now
+// serves only short columns (m < 8192) and the Re+Im variant: 32-wide tiles, narrower ones where the column is too short
+// for them (m >= 32: 2W <= m / 2).
 static int k1_tile_w(int64_t m, int prec, int s, int reim)
 {
+    (void)prec; (void)s; (void)reim;
     int w = 32;
-    if (!reim) {                                       // the Re+Im variant is built for the 32-wide tile only
-        if (prec == 64) w = (s >= 512 && m >= 512 * 32) ? 8 : (m >= 256 * 32 ? 16 : 32);
-        else w = (s >= 1024 && m >= 512 * 32) ? 16 : 32;   // measured: s = 256 slower (0.50 -> 0.58 ms at C2), 512 equal, 1024 6.9 -> 6.0 ms
-    }
-    while (w > 8 && 4 * (int64_t)w > m) w >>= 1;       // m >= 32: 2W <= m / 2
+    while (w > 8 && 4 * (int64_t)w > m) w >>= 1;
     return w;
 }
 
@@ -450,8 +446,7 @@ size_t k1_workspace_bytes(int64_t m, int n, int s, int prec)
         const size_t b = (size_t)n * p.chunks * (reim ? 2 : 1) * (size_t)s * sizeof(double);
         if (b > fft) fft = b;
     }
-    const size_t tc = k1_tc_workspace_bytes();
-    return fft > tc ? fft : tc;
+    return fft;
 }
 
 template <typename T, int PREC, int W, bool REIM = false>
@@ -488,10 +483,6 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
                    Status* st, cudaStream_t stream, int reim)
 {
     double* partial = reinterpret_cast<double*>(k1_work);
-    if (!reim && k1_tc_usable(m, n, lda, A, prec, s)) {
-        const int k = launch_k1_tc(m, n, lda, A, s, signs, idx, k1_work, As, st, stream);
-        if (k > 0) return k;                          // < 0: the tensor map could not be encoded -> FFT form
-    }
     K1Params p = k1_params(m, n, lda, s, prec, reim);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
     if (k1_fft16_usable(m, reim)) {

@@ -119,12 +119,6 @@ int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
                    Status* st, cudaStream_t stream, int reim = 0);      // reim: 2s rows, Im X[S] below Re X[S]
 
-// K1, tensor-core form for the FP16 sketch with s <= 128 (k1_tc.cu)
-bool k1_tc_usable(int64_t m, int n, int64_t lda, const double* A, int prec, int s);
-size_t k1_tc_workspace_bytes();
-int launch_k1_tc(int64_t m, int n, int64_t lda, const double* A, int s, const uint64_t* signs,
-                 const int64_t* idx, void* work, double* As, Status* st, cudaStream_t stream);
-
 // batched small problems, one CTA per problem (k_batched.cu); codes_dev: batch x 2 ints (code, info)
 bool batched_fused_usable(int64_t m, int n, int s);
 int launch_factor_batched(int batch, int64_t m, int n, int64_t lda, int64_t strideA, const double* A, int64_t ldq,

@@ -1,5 +1,5 @@
 """GPU parity of the kernel variants mrcqr_factor dispatches to beyond the basic shapes of
-test_gpu_parity.py: the tensor-core form of K1 (FP16 sketch, s <= 128, padded bin counts), the
+test_gpu_parity.py: the register radix-16 form of K1 for the FP16 sketch (odd bin counts, one and several tiles), the
 store-Y form of stage 2 for n16 > 128 (panel passes + SYRK Gram, every panel width, ragged n),
 and the fall-backs taken for unaligned operands.  Same tolerances as test_gpu_parity.py."""
 import numpy as np
@@ -15,13 +15,13 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("m,n,s", [
-    (1 << 13, 8, 24),        # s padded to 32: 2 m-tiles x 4 column groups, single tile per column
-    (1 << 14, 25, 50),       # s padded to 64, odd n
-    (1 << 15, 33, 100),      # s padded to 128, CTA ranges spanning two columns
+    (1 << 13, 8, 24),        # one tile per column (m2 = 32)
+    (1 << 14, 25, 50),       # two tiles per column, odd n
+    (1 << 15, 33, 100),      # four tiles, s not a multiple of 32
     (1 << 14, 64, 128),      # the C1 geometry at small m
-    (1 << 13, 150, 128),     # n > s is illegal for QR, but the sketch alone must still be right -> use stage call only
+    (1 << 13, 150, 128),     # n > s is illegal for QR: the stage call rejects it
 ])
-def test_tensor_core_sketch_matches_oracle(orc, m, n, s):
+def test_half_sketch_matches_oracle(orc, m, n, s):
     AT = inputs.make_A(m, n, 2, 300 + n, 301 + n, "cuda")
     A = to_np(AT)
     signs, idx = orc.draw(m, s, 77 + n)
@@ -39,7 +39,7 @@ def test_tensor_core_sketch_matches_oracle(orc, m, n, s):
             B.mrcqr_sketch(AT, B.FP16, dsigns, didx, want_As=True)
 
 
-def test_tensor_core_sketch_closed_form(orc):
+def test_half_sketch_closed_form(orc):
     """Column j = d * cos(2 pi k_j t / m) (signs undone): the transform has one line, at bin k_j, of height
     m/2 (m at DC / Nyquist); after the sqrt(s/m) scale the sketch is that value at (j, j) and zero elsewhere."""
     m, n, s = 1 << 13, 16, 32
@@ -61,15 +61,20 @@ def test_tensor_core_sketch_closed_form(orc):
 
 
 @pytest.mark.parametrize("m,n,s,prec,tol", [
-    (1 << 13, 5, 40, 64, 1e-12),       # FP64: 16-wide tiles, m1 = 256, m2 = 32 (one sign word per tile row pair)
-    (1 << 15, 6, 96, 64, 1e-12),       # FP64: several tiles per chunk, even n
-    (1 << 14, 4, 520, 64, 1e-12),      # FP64, s >= 512: 8-wide tiles, m1 = 512
-    (1 << 14, 3, 1024, 32, 5e-5),      # FP32, s >= 1024: 16-wide tiles, m1 = 512, odd n
-    (1 << 15, 4, 1030, 16, 1e-2),      # FP16 rounding of the same form, ragged s
-    (1 << 12, 5, 40, 64, 1e-12),       # FP64 below the 16-wide threshold: 32-wide tiles, m1 = 128
+    (1 << 13, 5, 40, 64, 1e-12),       # radix-16 form, FP64: one tile per column (m2 = 32)
+    (1 << 15, 6, 96, 64, 1e-12),       # radix-16 form, FP64: four tiles per column, even n
+    (1 << 14, 4, 520, 64, 1e-12),      # radix-16 form, s > 256: three bins per thread in stage 2
+    (1 << 14, 3, 1024, 32, 5e-5),      # radix-16 form, FP32, s = 1024, odd n
+    (1 << 15, 4, 1030, 16, 1e-2),      # radix-16 form, FP16 tile storage, ragged s
+    (1 << 17, 3, 48, 32, 5e-5),        # radix-16 form, several tiles per chunk
+    (1 << 12, 5, 40, 64, 1e-12),       # radix-4 form (m < 8192): 32-wide tiles, m1 = 64
+    (1 << 12, 6, 200, 32, 5e-5),       # radix-4 form, FP32
+    (1 << 10, 4, 100, 16, 1e-2),       # radix-4 form, FP16 rounding, m1 = 16
+    (256, 3, 129, 64, 1e-12),          # radix-4 form, every bin (s = m/2 + 1), m1 = 4
 ])
 def test_fft_sketch_tile_widths_match_oracle(orc, m, n, s, prec, tol):
-    """The FFT form of K1 (k1_srtt.cu) picks the tile width from (m, prec, s); every choice is the same transform."""
+    """K1 (k1_srtt.cu) takes the register radix-16 form for m >= 8192 and the shared-memory radix-4 form, whose tile
+    width depends on (m, prec, s), below; every choice is the same transform."""
     AT = inputs.make_A(m, n, 3, 500 + n, 501 + n, "cuda")
     A = to_np(AT)
     signs, idx = orc.draw(m, s, 900 + n)
@@ -265,7 +270,7 @@ def test_graph_replay_gives_the_same_bits(orc, m, n, prec):
     """mrcqr_set_graph(1): the captured pipeline replays with new seeds (seed and bins are graph data) and returns
     exactly what the ordinary path returns, positive codes included.  Capture is illegal on the legacy default stream,
     so the replays run on a stream of their own and mrcqr_last_used_graph() must say that a graph ran (n = 16: the
-    register QR, n = 64: the tensor-core sketch with its TMA descriptor, n > 128: the cooperative K2 / K4 launches
+    register QR, n = 64: the half-storage sketch, n > 128: the cooperative K2 / K4 launches
     and the panel passes)."""
     AT = inputs.make_A(m, n, 3, 300 + n, 301 + n, "cuda")
     QT = torch.empty_like(AT); R = torch.empty((n, n), dtype=torch.float64, device="cuda")
@@ -354,7 +359,7 @@ def _margins_intact(buf, inner_elems, margin=4096, fill=-1234.5):
 
 @pytest.mark.parametrize("m,n,s,prec,pad", [
     (4096, 16, 32, 32, 0),       # register K2, K3 / K5 at n16 = 16, single-CTA Cholesky
-    (1 << 14, 64, 128, 16, 0),   # tensor-core K1 (TMA), n16 = 64
+    (1 << 14, 64, 128, 16, 0),   # FP16 tile storage in K1, n16 = 64
     (1 << 13, 50, 150, 64, 6),   # ragged n, lda > m: the padding rows of Q must stay untouched
     (1 << 13, 100, 200, 32, 0),  # blocked (cooperative) K2, n16 = 112
     (1 << 12, 136, 272, 64, 2),  # panel passes + SYRK, cooperative K4... n16 = 144, lda > m
