@@ -232,11 +232,12 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
 // straight from its row form (lane = row: 256 contiguous bytes per column and warp), so there is no store phase.
 // The panel's diagonal blocks sit at the start of c_pdiag (uploaded per launch): compile-time constant-bank operands.
 // The -R fragments of the left-looking sweep are shared by the 4 warps of the CTA: chunks of PP_KC block rows
-// (PP_KC x PB x 512 B) are staged in shared memory by cp.async, double buffered, one barrier per chunk; the panel's own
-// off-diagonal pairs (14 KB) are staged once per CTA (from L1 / L2 they cost an exposed ~600-cycle load per block step:
-// with 228 KB of shared memory carved out the L1 is 28 KB).  Two CTAs per SM.
+// (PP_KC x PB x 512 B) are staged in shared memory by cp.async, double buffered, one barrier per chunk.  The panel's own
+// off-diagonal pairs come from L1 / L2 (panel_core requests the one on its critical path a step ahead); staging them in
+// shared memory was measured slower either way it fits (once per CTA beside 2-row chunks: 5.45 ms per solve at C3; as two
+// more chunks of the pipeline: 5.44; this form: 5.36): every CTA barrier per round costs more than the loads.  Two CTAs per SM.
 constexpr int PP_NW = 4;              // warps per CTA
-constexpr int PP_KC = 2;              // block rows of R per staged chunk (two chunk buffers + the panel's own pairs fit beside two CTAs' slabs)
+constexpr int PP_KC = 4;              // block rows of R per staged chunk
 constexpr int PP_CTAS = 2;            // CTAs per SM
 
 template <int FAC, int PB>
@@ -252,7 +253,6 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
     double* slab = Ysm + (size_t)warp * (8 * PB) * LDS_;
     double* scr = Ysm + (size_t)PP_NW * (8 * PB) * LDS_ + (size_t)warp * 8 * LDS_;
     double2* Bsm = reinterpret_cast<double2*>(Ysm + (size_t)PP_NW * (8 * PB + 8) * LDS_);   // [2][PB][PP_KC][32]
-    double2* Own = Bsm + 2 * PB * PP_KC * 32;                                               // [PB (PB-1) / 2][32]: pairs inside the panel
     zero_pad_columns<SR>(slab, ncols, 8 * PB, lane);       // the loads below never touch the padding columns
     double* yw = slab + t * LDS_ + g;
     const int nchunks = (P0 + PP_KC - 1) / PP_KC;
@@ -266,13 +266,7 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     const int64_t rounds = (nslabs + (int64_t)gridDim.x * PP_NW - 1) / ((int64_t)gridDim.x * PP_NW);
-    const PanelFactor<FAC, PB> fac{Own, P0};
-    for (int e = tid; e < PB * (PB - 1) / 2 * 32; e += PP_NW * 32) {     // once per CTA: the first round's barrier publishes them
-        int J = 1;
-        while ((J + 1) * J / 2 <= e / 32) ++J;
-        const int K = e / 32 - J * (J - 1) / 2;
-        Own[e] = __ldg(fragpair(frag, P0 + K, P0 + J, e & 31));
-    }
+    const PanelFactor<FAC> fac{frag, P0};
     {                                                // round 0's slab
         const int64_t i0 = (int64_t)blockIdx.x * PP_NW + warp;
         __syncwarp();
@@ -290,7 +284,7 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
         double a0[RG], a1[RG];
         if (P0 > 0 && active) {
 #pragma unroll
-            for (int rg = 0; rg < RG; ++rg) { a0[rg] = yp[8 * rg]; a1[rg] = yp[(size_t)4 * ldy + 8 * rg]; }
+            for (int rg = 0; rg < RG; ++rg) { a0[rg] = __ldcs(yp + 8 * rg); a1[rg] = __ldcs(yp + (size_t)4 * ldy + 8 * rg); }
         }
         if (nchunks > 0) asm volatile("cp.async.wait_group 1;" ::: "memory");     // own panel landed (requested a round ago)
         else asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -325,7 +319,7 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
                     const int Kn = (Kg + 1 < P0) ? Kg + 1 : Kg;
                     const double* yn = yp + (size_t)(8 * Kn) * (size_t)ldy;
 #pragma unroll
-                    for (int rg = 0; rg < RG; ++rg) { n0[rg] = yn[8 * rg]; n1[rg] = yn[(size_t)4 * ldy + 8 * rg]; }
+                    for (int rg = 0; rg < RG; ++rg) { n0[rg] = __ldcs(yn + 8 * rg); n1[rg] = __ldcs(yn + (size_t)4 * ldy + 8 * rg); }
 #pragma unroll
                     for (int J = 0; J < PB; ++J) {
                         const double2 b = bs[(J * PP_KC + kl) * 32];
@@ -506,7 +500,7 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
         const int pb = (nB - P0 >= 8) ? 8 : nB - P0;
         int ncols = n - 8 * P0;
         if (ncols > 8 * pb) ncols = 8 * pb;
-        const int smem = nw * (8 * pb + 8) * 36 * 8 + 2 * pb * PP_KC * 512 + pb * (pb - 1) / 2 * 512;
+        const int smem = nw * (8 * pb + 8) * 36 * 8 + 2 * pb * PP_KC * 512;
         cudaMemcpyToSymbolAsync(c_pdiag, prep + prep_diag_offset(nB) + (size_t)P0 * PREP_DIAG, sizeof(double) * PREP_DIAG * pb,
                                 sizeof(double) * (size_t)fac * 8 * PREP_DIAG, cudaMemcpyDeviceToDevice, s);
         const double* own = src + (size_t)(8 * P0) * (size_t)lds;

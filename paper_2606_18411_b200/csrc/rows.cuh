@@ -148,18 +148,14 @@ struct ConstFactor {
 };
 #endif
 #ifndef MRCQR_NO_CONST_DIAG
-// PanelFactor: one 64-column panel starting at block P0 (the panel passes): its off-diagonal pairs staged in shared memory, the
+// PanelFactor: one 64-column panel starting at block P0 (the panel passes): off-diagonal pairs from global memory, the
 // panel's own diagonal blocks at the START of c_pdiag[FAC] (uploaded per launch), so that block K of the panel has
 // compile-time constant-bank offsets and the coefficients are instruction operands, not loads.
 __constant__ double c_pdiag[2][8 * PREP_DIAG];
-template <int FAC, int PB>
+template <int FAC>
 struct PanelFactor {
-    const double2* own; int P0;                     // own: the panel's off-diagonal pairs (K < J inside the panel) in shared memory
-    __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const
-    {
-        const int K = Kg - P0, J = Jg - P0;
-        return own[(J * (J - 1) / 2 + K) * 32 + lane];
-    }
+    const double2* __restrict__ frag; int P0;
+    __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const { return __ldg(fragpair(frag, Kg, Jg, lane)); }
     __device__ __forceinline__ const double* diag(int Kg) const { return &c_pdiag[FAC][(Kg - P0) * PREP_DIAG]; }
 };
 #endif
@@ -212,6 +208,11 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
     double ap0[RG], ap1[RG];                                  // A fragments of block K-1
 #pragma unroll
     for (int K = 0; K < PB; ++K) {
+        // the pair this step's critical update needs is requested before the transposition (the __syncwarp()s below
+        // keep the compiler from hoisting it): an L1 miss then hides under the substitution
+        // (panel passes only: K3 / K5 run more warps on fewer registers and lose by the longer live range)
+        double2 bnext = make_double2(0.0, 0.0);
+        if (X::REUSE && K + 1 < PB) bnext = fac.pair(P0 + K, P0 + K + 1, lane);
 #pragma unroll
         for (int rg = 0; rg < RG; ++rg) { *xp.accp(P0 + K, rg, 0) = acc[rg][K][0]; *xp.accp(P0 + K, rg, 1) = acc[rg][K][1]; }
         __syncwarp();
@@ -244,11 +245,11 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
             for (int rg = 0; rg < RG; ++rg) { acc[rg][K][0] = ap0[rg]; acc[rg][K][1] = ap1[rg]; }
         }
         if (K + 1 < PB) {
-            const double2 b = fac.pair(P0 + K, P0 + K + 1, lane);
+            if (!X::REUSE) bnext = fac.pair(P0 + K, P0 + K + 1, lane);
 #pragma unroll
-            for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][K + 1], ap0[rg], b.x);
+            for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][K + 1], ap0[rg], bnext.x);
 #pragma unroll
-            for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][K + 1], ap1[rg], b.y);
+            for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][K + 1], ap1[rg], bnext.y);
         }
         if (X::REUSE) __syncwarp();
     }
