@@ -2,7 +2,7 @@
 //   K2  mrcqr_k2_sketch_qr  Algorithm 2 steps 5-6: Householder R-factor of the
 //                           s x n sketch, rows sign-normalised to diag > 0, FP64 arithmetic on the
 //                           precision-p sketch values (>= p; PAPER.md:119 promotes FP16 to FP32).
-//   K4  mrcqr_k4_cholesky   Algorithm 1 step 2: G = Rc^T Rc; a pivot <= 0 or NaN is
+//   K4  mrcqr_k4_cholesky_sm   Algorithm 1 step 2: G = Rc^T Rc; a pivot <= 0 or NaN is
 //                           reported, never shifted away.
 //   prep_R                  builds the "prepared" factor the tile solve consumes.
 //   triu_mul                Algorithm 2 step 9: R = Rc Rs.
@@ -38,108 +38,10 @@ __global__ void mrcqr_triu_mul(const double* __restrict__ Rc, const double* __re
 }
 
 // ---- K4 ---------------------------------------------------------------------------------------
-// Blocked right-looking Cholesky, 8 columns per outer step (3 barriers per 8 columns instead of 16):
-//   (1) warp 0 factors the 8x8 diagonal block (lane j owns column j in registers, shuffles); a pivot
-//       costs one rsqrt: Rc[p,p] = piv * rsqrt(piv), and rows are scaled by rsqrt(piv),
-//   (2) one thread per trailing column solves its 8 rows against the block (the row panel) with the
-//       stored reciprocals of the diagonal,
-//   (3) rank-8 update of the trailing upper triangle.
-// W: working copy of G (upper triangle used), col-major with leading dimension ldw.
-// Pn: the current row panel, Pn[p * n16 + j] = Rc[k0+p, j].  dinv[j] = 1 / Rc[j,j].
-// Epilogue: Rc, the prepared Rc (fragment order) and, if Rs is given, R = Rc Rs (Algorithm 2 step 9).
-__global__ void __launch_bounds__(SMALL_NT)
-mrcqr_k4_cholesky(double* __restrict__ G16, int n, int n16, int use_smem, double* __restrict__ G_out,
-                  double* __restrict__ Rc, double* __restrict__ RcPrep, const double* __restrict__ Rs,
-                  double* __restrict__ R, Status* st)
-{
-    extern __shared__ __align__(16) double sm[];
-    double* Pn = sm;                         // 8 * n16
-    double* dinv = sm + 8 * n16;             // n16
-    double* W = use_smem ? sm + 9 * n16 : G16;
-    const int ldw = use_smem ? n16 + 1 : n16;
-    const int tid = threadIdx.x, NT = blockDim.x;
-
-    for (int e = tid; e < n * n; e += NT) {
-        const int i = e % n, j = e / n;
-        const double v = G16[(size_t)j * n16 + i];
-        if (G_out) G_out[e] = v;
-        if (use_smem) W[j * ldw + i] = v;
-    }
-    __syncthreads();
-    for (int k0 = 0; k0 < n; k0 += 8) {
-        const int kb = min(8, n - k0);
-        if (tid < 32) {                      // (1) diagonal block, lane j < kb owns column k0 + j
-            const int j = tid;
-            double c[8];
-#pragma unroll
-            for (int p = 0; p < 8; ++p) c[p] = (j < kb && p <= j && p < kb) ? W[(k0 + j) * ldw + k0 + p] : 0.0;
-#pragma unroll
-            for (int p = 0; p < 8; ++p) {
-                if (p < kb) {                                        // uniform
-                    const double piv = __shfl_sync(0xffffffffu, c[p], p);
-                    if (j == p && (!(piv > 0.0) || isinf(piv))) report(st, 3, k0 + p);
-                    const double ri = rsqrt(piv);
-                    const double rp = (j == p) ? piv * ri : c[p] * ri;   // Rc[k0+p, k0+j] for j >= p
-                    c[p] = rp;
-                    if (j == p) dinv[k0 + p] = ri;
-#pragma unroll
-                    for (int q = p + 1; q < 8; ++q) {                // c[q] -= Rc[p, q] * Rc[p, j]  (q <= j)
-                        const double rq = __shfl_sync(0xffffffffu, rp, q);
-                        if (q <= j) c[q] = fma(-rq, rp, c[q]);
-                    }
-                }
-            }
-#pragma unroll
-            for (int p = 0; p < 8; ++p)
-                if (j < kb && p <= j && p < kb) W[(k0 + j) * ldw + k0 + p] = c[p];
-        }
-        __syncthreads();
-        for (int j = k0 + kb + tid; j < n; j += NT) {               // (2) row panel: U^T x = w, U the 8x8 block
-            double x[8];
-#pragma unroll
-            for (int p = 0; p < 8; ++p) {
-                if (p < kb) {
-                    double t = W[j * ldw + k0 + p];
-#pragma unroll
-                    for (int q = 0; q < p; ++q) t = fma(-W[(k0 + p) * ldw + k0 + q], x[q], t);
-                    x[p] = t * dinv[k0 + p];
-                    W[j * ldw + k0 + p] = x[p];
-                    Pn[p * n16 + j] = x[p];
-                } else x[p] = 0.0;
-            }
-        }
-        __syncthreads();
-        const int t0 = k0 + kb, L = n - t0;                          // (3) trailing update
-        for (int e = tid; e < L * L; e += NT) {
-            const int i = t0 + e % L, j = t0 + e / L;
-            if (i <= j) {
-                double acc = W[j * ldw + i];
-#pragma unroll
-                for (int p = 0; p < 8; ++p)
-                    if (p < kb) acc = fma(-Pn[p * n16 + i], Pn[p * n16 + j], acc);
-                W[j * ldw + i] = acc;
-            }
-        }
-        __syncthreads();
-    }
-    for (int e = tid; e < n * n; e += NT) {
-        const int i = e % n, j = e / n;
-        double w = 0.0, r = 0.0;
-        if (i <= j) {
-            w = W[j * ldw + i];
-            if (R) for (int k = i; k <= j; ++k) r = fma(W[k * ldw + i], Rs[(size_t)j * n + k], r);
-        }
-        Rc[e] = w;
-        if (R) R[e] = r;
-    }
-    {                                        // prepared Rc (fragment order + diagonal blocks), from W
-        const int nB = n16 >> 3;
-        const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
-        int bad = -1;
-        for (size_t o = tid; o < total; o += NT) RcPrep[o] = prep_value(W, ldw, n, nB, o, &bad);
-    }
-}
-
+// (A blocked single-CTA form -- 8-column steps: diagonal block by one warp, row panel by one thread per column, rank-8
+// update -- was measured slower than the one-barrier-per-pivot kernel below at every n <= 128: 71 vs 48 us at n = 64,
+// 212 vs 183 us at n = 128; its panel solve is a 36-deep chain of shared-memory loads and its diagonal block 8 software
+// rsqrt.  It is not kept.)
 // 1/sqrt(x) for a positive finite double: hardware seed + two Newton steps (a few ulp; the pivot's own
 // rounding error is of the same size).  Short dependent chain: it sits on the critical path of every pivot.
 __device__ __forceinline__ double rsqrt_fast(double x)
