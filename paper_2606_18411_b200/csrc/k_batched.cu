@@ -31,7 +31,7 @@ struct BatchParams {
     int64_t m, lda, strideA, ldq, strideQ;
     uint64_t seed;
     const double* A; double* Q; double* R; int* codes;        // codes: batch x 2 ints (code, info), device
-    int tr;                                                    // rows per sketch tile (min(m, 128))
+    int tr, tr_sh;                                             // rows per sketch tile (min(m, 128), a power of two) and its log2
     // shared-memory layout (byte offsets)
     int o_idx, o_kept, o_as, o_rs, o_prepS, o_prepC, o_w, o_work, total;
 };
@@ -147,7 +147,7 @@ __device__ __forceinline__ void bt_householder(const double* As, int s, int n, d
 }
 
 template <typename T, int PREC, int NB>
-__global__ void __launch_bounds__(BT_NT)
+__global__ void __launch_bounds__(BT_NT, NB == 2 ? 2 : 1)
 mrcqr_factor_batched_kernel(const BatchParams p)
 {
     extern __shared__ __align__(16) unsigned char bsm[];
@@ -176,7 +176,7 @@ mrcqr_factor_batched_kernel(const BatchParams p)
     const int nrg = BT_NW / nbp;                                         // row groups
     const int bw = warp % nbp, rgi = warp / nbp;
     const int bin = 32 * bw + lane;
-    const int TR = p.tr, rows_w = TR / nrg;                              // rows of a tile per row group
+    const int TR = p.tr, TSH = p.tr_sh, rows_w = TR / nrg;               // rows of a tile per row group
     const int ntile = (int)(m / TR);
 
     for (int b = blockIdx.x; b < p.batch; b += gridDim.x) {
@@ -223,12 +223,12 @@ mrcqr_factor_batched_kernel(const BatchParams p)
                 if (p.vec) {
                     const int H = TR / 2;
                     for (int e = tid; e < n * H; e += BT_NT) {
-                        const int j = e / H, r2 = (e % H) * 2;
+                        const int j = e >> (TSH - 1), r2 = (e & (H - 1)) * 2;
                         cp_async16(dst + j * RLD + r2, A + (size_t)j * (size_t)p.lda + t0 + r2, 16);
                     }
                 } else {
                     for (int e = tid; e < n * TR; e += BT_NT) {
-                        const int j = e / TR, r = e % TR;
+                        const int j = e >> TSH, r = e & (TR - 1);
                         dst[j * RLD + r] = A[(size_t)j * (size_t)p.lda + t0 + r];
                     }
                 }
@@ -237,12 +237,17 @@ mrcqr_factor_batched_kernel(const BatchParams p)
             const bool live = bin < s;
             const int64_t k = live ? idx[bin] : 0;
             Cx2<T> d1, d8;
+            Cx2<double> wt, dt;                                             // W_m^{k (t0 + r0)} of the current tile and its step W_m^{k TR}, in double
             {
                 double sn, cs;
                 sincospi(2.0 * (double)(k & (m - 1)) / (double)m, &sn, &cs);
                 d1 = Cx2<T>{(T)cs, (T)sn};
                 sincospi(2.0 * (double)((8 * k) & (m - 1)) / (double)m, &sn, &cs);
                 d8 = Cx2<T>{(T)cs, (T)sn};
+                sincospi(2.0 * (double)((k * (int64_t)(rgi * rows_w)) & (m - 1)) / (double)m, &sn, &cs);
+                wt = Cx2<double>{cs, sn};
+                sincospi(2.0 * (double)((k * (int64_t)TR) & (m - 1)) / (double)m, &sn, &cs);
+                dt = Cx2<double>{cs, sn};
             }
             T acc[N16];
 #pragma unroll
@@ -261,7 +266,7 @@ mrcqr_factor_batched_kernel(const BatchParams p)
                 {                                                           // DiagMult + cast, once per element
                     const double* src = raw + (size_t)(tl & 1) * N16 * RLD;
                     for (int e = tid; e < n * TR; e += BT_NT) {
-                        const int j = e / TR, r = e % TR;
+                        const int j = e >> TSH, r = e & (TR - 1);
                         const unsigned neg = (sgn[r >> 5] >> (r & 31)) & 1u;
                         tt[r * TLD + j] = bt_diag_cast<T, PREC>(src[j * RLD + r], neg);
                     }
@@ -269,12 +274,8 @@ mrcqr_factor_batched_kernel(const BatchParams p)
                 __syncthreads();
                 if (live) {
                     const int r0 = rgi * rows_w;
-                    Cx2<T> w0;
-                    {
-                        double sn, cs;
-                        sincospi(2.0 * (double)((k * (t0 + r0)) & (m - 1)) / (double)m, &sn, &cs);
-                        w0 = Cx2<T>{(T)cs, (T)sn};
-                    }
+                    Cx2<T> w0{(T)wt.x, (T)wt.y};                            // one double rotation per tile instead of a sincospi
+                    wt = cmul2(wt, dt);
                     Cx2<T> w = w0;
                     for (int r = 0; r < rows_w; ++r) {
                         if ((r & 7) == 0 && r > 0) { w0 = cmul2(w0, d8); w = w0; }
@@ -452,6 +453,7 @@ int launch_factor_batched(int batch, int64_t m, int n, int64_t lda, int64_t stri
     p.m = m; p.lda = lda; p.strideA = strideA; p.ldq = ldq; p.strideQ = strideQ; p.seed = seed;
     p.A = A; p.Q = Q; p.R = R; p.codes = codes_dev;
     p.tr = m >= BT_TR ? BT_TR : (int)m;
+    p.tr_sh = 0; while ((1 << p.tr_sh) < p.tr) ++p.tr_sh;
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0) && (strideA % 2 == 0) &&
             ((uintptr_t)Q % 16 == 0) && (ldq % 2 == 0) && (strideQ % 2 == 0);
     p = batched_layout(p, prec == 64 ? 8 : 4);
