@@ -308,24 +308,25 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
     const int tile_hi = min(p.tiles_per_col, tile_lo + p.tiles_per_chunk);
     double2 v[16];
     unsigned sw = 0;                                                                // sign word of row a = lane % 16 (this half warp's b)
-    auto fetch = [&](int tl) {
+    // rows a = A0 .. A0+7 of tile tl (the request is split in two so that at most 8 rows are in flight beside a butterfly)
+    auto fetch = [&](int tl, int A0) {
         const int64_t t2_0 = (int64_t)tl * (2 * F16_W);
         if (p.vec) {
             const double2* src = reinterpret_cast<const double2*>(colA + t2_0) + u;
             const int64_t m2h = p.m2 >> 1;
 #pragma unroll
-            for (int a = 0; a < 16; ++a) v[a] = __ldcs(src + (int64_t)(16 * a + b) * m2h);
+            for (int a = 0; a < 8; ++a) v[A0 + a] = __ldcs(src + (int64_t)(16 * (A0 + a) + b) * m2h);
         } else {
             const double* src = colA + t2_0 + 2 * u;
 #pragma unroll
-            for (int a = 0; a < 16; ++a) {
-                const int64_t off = (int64_t)(16 * a + b) * p.m2;
-                v[a] = make_double2(__ldcs(src + off), __ldcs(src + off + 1));
+            for (int a = 0; a < 8; ++a) {
+                const int64_t off = (int64_t)(16 * (A0 + a) + b) * p.m2;
+                v[A0 + a] = make_double2(__ldcs(src + off), __ldcs(src + off + 1));
             }
         }
-        sw = __ldg(signs32 + (((int64_t)(16 * (lane & 15) + b) * p.m2 + t2_0) >> 5));   // m2 % 32 == 0: one word per row and tile
+        if (A0 == 0) sw = __ldg(signs32 + (((int64_t)(16 * (lane & 15) + b) * p.m2 + t2_0) >> 5));   // m2 % 32 == 0: one word per row and tile
     };
-    if (tile_lo < tile_hi) fetch(tile_lo);
+    if (tile_lo < tile_hi) { fetch(tile_lo, 0); fetch(tile_lo, 8); }
     for (int tl = tile_lo; tl < tile_hi; ++tl) {
         const int64_t t2_0 = (int64_t)tl * (2 * F16_W);
         Cx<T> x[16];
@@ -334,7 +335,7 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
             const unsigned bits = __shfl_sync(0xffffffffu, sw, (lane & 16) + a) >> (2 * u);
             x[a] = Cx<T>{diag_cast<T, PREC>(v[a].x, bits & 1u), diag_cast<T, PREC>(v[a].y, (bits >> 1) & 1u)};
         }
-        if (tl + 1 < tile_hi) fetch(tl + 1);                                        // in flight during both passes and stage 2
+        if (tl + 1 < tile_hi) fetch(tl + 1, 0);                                     // first half of the next tile: in flight from here on
         fft16(x);
         __syncthreads();                                                            // stage 2 of the previous tile has read the tile
 #pragma unroll
@@ -349,35 +350,37 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
         fft16(x);
 #pragma unroll
         for (int kb = 0; kb < 16; ++kb) st_tile(tile + (size_t)(16 * b + kb) * F16_LD + u, x[f16pos(kb)]);
+        if (tl + 1 < tile_hi) fetch(tl + 1, 8);                                     // second half: the butterfly registers are free now
         __syncthreads();
-        // ---- stage 2: thread = bin; Z[k1] sits in row 16 (k1 & 15) + (k1 >> 4)
+        // ---- stage 2: thread = bin; Z[k1] sits in row 16 (k1 & 15) + (k1 >> 4).  With P = Z[k1], Qn = Z[m1 - k1], q = conj(d2),
+        //      d1 = W_m^{-k} conjugated (cos, sin of 2 pi k / m), d2 = d1^2 and w0 the twiddle of the tile's first t2:
+        //        sum_u Re(conj(w_2u) E_u + conj(w_2u+1) O_u) = Re( conj(w0) (SE + conj(d1) SO) ),
+        //        SE = (SP + conj(SQ)) / 2,  SO = -i (SP - conj(SQ)) / 2,  SP = sum_u q^u P_u,  SQ = sum_u d2^u Qn_u,
+        //      so the tile costs two Horner recurrences (4 fma per step each) instead of two twiddle recurrences and 8 more
+        //      operations per step; the recurrences run over 16 steps: a few ulp in T.
         for (int i = tid; i < p.s; i += F16_NT) {
             const int64_t k = idx[i];
             const int k1 = (int)(k & (F16_M1 - 1));
             const int k1n = (F16_M1 - k1) & (F16_M1 - 1);
             const ST* rowP = tile + (size_t)(16 * (k1 & 15) + (k1 >> 4)) * F16_LD;
             const ST* rowQ = tile + (size_t)(16 * (k1n & 15) + (k1n >> 4)) * F16_LD;
-            Cx<T> w0, d1, d2, d16;
+            Cx<T> w0, d1, d2;
             sincospi_t((T)(2.0 * (double)((k * t2_0) & (p.m - 1)) / (double)p.m), &w0.y, &w0.x);
-            if (p.dtab) d1 = dstep[i];
-            else sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d1.y, &d1.x);
+            d1 = dstep[i];
             d2 = cmul(d1, d1);
-            d16 = cmul(d2, d2); d16 = cmul(d16, d16); d16 = cmul(d16, d16);
-            T va = (T)0;
+            Cx<T> sp = ld_tile(rowP + F16_W - 1), sq = ld_tile(rowQ + F16_W - 1);
 #pragma unroll
-            for (int j8 = 0; j8 < F16_W; j8 += 8) {
-                Cx<T> we = w0;
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    const Cx<T> P = ld_tile(rowP + j8 + q), Qn = ld_tile(rowQ + j8 + q);
-                    const Cx<T> wo = cmul(we, d1);
-                    va = fma(we.x, P.x + Qn.x, va); va = fma(we.y, P.y - Qn.y, va);
-                    va = fma(wo.x, P.y + Qn.y, va); va = fma(wo.y, Qn.x - P.x, va);
-                    we = cmul(we, d2);
-                }
-                w0 = cmul(w0, d16);
+            for (int q = F16_W - 2; q >= 0; --q) {
+                const Cx<T> P = ld_tile(rowP + q), Qn = ld_tile(rowQ + q);
+                // sp <- sp * conj(d2) + P ;  sq <- sq * d2 + Qn
+                const Cx<T> spn{fma(sp.x, d2.x, fma(sp.y, d2.y, P.x)), fma(sp.y, d2.x, fma(-sp.x, d2.y, P.y))};
+                const Cx<T> sqn{fma(sq.x, d2.x, fma(-sq.y, d2.y, Qn.x)), fma(sq.y, d2.x, fma(sq.x, d2.y, Qn.y))};
+                sp = spn; sq = sqn;
             }
-            colacc[i] += 0.5 * (double)va;
+            // 2 SE = sp + conj(sq), 2 SO = -i (sp - conj(sq));  z = 2 (SE + conj(d1) SO);  result = Re(conj(w0) z) / 2
+            const Cx<T> se{sp.x + sq.x, sp.y - sq.y}, so{sp.y + sq.y, sq.x - sp.x};
+            const Cx<T> z{se.x + fma(d1.x, so.x, d1.y * so.y), se.y + fma(d1.x, so.y, -(d1.y * so.x))};
+            colacc[i] += 0.5 * (double)fma(w0.x, z.x, w0.y * z.y);
         }
     }
     __syncthreads();
