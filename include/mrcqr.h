@@ -10,9 +10,15 @@
  *              (G is written full symmetric).
  *   Pointers   DEVICE pointers unless the argument name ends in _host.  The caller owns every
  *              buffer it passes; A is never modified; Q must not overlap A.
- *   Workspace  the library owns one grow-only device workspace (sketch partials, A_s, R_s, Gram
- *              partials, status word), allocated on first use, freed by mrcqr_shutdown().
- *              Not thread-safe: one call at a time per process.
+ *   Workspace  every CONTEXT owns one grow-only device workspace (sketch partials, A_s, R_s, Gram
+ *              partials, status word), its staging buffers, its switches (mrcqr_set_*), its status
+ *              (mrcqr_last_*) and its graph cache, allocated on first use, freed by mrcqr_shutdown().
+ *              All entry points act on the calling thread's CURRENT context: the process default
+ *              one, or a handle made current by mrcqr_set_current (mrcqr_create / mrcqr_destroy).
+ *              One call at a time per context; host threads with a context and a stream each may
+ *              call concurrently (the library orders, on the device, the one stretch of a
+ *              factorization that uses a device-wide resource, the constant-bank coefficients of
+ *              the row kernels; sketches and batched calls overlap freely).
  *   stream     a cudaStream_t passed as void* (NULL = default stream).  Kernels are enqueued on
  *              it; the call then reads back an 8-byte status word and synchronises the stream, so
  *              the return value is final when the call returns.
@@ -30,6 +36,16 @@
 #ifdef __cplusplus
 extern "C" {
 #endif
+
+/*
+ * Contexts.  mrcqr_create makes a new context (nothing is allocated until its first use), mrcqr_set_current makes it the
+ * calling thread's current one (NULL: back to the process default context), mrcqr_destroy frees everything it owns (it
+ * must not be current in another thread, nor in use).  Return 0, or -1 for a null argument.
+ */
+typedef struct mrcqr_handle_s* mrcqr_handle_t;
+int mrcqr_create(mrcqr_handle_t* handle);
+int mrcqr_set_current(mrcqr_handle_t handle);
+int mrcqr_destroy(mrcqr_handle_t handle);
 
 /* sketch precision p of Algorithm 2: half, single, double */
 typedef enum { MRCQR_FP16 = 16, MRCQR_FP32 = 32, MRCQR_FP64 = 64 } mrcqr_prec_t;
@@ -238,7 +254,7 @@ int mrcqr_last_used_graph(void);
 int mrcqr_debug_dump_y(int64_t m, int n, int64_t lda, const double* A, const double* Rs,
                        double* Y_stage2a, double* Y_stage2b, void* stream);
 
-/* Frees the workspace (and the host-path device buffers). */
+/* Frees everything the current context owns (workspace, staging buffers, graph); the context stays usable. */
 void mrcqr_shutdown(void);
 
 #ifdef __cplusplus

@@ -39,6 +39,9 @@ def lib():
         L = C.CDLL(path)
         i64, u64, vp, ci = C.c_int64, C.c_uint64, C.c_void_p, C.c_int
         L.mrcqr_draw.argtypes = [i64, ci, u64, vp, vp]
+        L.mrcqr_create.argtypes = [vp]
+        L.mrcqr_set_current.argtypes = [vp]
+        L.mrcqr_destroy.argtypes = [vp]
         L.mrcqr_draw_device.argtypes = [i64, ci, u64, vp, vp, vp]
         L.mrcqr_sketch.argtypes = [i64, ci, i64, vp, ci, ci, vp, vp, vp, vp, vp]
         L.mrcqr_precondition_gram.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
@@ -59,7 +62,7 @@ def lib():
         L.mrcqr_set_sketch_reim.argtypes = [ci]
         L.mrcqr_set_graph.argtypes = [ci]
         L.mrcqr_last_timing.argtypes = [vp]
-        for f in ("mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
+        for f in ("mrcqr_create", "mrcqr_set_current", "mrcqr_destroy", "mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
                   "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
                   "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"):
             getattr(L, f).restype = ci
@@ -67,7 +70,7 @@ def lib():
     return _lib
 
 
-EXPORTS = ["mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
+EXPORTS = ["mrcqr_create", "mrcqr_set_current", "mrcqr_destroy", "mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
            "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"]
 
@@ -89,6 +92,24 @@ def _mat(AT):
     assert AT.is_cuda and AT.dtype == torch.float64 and AT.dim() == 2 and AT.stride(1) == 1
     n, m = AT.shape
     return m, n, AT.stride(0), AT.data_ptr()
+
+
+def mrcqr_create():
+    """A new context (own workspace, switches, status); make it the calling thread's with mrcqr_set_current."""
+    h = C.c_void_p(None)
+    rc = lib().mrcqr_create(C.byref(h))
+    if rc != 0:
+        raise MrcqrError(rc)
+    return h
+
+
+def mrcqr_set_current(handle):
+    """handle from mrcqr_create, or None for the process default context."""
+    lib().mrcqr_set_current(handle)
+
+
+def mrcqr_destroy(handle):
+    lib().mrcqr_destroy(handle)
 
 
 def mrcqr_draw(m, s, seed):

@@ -3,6 +3,7 @@
 #include "../../include/mrcqr.h"
 #include "mrcqr_internal.cuh"
 #include <algorithm>
+#include <mutex>
 #include <cstring>
 #include <vector>
 
@@ -88,7 +89,45 @@ struct Ctx {
     cudaGraphExec_t gexec = nullptr; int glaunches = 0; uint64_t* h_seed = nullptr;
     struct { int64_t m, lda; int n, prec, s; const void *A, *Q, *R, *ws, *hidx; bool store_y, reim; } gkey = {};
 };
-static Ctx g;
+// Every entry point works on the calling thread's CURRENT context: the process default one, or the handle made current
+// with mrcqr_set_current (mrcqr_create / mrcqr_destroy).  A context owns its workspace, staging buffers, settings,
+// status and graph cache, so two host threads with a handle and a stream each may factor at the same time.
+static Ctx g_default;
+static thread_local Ctx* t_current = nullptr;
+static inline Ctx& ctx() { return t_current ? *t_current : g_default; }
+#define g (ctx())
+
+// The diagonal-block coefficients of the row kernels are constant-bank operands (rows.cuh: c_diag, c_pdiag), a device-wide
+// resource: the stretch "upload the prepared diagonal blocks ... last kernel that reads them" of one factorization must not
+// interleave with another context's.  The gate orders such stretches ON THE DEVICE (a stream waits for the event the
+// previous stretch recorded) and on the host (a mutex held while the stretch is enqueued); everything before it (K1, K2)
+// and the batched kernel (coefficients in shared memory) overlap freely.
+struct ConstGate {
+    std::recursive_mutex mu;                 // recursive: a call that spans two stretches (the debug dump) nests them
+    cudaEvent_t ev = nullptr;
+    bool pending = false;
+    void acquire(cudaStream_t st)
+    {
+        mu.lock();
+        if (!ev) cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        cudaStreamIsCapturing(st, &cs);
+        if (pending && cs == cudaStreamCaptureStatusNone) cudaStreamWaitEvent(st, ev, 0);
+    }
+    void release(cudaStream_t st)
+    {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        cudaStreamIsCapturing(st, &cs);
+        if (cs == cudaStreamCaptureStatusNone) { cudaEventRecord(ev, st); pending = true; }
+        mu.unlock();
+    }
+};
+static ConstGate g_gate;
+struct GateScope {
+    cudaStream_t st;
+    explicit GateScope(cudaStream_t s) : st(s) { g_gate.acquire(st); }
+    ~GateScope() { g_gate.release(st); }
+};
 
 static void drop_graph()
 {
@@ -166,6 +205,7 @@ static int enqueue_gram(const Layout& L, int64_t m, int n, int64_t lda, const do
     double* G16 = reinterpret_cast<double*>(g.ws + L.G16);
     double* part = reinterpret_cast<double*>(g.ws + L.k3);
     int np = 0;
+    GateScope gate(st);
     int k = launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st);
     k += upload_diag(RsPrep, n16, 0, st);
     k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, Ydump, nullptr, 0, st);
@@ -184,6 +224,7 @@ static int enqueue_formq(const Layout& L, int64_t m, int n, int64_t lda, const d
     double* RsPrep = reinterpret_cast<double*>(g.ws + L.RsPrep);
     double* RcPrep = reinterpret_cast<double*>(g.ws + L.RcPrep);
     int k = 0;
+    GateScope gate(st);
     if (prep_rs) { k += launch_prep_R(Rs, n, RsPrep, n16, stat, MRCQR_ERR_SINGULAR, st); k += upload_diag(RsPrep, n16, 0, st); }
     if (prep_rc) { k += launch_prep_R(Rc, n, RcPrep, n16, stat, MRCQR_ERR_BREAKDOWN, st); k += upload_diag(RcPrep, n16, 1, st); }
     k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, Ydump, 3, st);
@@ -242,23 +283,48 @@ extern "C" int mrcqr_last_info(void) { return g.last_info; }
 extern "C" int mrcqr_last_launch_count(void) { return g.last_launches; }
 extern "C" int mrcqr_last_used_graph(void) { return g.last_graph ? 1 : 0; }
 
-extern "C" void mrcqr_shutdown(void)
+static void free_ctx(Ctx& c)
 {
-    if (!g.probed || !g.have_device) return;
+    if (!c.probed || !c.have_device) { c = Ctx(); return; }
     cudaDeviceSynchronize();
-    drop_graph();
-    if (g.h_seed) cudaFreeHost(g.h_seed);
-    if (g.ws) cudaFree(g.ws);
-    if (g.h_status) cudaFreeHost(g.h_status);
-    if (g.h_idx) cudaFreeHost(g.h_idx);
-    if (g.ev_ok) for (int i = 0; i < 8; ++i) cudaEventDestroy(g.ev[i]);
-    if (g.hA) cudaFree(g.hA);
-    if (g.hQ) cudaFree(g.hQ);
-    if (g.hR) cudaFree(g.hR);
-    if (g.host_stream) cudaStreamDestroy(g.host_stream);
-    if (g.bcodes) cudaFree(g.bcodes);
-    if (g.h_bcodes) cudaFreeHost(g.h_bcodes);
-    g = Ctx();
+    if (c.gexec) { cudaGraphExecDestroy(c.gexec); c.gexec = nullptr; }
+    if (c.h_seed) cudaFreeHost(c.h_seed);
+    if (c.ws) cudaFree(c.ws);
+    if (c.h_status) cudaFreeHost(c.h_status);
+    if (c.h_idx) cudaFreeHost(c.h_idx);
+    if (c.ev_ok) for (int i = 0; i < 8; ++i) cudaEventDestroy(c.ev[i]);
+    if (c.hA) cudaFree(c.hA);
+    if (c.hQ) cudaFree(c.hQ);
+    if (c.hR) cudaFree(c.hR);
+    if (c.host_stream) cudaStreamDestroy(c.host_stream);
+    if (c.bcodes) cudaFree(c.bcodes);
+    if (c.h_bcodes) cudaFreeHost(c.h_bcodes);
+    c = Ctx();
+}
+
+extern "C" void mrcqr_shutdown(void) { free_ctx(ctx()); }
+
+extern "C" int mrcqr_create(mrcqr_handle_t* handle)
+{
+    if (!handle) return -1;
+    *handle = reinterpret_cast<mrcqr_handle_t>(new Ctx());
+    return 0;
+}
+
+extern "C" int mrcqr_destroy(mrcqr_handle_t handle)
+{
+    if (!handle) return -1;
+    Ctx* c = reinterpret_cast<Ctx*>(handle);
+    if (t_current == c) t_current = nullptr;
+    free_ctx(*c);
+    delete c;
+    return 0;
+}
+
+extern "C" int mrcqr_set_current(mrcqr_handle_t handle)
+{
+    t_current = reinterpret_cast<Ctx*>(handle);       // NULL: the process default context
+    return 0;
 }
 
 extern "C" int mrcqr_sketch(int64_t m, int n, int64_t lda, const double* A, mrcqr_prec_t prec, int s,
@@ -335,6 +401,7 @@ extern "C" int mrcqr_debug_dump_y(int64_t m, int n, int64_t lda, const double* A
     cudaStream_t st = (cudaStream_t)stream;
     mrcqr_reset_status<<<1, 1, 0, st>>>(reinterpret_cast<Status*>(g.ws + L.status));
     double* Rc = reinterpret_cast<double*>(g.ws + L.Rc);
+    GateScope gate(st);                              // stage 2b below reuses the coefficients stage 2a uploaded
     int k = 1 + enqueue_gram(L, m, n, lda, A, Rs, nullptr, Rc, Y_stage2a, st);
     k += enqueue_formq(L, m, n, lda, A, Rs, Rc, false, false, m, nullptr, nullptr, Y_stage2b, st);   // Q = nullptr: not stored
     int rc = finish(L, st, k);
@@ -377,6 +444,7 @@ static int enqueue_stage23(const Layout& L, int64_t m, int n, int64_t lda, const
         double* G16 = reinterpret_cast<double*>(g.ws + L.G16);
         double* part = reinterpret_cast<double*>(g.ws + L.k3);
         int np = 0;
+        GateScope gate(st);
         k += upload_diag(RsPrep, n16, 0, st);
         if (tm) cudaEventRecord(g.ev[3], st);
         const bool store_y = n16 > 128;          // Gram of a stored Y (k3_syrk.cu): Y = A Rs^-1 lives in the Q buffer
@@ -464,8 +532,9 @@ static int factor_device(int64_t m, int n, int64_t lda, const double* A, int64_t
             *g.h_seed = seed;
             g.last_launches = g.glaunches;
             g.last_graph = true;
-            if (cudaGraphLaunch(g.gexec, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess ||
-                cudaGetLastError() != cudaSuccess) return MRCQR_ERR_CUDA;
+            cudaError_t le;
+            { GateScope gate(st); le = cudaGraphLaunch(g.gexec, st); }
+            if (le != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) return MRCQR_ERR_CUDA;
             g.last_info = g.h_status[1];
             return g.h_status[0];
         }

@@ -422,3 +422,50 @@ def test_batched_writes_stay_inside(orc):
     QB, RB, codes = B.mrcqr_factor_batched(AB, 64, s, 1, qflat.view(batch, n, m), rflat.view(batch, n, n))
     assert codes == [0] * batch
     assert _margins_intact(qbuf, batch * n * m) and _margins_intact(rbuf, batch * n * n) and torch.equal(abuf, a_before)
+
+
+def test_two_contexts_factor_concurrently(orc):
+    """mrcqr_create / mrcqr_set_current: two host threads, each with a context and a stream of its own, factor different
+    matrices at the same time (ctypes drops the GIL during the calls), interleaving the small-n kernels, the panel passes
+    and batched calls.  Every result is bit for bit the one a lone call gives: the contexts share nothing but the
+    constant-bank gate, which orders their coefficient uploads on the device."""
+    import threading
+    jobs = [(1 << 14, 64, 16), (1 << 12, 200, 64), (1 << 13, 24, 32), (1 << 12, 136, 32)]
+    mats = [inputs.make_A(m, n, 3, 70 + n, 71 + n, "cuda") for (m, n, _) in jobs]
+    ref = [B.mrcqr_factor(A, p, 2 * n, 5) for A, (m, n, p) in zip(mats, jobs)]
+    AB = torch.stack([inputs.make_A(1024, 12, 2, 90 + b, 91 + b, "cuda") for b in range(6)])
+    QBr, RBr, _ = B.mrcqr_factor_batched(AB, 64, 30, 1)
+    torch.cuda.synchronize()
+    errors = []
+
+    def worker(tix):
+        try:
+            h = B.mrcqr_create()
+            B.mrcqr_set_current(h)
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                for it in range(12):
+                    j = (2 * it + tix) % len(jobs)
+                    m, n, p = jobs[j]
+                    Q, R = B.mrcqr_factor(mats[j], p, 2 * n, 5, stream=st)
+                    if not (torch.equal(Q, ref[j][0]) and torch.equal(R, ref[j][1])):
+                        errors.append(("factor", tix, it, j))
+                    if it % 4 == tix:
+                        QB, RB, codes = B.mrcqr_factor_batched(AB, 64, 30, 1, stream=st)
+                        if not (torch.equal(QB, QBr) and torch.equal(RB, RBr)):
+                            errors.append(("batched", tix, it))
+                st.synchronize()
+            B.mrcqr_set_current(None)
+            B.mrcqr_destroy(h)
+        except Exception as e:                                   # noqa: BLE001
+            errors.append(("exception", tix, repr(e)))
+
+    threads = [threading.Thread(target=worker, args=(t,)) for t in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert errors == []
+    # the default context is untouched and still works
+    Q, R = B.mrcqr_factor(mats[0], jobs[0][2], 2 * jobs[0][1], 5)
+    assert torch.equal(Q, ref[0][0])
