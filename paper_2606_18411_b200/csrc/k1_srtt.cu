@@ -276,7 +276,7 @@ __device__ __forceinline__ Cx<float> ld_tile(const __half2* p) { const float2 f 
 constexpr int F16_W = 16, F16_NT = 256, F16_M1 = 256, F16_LD = F16_W + 1;
 
 template <typename T, typename ST, int PREC>
-__global__ void __launch_bounds__(F16_NT, sizeof(T) == 8 ? 1 : 2)
+__global__ void __launch_bounds__(F16_NT, 2)
 mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
                const int64_t* __restrict__ idx, double* __restrict__ partial)
 {
@@ -284,7 +284,9 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
     ST* tile = reinterpret_cast<ST*>(smraw);                                        // [256][17]
     Cx<T>* tw = reinterpret_cast<Cx<T>*>(smraw + (size_t)F16_M1 * F16_LD * sizeof(ST));   // [256]  W_256^e
     double* colacc = reinterpret_cast<double*>(tw + F16_M1);                        // [s]
-    Cx<T>* dstep = reinterpret_cast<Cx<T>*>(colacc + p.s);                          // [s]  (dtab only)
+    Cx<T>* dstep = reinterpret_cast<Cx<T>*>(colacc + p.s);                          // [s]  (cos, sin) of 2 pi k_i / m
+    unsigned short* perm = reinterpret_cast<unsigned short*>(dstep + p.s);          // [s]  stage-2 order of the bins
+    __shared__ int bucket[32];
     const int tid = threadIdx.x, lane = tid & 31;
     const int u = tid & (F16_W - 1), b = tid >> 4;                                  // pass 1: b = t1 mod 16; pass 2: b = ka
     const int col = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
@@ -296,13 +298,42 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
         tw[e] = Cx<T>{(T)cs, (T)sn};
     }
     for (int e = tid; e < p.s; e += F16_NT) colacc[e] = 0.0;
-    if (p.dtab)
-        for (int i = tid; i < p.s; i += F16_NT) {
-            const int64_t k = idx[i];
-            Cx<T> d;
-            sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d.y, &d.x);
-            dstep[i] = d;
+    for (int i = tid; i < p.s; i += F16_NT) {
+        const int64_t k = idx[i];
+        Cx<T> d;
+        sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d.y, &d.x);
+        dstep[i] = d;
+    }
+    // Stage 2 reads, per lane, one element of the tile row of its bin: 32 lanes, 32 unrelated rows.  The rows of the lanes
+    // that share a shared-memory wavefront (G = 128 bytes / element size: 8, 16 or 32 lanes) should fall into G different
+    // banks, i.e. differ in (row mod G).  The bins are therefore dealt to the threads bucket by bucket: bin i of bucket
+    // key_i = row_i mod G and rank r inside its bucket goes to position  sum_b min(count_b, r) + #{b < key_i : count_b > r},
+    // which walks the buckets round-robin.  Which thread owns a bin does not change the bin's arithmetic.
+    if (p.s <= 128) {                                                              // stage 2 is a small part there: identity order
+        for (int i = tid; i < p.s; i += F16_NT) perm[i] = (unsigned short)i;
+    } else {
+        constexpr int G = 128 / (int)sizeof(ST);
+        if (tid < 32) bucket[tid] = 0;
+        __syncthreads();
+        int myrank[16];                                                            // s <= 4096: at most 16 bins per thread here
+        int cnt = 0;
+        for (int i = tid; i < p.s; i += F16_NT, ++cnt) {
+            const int k1 = (int)(idx[i] & (F16_M1 - 1));
+            const int key = (16 * (k1 & 15) + (k1 >> 4)) & (G - 1);
+            myrank[cnt & 15] = atomicAdd(&bucket[key], 1);
         }
+        __syncthreads();
+        cnt = 0;
+        for (int i = tid; i < p.s; i += F16_NT, ++cnt) {
+            const int k1 = (int)(idx[i] & (F16_M1 - 1));
+            const int key = (16 * (k1 & 15) + (k1 >> 4)) & (G - 1);
+            const int r = myrank[cnt & 15];
+            int pos = 0;
+#pragma unroll
+            for (int q = 0; q < G; ++q) pos += min(bucket[q], r) + ((q < key && bucket[q] > r) ? 1 : 0);
+            perm[pos] = (unsigned short)i;
+        }
+    }
 
     const int tile_lo = chunk * p.tiles_per_chunk;
     const int tile_hi = min(p.tiles_per_col, tile_lo + p.tiles_per_chunk);
@@ -358,7 +389,8 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
         //        SE = (SP + conj(SQ)) / 2,  SO = -i (SP - conj(SQ)) / 2,  SP = sum_u q^u P_u,  SQ = sum_u d2^u Qn_u,
         //      so the tile costs two Horner recurrences (4 fma per step each) instead of two twiddle recurrences and 8 more
         //      operations per step; the recurrences run over 16 steps: a few ulp in T.
-        for (int i = tid; i < p.s; i += F16_NT) {
+        for (int ps = tid; ps < p.s; ps += F16_NT) {
+            const int i = perm[ps];
             const int64_t k = idx[i];
             const int k1 = (int)(k & (F16_M1 - 1));
             const int k1n = (F16_M1 - k1) & (F16_M1 - 1);
@@ -474,7 +506,7 @@ static void k1_launch_fft16(const K1Params& p_in, const double* A, const uint64_
     K1Params p = p_in;
     size_t smem = (size_t)F16_M1 * F16_LD * sizeof(ST) + (size_t)F16_M1 * sizeof(Cx<T>) + (size_t)p.s * sizeof(double);
     p.dtab = 1;
-    smem += (size_t)p.s * sizeof(Cx<T>);
+    smem += (size_t)p.s * sizeof(Cx<T>) + (size_t)((p.s + 7) & ~7) * sizeof(unsigned short);
     auto k = mrcqr_k1_fft16<T, ST, PREC>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k<<<p.n * p.chunks, F16_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
