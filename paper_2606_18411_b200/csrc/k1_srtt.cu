@@ -274,9 +274,12 @@ template <typename T> __device__ __forceinline__ Cx<T> ld_tile(const Cx<T>* p) {
 __device__ __forceinline__ Cx<float> ld_tile(const __half2* p) { const float2 f = __half22float2(*p); return Cx<float>{f.x, f.y}; }
 
 constexpr int F16_W = 16, F16_NT = 256, F16_M1 = 256, F16_LD = F16_W + 1;
+#ifndef F16_DBL_CTAS
+#define F16_DBL_CTAS 2
+#endif
 
 template <typename T, typename ST, int PREC>
-__global__ void __launch_bounds__(F16_NT, 2)
+__global__ void __launch_bounds__(F16_NT, sizeof(T) == 8 ? F16_DBL_CTAS : 2)
 mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
                const int64_t* __restrict__ idx, double* __restrict__ partial)
 {
@@ -285,7 +288,8 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
     Cx<T>* tw = reinterpret_cast<Cx<T>*>(smraw + (size_t)F16_M1 * F16_LD * sizeof(ST));   // [256]  W_256^e
     double* colacc = reinterpret_cast<double*>(tw + F16_M1);                        // [s]
     Cx<T>* dstep = reinterpret_cast<Cx<T>*>(colacc + p.s);                          // [s]  (cos, sin) of 2 pi k_i / m
-    unsigned short* perm = reinterpret_cast<unsigned short*>(dstep + p.s);          // [s]  stage-2 order of the bins
+    int* kbin = reinterpret_cast<int*>(dstep + p.s);                                // [s]  the bins k_i (< 2^31: m <= 2^31 here)
+    unsigned short* perm = reinterpret_cast<unsigned short*>(kbin + p.s);           // [s]  stage-2 order of the bins
     __shared__ int bucket[32];
     const int tid = threadIdx.x, lane = tid & 31;
     const int u = tid & (F16_W - 1), b = tid >> 4;                                  // pass 1: b = t1 mod 16; pass 2: b = ka
@@ -303,6 +307,7 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
         Cx<T> d;
         sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d.y, &d.x);
         dstep[i] = d;
+        kbin[i] = (int)k;
     }
     // Stage 2 reads, per lane, one element of the tile row of its bin: 32 lanes, 32 unrelated rows.  The rows of the lanes
     // that share a shared-memory wavefront (G = 128 bytes / element size: 8, 16 or 32 lanes) should fall into G different
@@ -391,7 +396,7 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
         //      operations per step; the recurrences run over 16 steps: a few ulp in T.
         for (int ps = tid; ps < p.s; ps += F16_NT) {
             const int i = perm[ps];
-            const int64_t k = idx[i];
+            const int64_t k = kbin[i];
             const int k1 = (int)(k & (F16_M1 - 1));
             const int k1n = (F16_M1 - k1) & (F16_M1 - 1);
             const ST* rowP = tile + (size_t)(16 * (k1 & 15) + (k1 >> 4)) * F16_LD;
@@ -450,7 +455,8 @@ static int k1_tile_w(int64_t m, int prec, int s, int reim)
     return w;
 }
 
-static bool k1_fft16_usable(int64_t m, int reim) { return !reim && m >= (int64_t)F16_M1 * 2 * F16_W; }   // m2 >= 32: whole sign words
+// m2 >= 32: whole sign words per tile row; bins kept as 32-bit integers in shared memory
+static bool k1_fft16_usable(int64_t m, int reim) { return !reim && m >= (int64_t)F16_M1 * 2 * F16_W && m <= ((int64_t)1 << 31); }
 
 static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec, int reim)
 {
@@ -506,7 +512,7 @@ static void k1_launch_fft16(const K1Params& p_in, const double* A, const uint64_
     K1Params p = p_in;
     size_t smem = (size_t)F16_M1 * F16_LD * sizeof(ST) + (size_t)F16_M1 * sizeof(Cx<T>) + (size_t)p.s * sizeof(double);
     p.dtab = 1;
-    smem += (size_t)p.s * sizeof(Cx<T>) + (size_t)((p.s + 7) & ~7) * sizeof(unsigned short);
+    smem += (size_t)p.s * (sizeof(Cx<T>) + sizeof(int)) + (size_t)((p.s + 7) & ~7) * sizeof(unsigned short);
     auto k = mrcqr_k1_fft16<T, ST, PREC>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k<<<p.n * p.chunks, F16_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
