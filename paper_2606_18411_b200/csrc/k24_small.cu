@@ -150,6 +150,137 @@ mrcqr_k4_cholesky_sm(const double* __restrict__ G16, int n, int n16, double* __r
     }
 }
 
+// ---- K4, blocked form with the trailing update on DMMA (n16 <= 160) ---------------------------------------
+// Eight pivots per step and three block barriers per step instead of one per pivot:
+//   (1) warp 0 factors the 8x8 diagonal block in registers (lane j owns column j; shuffles; rsqrt_fast pivots),
+//   (2) one thread per trailing column solves its 8 rows against the block, the block's 36 entries in registers first
+//       (the round-1 blocked kernel read them from shared memory inside the dependent chain and lost to the unblocked one),
+//   (3) the rank-8 update G22 -= R12^T R12 runs on the FP64 tensor cores: an 8x8 block of G22 is one accumulator
+//       fragment, R12^T / R12 are the A / B fragments (k = 8: two DMMAs per block), the upper-triangular blocks dealt
+//       round-robin to the 16 warps.
+// W: working copy of G (upper triangle), col-major, ld = n16 + 2 (conflict-free accumulator fragments); Pn: the current
+// 8-row panel, ld = n16 + 4 (conflict-free A / B fragments).  Same epilogue as the unblocked kernel.
+constexpr int K4B_NT = 512;
+
+__global__ void __launch_bounds__(K4B_NT)
+mrcqr_k4_blocked(const double* __restrict__ G16, int n, int n16, double* __restrict__ G_out,
+                 double* __restrict__ Rc, double* __restrict__ RcPrep, const double* __restrict__ Rs,
+                 double* __restrict__ R, Status* st)
+{
+    extern __shared__ __align__(16) double sm[];
+    const int ldw = n16 + 2, pld = n16 + 4;
+    double* W = sm;                              // n16 x ldw
+    double* Pn = W + (size_t)n16 * ldw;          // 8 x pld
+    double* D = Pn + 8 * pld;                    // 8 x 8: D[q * 8 + p] = Rc[k0 + p, k0 + q], p <= q
+    double* dinv = D + 64;                       // 8
+    double* rsd = dinv + 8;                      // n16
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+    for (int e = tid; e < n16 * ldw; e += K4B_NT) {
+        const int i = e % ldw, j = e / ldw;
+        double v = 0.0;
+        if (i < n && j < n) { v = G16[(size_t)j * n16 + i]; if (G_out) G_out[(size_t)j * n + i] = v; }
+        else if (i == j) v = 1.0;                // identity padding: its pivots are harmless
+        W[e] = v;
+    }
+    for (int e = tid; e < 8 * pld; e += K4B_NT) Pn[e] = 0.0;
+    __syncthreads();
+    const int nB = n16 >> 3;
+    for (int k0 = 0; k0 < n; k0 += 8) {
+        const int kb = min(8, n - k0);
+        if (warp == 0) {                         // (1) lane j < 8 owns column k0 + j of the diagonal block
+            const int j = lane;
+            double c[8];
+#pragma unroll
+            for (int p = 0; p < 8; ++p) c[p] = (j < 8 && p <= j) ? W[(k0 + j) * ldw + k0 + p] : 0.0;
+#pragma unroll
+            for (int p = 0; p < 8; ++p) {
+                const double piv = __shfl_sync(0xffffffffu, c[p], p);
+                if (p < kb && j == p && (!(piv > 0.0) || isinf(piv))) report(st, 3, k0 + p);
+                const double ri = rsqrt_fast(piv);
+                const double rp = (j == p) ? piv * ri : c[p] * ri;       // Rc[k0+p, k0+j] for j >= p
+                c[p] = rp;
+                if (j == p) dinv[p] = ri;
+#pragma unroll
+                for (int q = p + 1; q < 8; ++q) {                        // c[q] -= Rc[p, q] * Rc[p, j]  (q <= j)
+                    const double rq = __shfl_sync(0xffffffffu, rp, q);
+                    if (q <= j) c[q] = fma(-rq, rp, c[q]);
+                }
+            }
+#pragma unroll
+            for (int p = 0; p < 8; ++p)
+                if (j < 8) { const double v = (p <= j) ? c[p] : 0.0; D[j * 8 + p] = v; if (p <= j) W[(k0 + j) * ldw + k0 + p] = v; }
+        }
+        __syncthreads();
+        const int t0 = k0 + 8;
+        if (t0 < n16) {
+            if (tid < n16 - t0) {                // (2) row panel: column j = t0 + tid (padding columns give zeros)
+                const int j = t0 + tid;
+                double d[8][8], di[8], x[8];
+#pragma unroll
+                for (int p = 0; p < 8; ++p) {
+                    di[p] = dinv[p];
+#pragma unroll
+                    for (int q = 0; q < p; ++q) d[p][q] = D[p * 8 + q];  // Rc[k0+q, k0+p]
+                }
+#pragma unroll
+                for (int p = 0; p < 8; ++p) x[p] = W[j * ldw + k0 + p];
+#pragma unroll
+                for (int p = 0; p < 8; ++p) {
+                    double acc = x[p];
+#pragma unroll
+                    for (int q = 0; q < p; ++q) acc = fma(-d[p][q], x[q], acc);
+                    x[p] = acc * di[p];
+                }
+#pragma unroll
+                for (int p = 0; p < 8; ++p) { W[j * ldw + k0 + p] = x[p]; Pn[p * pld + j] = x[p]; }
+            }
+            __syncthreads();
+            // (3) trailing update on DMMA: blocks (I, J), t0/8 <= I <= J < nB
+            const int b0 = t0 >> 3, T = nB - b0, nblk = T * (T + 1) / 2;
+            for (int bi = warp; bi < nblk; bi += K4B_NT / 32) {
+                int jj = 0;
+                while ((jj + 1) * (jj + 2) / 2 <= bi) ++jj;
+                const int I = b0 + bi - jj * (jj + 1) / 2, J = b0 + jj;
+                double* cp = W + (size_t)(8 * J + 2 * t) * ldw + 8 * I + g;
+                double c2[2] = {cp[0], cp[ldw]};
+                const double a0 = -Pn[t * pld + 8 * I + g], a1 = -Pn[(t + 4) * pld + 8 * I + g];
+                const double bb0 = Pn[t * pld + 8 * J + g], bb1 = Pn[(t + 4) * pld + 8 * J + g];
+                asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c2[0]), "+d"(c2[1]) : "d"(a0), "d"(bb0));
+                asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c2[0]), "+d"(c2[1]) : "d"(a1), "d"(bb1));
+                cp[0] = c2[0]; cp[ldw] = c2[1];
+            }
+            __syncthreads();
+        }
+    }
+    __syncthreads();
+    // stage Rs in the free strictly-lower triangle, transposed: Rs[k,j] (k < j) at W[k*ldw + j], diag(Rs) in rsd
+    if (R)
+        for (int e = tid; e < n * n; e += K4B_NT) {
+            const int i = e % n, j = e / n;
+            if (i < j) W[i * ldw + j] = Rs[(size_t)j * n + i];
+            else if (i == j) rsd[j] = Rs[(size_t)j * n + i];
+        }
+    __syncthreads();
+    for (int e = tid; e < n * n; e += K4B_NT) {
+        const int i = e % n, j = e / n;
+        double w = 0.0, r = 0.0;
+        if (i <= j) {
+            w = W[j * ldw + i];
+            if (R) {
+                for (int k = i; k < j; ++k) r = fma(W[k * ldw + i], W[k * ldw + j], r);
+                r = fma(w, rsd[j], r);
+            }
+        }
+        Rc[e] = w;
+        if (R) R[e] = r;
+    }
+    {
+        const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
+        int bad = -1;
+        for (size_t o = tid; o < total; o += K4B_NT) RcPrep[o] = prep_value(W, ldw, n, nB, o, &bad);
+    }
+}
+
 // ---- K2 ---------------------------------------------------------------------------------------
 __device__ __forceinline__ double warp_sum(double v)
 {
@@ -335,11 +466,9 @@ int launch_k4_cholesky(const double* G16, int n, int n16, double* G_out, double*
     size_t need = ((size_t)9 * n16 + 2 + (size_t)n16 * (n16 + 1)) * sizeof(double);
     const int use_smem = need <= (size_t)SMALL_SMEM_MAX;
     if (use_smem) {
-        const size_t sm2 = ((size_t)2 * n16 + 2 + (size_t)n16 * (n16 + 1)) * sizeof(double);
-#define K4_GO(JM_) { cudaFuncSetAttribute(mrcqr_k4_cholesky_sm<JM_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2); \
-                     mrcqr_k4_cholesky_sm<JM_><<<1, SMALL_NT, sm2, s>>>(G16, n, n16, G_out, Rc, RcPrep, Rs, R, st); }
-        if (n <= 32) K4_GO(1) else if (n <= 64) K4_GO(2) else if (n <= 96) K4_GO(3) else if (n <= 128) K4_GO(4) else K4_GO(5)
-#undef K4_GO
+        const size_t smb = ((size_t)n16 * (n16 + 2) + 8 * (size_t)(n16 + 4) + 72 + n16) * sizeof(double);
+        cudaFuncSetAttribute(mrcqr_k4_blocked, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smb);
+        mrcqr_k4_blocked<<<1, K4B_NT, smb, s>>>(G16, n, n16, G_out, Rc, RcPrep, Rs, R, st);
         return 1;
     }
     return launch_k4_coop(const_cast<double*>(G16), n, n16, G_out, Rc, RcPrep, Rs, R, st, s);
