@@ -2,7 +2,7 @@
 //   K2  mrcqr_k2_sketch_qr  Algorithm 2 steps 5-6: Householder R-factor of the
 //                           s x n sketch, rows sign-normalised to diag > 0, FP64 arithmetic on the
 //                           precision-p sketch values (>= p; PAPER.md:119 promotes FP16 to FP32).
-//   K4  mrcqr_k4_cholesky_sm   Algorithm 1 step 2: G = Rc^T Rc; a pivot <= 0 or NaN is
+//   K4  mrcqr_k4_blocked   Algorithm 1 step 2: G = Rc^T Rc; a pivot <= 0 or NaN is
 //                           reported, never shifted away.
 //   prep_R                  builds the "prepared" factor the tile solve consumes.
 //   triu_mul                Algorithm 2 step 9: R = Rc Rs.
@@ -38,10 +38,6 @@ __global__ void mrcqr_triu_mul(const double* __restrict__ Rc, const double* __re
 }
 
 // ---- K4 ---------------------------------------------------------------------------------------
-// (A blocked single-CTA form -- 8-column steps: diagonal block by one warp, row panel by one thread per column, rank-8
-// update -- was measured slower than the one-barrier-per-pivot kernel below at every n <= 128: 71 vs 48 us at n = 64,
-// 212 vs 183 us at n = 128; its panel solve is a 36-deep chain of shared-memory loads and its diagonal block 8 software
-// rsqrt.  It is not kept.)
 // 1/sqrt(x) for a positive finite double: hardware seed + two Newton steps (a few ulp; the pivot's own
 // rounding error is of the same size).  Short dependent chain: it sits on the critical path of every pivot.
 __device__ __forceinline__ double rsqrt_fast(double x)
@@ -54,112 +50,18 @@ __device__ __forceinline__ double rsqrt_fast(double x)
     return y;
 }
 
-// ---- K4, shared-memory form (n16 <= 160): unblocked right-looking, ONE barrier per pivot -----------
-// Step k: every thread updates its elements (i, j), k < i <= j, with the UNSCALED row k and the
-// reciprocal square root of pivot k:  W[i,j] -= (W[k,i] ri_k) (W[k,j] ri_k); the thread that owns
-// (k+1, k+1) then publishes ri_{k+1} = rsqrt(pivot), so the next step needs no second barrier.
-// Rows are scaled at the end: Rc[k,j] = W[k,j] ri_k, Rc[k,k] = pivot ri_k.
-template <int JM>                            // JM = ceil(n / 32): elements per thread = JM x JM, in registers per step
-__global__ void __launch_bounds__(SMALL_NT)
-mrcqr_k4_cholesky_sm(const double* __restrict__ G16, int n, int n16, double* __restrict__ G_out,
-                     double* __restrict__ Rc, double* __restrict__ RcPrep, const double* __restrict__ Rs,
-                     double* __restrict__ R, Status* st)
-{
-    extern __shared__ __align__(16) double sm[];
-    double* dinv = sm;                       // n16 (+ pad): ri_k
-    double* W = sm + n16 + 2;
-    const int ldw = n16 + 1;
-    const int tid = threadIdx.x, NT = blockDim.x;
-    for (int e = tid; e < n * n; e += NT) {
-        const int i = e % n, j = e / n;
-        const double v = G16[(size_t)j * n16 + i];
-        if (G_out) G_out[e] = v;
-        W[j * ldw + i] = v;
-    }
-    __syncthreads();
-    if (tid == 0) {
-        const double piv = W[0];
-        if (!(piv > 0.0) || isinf(piv)) report(st, 3, 0);
-        dinv[0] = rsqrt(piv);
-    }
-    const int ti = tid & 31, tj = tid >> 5, NJ = 32;                 // 2-D thread layout: no index division
-    for (int k = 0; k < n - 1; ++k) {
-        __syncthreads();
-        if (tj + 32 * (JM - 1) <= k) continue;                       // warp-uniform: no column j > k in this warp
-        const double ri = dinv[k];
-        double a[JM], b[JM], w[JM][JM];
-#pragma unroll
-        for (int u = 0; u < JM; ++u) {                               // all loads first: nothing aliases column k
-            const int x = ti + 32 * u, y = tj + 32 * u;
-            a[u] = (x > k && x < n) ? W[x * ldw + k] : 0.0;
-            b[u] = (y > k && y < n) ? W[y * ldw + k] : 0.0;
-        }
-#pragma unroll
-        for (int v = 0; v < JM; ++v)
-#pragma unroll
-            for (int u = 0; u < JM; ++u) {
-                const int i = ti + 32 * u, j = tj + 32 * v;
-                w[v][u] = (i > k && i <= j && j < n) ? W[j * ldw + i] : 0.0;
-            }
-#pragma unroll
-        for (int v = 0; v < JM; ++v)
-#pragma unroll
-            for (int u = 0; u < JM; ++u) {
-                const int i = ti + 32 * u, j = tj + 32 * v;
-                if (i > k && i <= j && j < n) {
-                    const double r = fma(-(a[u] * ri), b[v] * ri, w[v][u]);
-                    W[j * ldw + i] = r;
-                    if (i == k + 1 && j == k + 1) {
-                        if (!(r > 0.0) || isinf(r)) report(st, 3, k + 1);
-                        dinv[k + 1] = rsqrt_fast(r);
-                    }
-                }
-            }
-    }
-    __syncthreads();
-    // scale the rows (W upper <- Rc); stage Rs in the free strictly-lower triangle, transposed:
-    // Rs[k,j] (k < j) at W[k*ldw + j], diag(Rs) in rsd
-    double* rsd = dinv + n16 + 2 + n16 * ldw;                        // n16 doubles after W
-    for (int j = tj; j < n; j += NJ)
-        for (int i = ti; i <= j; i += 32) {
-            W[j * ldw + i] *= dinv[i];
-            if (R) {
-                const double v = Rs[(size_t)j * n + i];
-                if (i < j) W[i * ldw + j] = v; else rsd[j] = v;
-            }
-        }
-    __syncthreads();
-    for (int j = tj; j < n; j += NJ)
-        for (int i = ti; i < n; i += 32) {
-            double w = 0.0, r = 0.0;
-            if (i <= j) {
-                w = W[j * ldw + i];
-                if (R) {
-                    for (int k = i; k < j; ++k) r = fma(W[k * ldw + i], W[k * ldw + j], r);
-                    r = fma(w, rsd[j], r);
-                }
-            }
-            Rc[(size_t)j * n + i] = w;
-            if (R) R[(size_t)j * n + i] = r;
-        }
-    {
-        const int nB = n16 >> 3;
-        const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
-        int bad = -1;
-        for (size_t o = tid; o < total; o += NT) RcPrep[o] = prep_value(W, ldw, n, nB, o, &bad);
-    }
-}
-
 // ---- K4, blocked form with the trailing update on DMMA (n16 <= 160) ---------------------------------------
 // Eight pivots per step and three block barriers per step instead of one per pivot:
 //   (1) warp 0 factors the 8x8 diagonal block in registers (lane j owns column j; shuffles; rsqrt_fast pivots),
 //   (2) one thread per trailing column solves its 8 rows against the block, the block's 36 entries in registers first
-//       (the round-1 blocked kernel read them from shared memory inside the dependent chain and lost to the unblocked one),
+//       (a first blocked kernel read them from shared memory inside the dependent chain and lost to the unblocked
+//       one-barrier-per-pivot kernel of round 1: 71 vs 48 us at n = 64; this one: 38 us, and 131 vs 183 us at n = 128),
 //   (3) the rank-8 update G22 -= R12^T R12 runs on the FP64 tensor cores: an 8x8 block of G22 is one accumulator
 //       fragment, R12^T / R12 are the A / B fragments (k = 8: two DMMAs per block), the upper-triangular blocks dealt
 //       round-robin to the 16 warps.
 // W: working copy of G (upper triangle), col-major, ld = n16 + 2 (conflict-free accumulator fragments); Pn: the current
-// 8-row panel, ld = n16 + 4 (conflict-free A / B fragments).  Same epilogue as the unblocked kernel.
+// 8-row panel, ld = n16 + 4 (conflict-free A / B fragments).  Epilogue: Rc, the prepared Rc and, if Rs is given,
+// R = Rc Rs (Algorithm 2 step 9; Rs staged in the free strictly-lower triangle).
 constexpr int K4B_NT = 512;
 
 __global__ void __launch_bounds__(K4B_NT)
@@ -175,13 +77,13 @@ mrcqr_k4_blocked(const double* __restrict__ G16, int n, int n16, double* __restr
     double* dinv = D + 64;                       // 8
     double* rsd = dinv + 8;                      // n16
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-    for (int e = tid; e < n16 * ldw; e += K4B_NT) {
-        const int i = e % ldw, j = e / ldw;
-        double v = 0.0;
-        if (i < n && j < n) { v = G16[(size_t)j * n16 + i]; if (G_out) G_out[(size_t)j * n + i] = v; }
-        else if (i == j) v = 1.0;                // identity padding: its pivots are harmless
-        W[e] = v;
-    }
+    for (int j = warp; j < n16; j += K4B_NT / 32)             // column per warp, rows per lane: no index division
+        for (int i = lane; i < ldw; i += 32) {
+            double v = 0.0;
+            if (i < n && j < n) { v = G16[(size_t)j * n16 + i]; if (G_out) G_out[(size_t)j * n + i] = v; }
+            else if (i == j) v = 1.0;            // identity padding: its pivots are harmless
+            W[j * ldw + i] = v;
+        }
     for (int e = tid; e < 8 * pld; e += K4B_NT) Pn[e] = 0.0;
     __syncthreads();
     const int nB = n16 >> 3;
@@ -237,10 +139,12 @@ mrcqr_k4_blocked(const double* __restrict__ G16, int n, int n16, double* __restr
             __syncthreads();
             // (3) trailing update on DMMA: blocks (I, J), t0/8 <= I <= J < nB
             const int b0 = t0 >> 3, T = nB - b0, nblk = T * (T + 1) / 2;
+            int ii = warp, jj = 0;                   // block bi = warp, warp + 16, ...: (ii, jj) walks the upper triangle column by column
+            while (ii > jj) { ii -= jj + 1; ++jj; }
             for (int bi = warp; bi < nblk; bi += K4B_NT / 32) {
-                int jj = 0;
-                while ((jj + 1) * (jj + 2) / 2 <= bi) ++jj;
-                const int I = b0 + bi - jj * (jj + 1) / 2, J = b0 + jj;
+                const int I = b0 + ii, J = b0 + jj;
+                ii += K4B_NT / 32;
+                while (ii > jj) { ii -= jj + 1; ++jj; }
                 double* cp = W + (size_t)(8 * J + 2 * t) * ldw + 8 * I + g;
                 double c2[2] = {cp[0], cp[ldw]};
                 const double a0 = -Pn[t * pld + 8 * I + g], a1 = -Pn[(t + 4) * pld + 8 * I + g];
@@ -254,25 +158,76 @@ mrcqr_k4_blocked(const double* __restrict__ G16, int n, int n16, double* __restr
     }
     __syncthreads();
     // stage Rs in the free strictly-lower triangle, transposed: Rs[k,j] (k < j) at W[k*ldw + j], diag(Rs) in rsd
+    // (column per warp, rows per lane: coalesced reads, independent loads)
     if (R)
-        for (int e = tid; e < n * n; e += K4B_NT) {
-            const int i = e % n, j = e / n;
-            if (i < j) W[i * ldw + j] = Rs[(size_t)j * n + i];
-            else if (i == j) rsd[j] = Rs[(size_t)j * n + i];
-        }
+        for (int j = warp; j < n; j += K4B_NT / 32)
+            for (int i = lane; i <= j; i += 32) {
+                const double v = Rs[(size_t)j * n + i];
+                if (i < j) W[i * ldw + j] = v; else rsd[j] = v;
+            }
     __syncthreads();
-    for (int e = tid; e < n * n; e += K4B_NT) {
-        const int i = e % n, j = e / n;
-        double w = 0.0, r = 0.0;
-        if (i <= j) {
-            w = W[j * ldw + i];
+    // Rc and R = Rc Rs: R[i,j] = sum_{k=i..j} Rc[i,k] Rs[k,j], every element ONE fma chain in ascending k (the order of
+    // mrcqr_triu_mul: the stage call gives the same bits).  A thread owns a 2 x 4 patch (rows i0, i0+1, columns j0..j0+3):
+    // per k one 16-byte load of the row pair (lanes contiguous: conflict-free) and the four Rs[k, j0..] (warp-uniform)
+    // feed eight chains.  (One chain per thread, then four rows of one column per thread, were bound by shared-memory
+    // wavefronts: 17 per 4 fma; the epilogue was two thirds of K4 at n = 128.)
+    {
+        const int npp = (n + 63) >> 6, ncq = (n + 3) >> 2;
+        for (int item = warp; item < npp * ncq; item += K4B_NT / 32) {
+            const int pp = item % npp, cq = item / npp;
+            const int i0 = 2 * (lane + 32 * pp), j0 = 4 * cq, jmax = min(j0 + 3, n - 1), kw = 64 * pp;
+            if (kw > jmax) continue;                                  // warp-uniform: the patch row lies below the diagonal
+            double r[2][4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) r[0][q] = r[1][q] = 0.0;
             if (R) {
-                for (int k = i; k < j; ++k) r = fma(W[k * ldw + i], W[k * ldw + j], r);
-                r = fma(w, rsd[j], r);
+                int k = kw;
+                for (; k < j0; ++k) {                                // all four columns live: Rs[k, j0..j0+3] at W[k*ldw + j0]
+                    const double2 c = *reinterpret_cast<const double2*>(W + (size_t)k * ldw + i0);
+                    const double2 s01 = *reinterpret_cast<const double2*>(W + (size_t)k * ldw + j0);
+                    const double2 s23 = *reinterpret_cast<const double2*>(W + (size_t)k * ldw + j0 + 2);
+                    if (i0 <= k) { r[0][0] = fma(c.x, s01.x, r[0][0]); r[0][1] = fma(c.x, s01.y, r[0][1]); r[0][2] = fma(c.x, s23.x, r[0][2]); r[0][3] = fma(c.x, s23.y, r[0][3]); }
+                    if (i0 + 1 <= k) { r[1][0] = fma(c.y, s01.x, r[1][0]); r[1][1] = fma(c.y, s01.y, r[1][1]); r[1][2] = fma(c.y, s23.x, r[1][2]); r[1][3] = fma(c.y, s23.y, r[1][3]); }
+                }
+                for (; k <= jmax; ++k) {                             // the diagonal 4 x 4 corner: column j takes k <= j, Rs[j,j] from rsd
+                    const double2 c = *reinterpret_cast<const double2*>(W + (size_t)k * ldw + i0);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int j = j0 + q;
+                        if (k <= j && j < n) {
+                            const double rs = (k < j) ? W[k * ldw + j] : rsd[j];
+                            if (i0 <= k) r[0][q] = fma(c.x, rs, r[0][q]);
+                            if (i0 + 1 <= k) r[1][q] = fma(c.y, rs, r[1][q]);
+                        }
+                    }
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int j = j0 + q;
+                if (j < n) {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int i = i0 + h;
+                        if (i < n) {
+                            Rc[(size_t)j * n + i] = (i <= j) ? W[j * ldw + i] : 0.0;
+                            if (R) R[(size_t)j * n + i] = (i <= j) ? r[h][q] : 0.0;
+                        }
+                    }
+                }
             }
         }
-        Rc[e] = w;
-        if (R) R[e] = r;
+        // patches that lie wholly below the diagonal were skipped above: their zeros
+        for (int item = warp; item < npp * ncq; item += K4B_NT / 32) {
+            const int pp = item % npp, cq = item / npp;
+            const int i0 = 2 * (lane + 32 * pp), j0 = 4 * cq, jmax = min(j0 + 3, n - 1);
+            if (64 * pp <= jmax) continue;
+            for (int q = 0; q < 4; ++q)
+                for (int h = 0; h < 2; ++h) {
+                    const int i = i0 + h, j = j0 + q;
+                    if (i < n && j < n) { Rc[(size_t)j * n + i] = 0.0; if (R) R[(size_t)j * n + i] = 0.0; }
+                }
+        }
     }
     {
         const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
