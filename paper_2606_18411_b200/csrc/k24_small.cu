@@ -182,6 +182,7 @@ mrcqr_k4_blocked(const double* __restrict__ G16, int n, int n16, double* __restr
             for (int q = 0; q < 4; ++q) r[0][q] = r[1][q] = 0.0;
             if (R) {
                 int k = kw;
+#pragma unroll 4
                 for (; k < j0; ++k) {                                // all four columns live: Rs[k, j0..j0+3] at W[k*ldw + j0]
                     const double2 c = *reinterpret_cast<const double2*>(W + (size_t)k * ldw + i0);
                     const double2 s01 = *reinterpret_cast<const double2*>(W + (size_t)k * ldw + j0);
@@ -230,9 +231,8 @@ mrcqr_k4_blocked(const double* __restrict__ G16, int n, int n16, double* __restr
         }
     }
     {
-        const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
         int bad = -1;
-        for (size_t o = tid; o < total; o += K4B_NT) RcPrep[o] = prep_value(W, ldw, n, nB, o, &bad);
+        prep_cta(W, ldw, n, nB, RcPrep, &bad);
     }
 }
 

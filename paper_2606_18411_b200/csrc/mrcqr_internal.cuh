@@ -69,6 +69,28 @@ __device__ __forceinline__ double prep_value(const double* R, int ldr, int n, in
     return (row < n && col < n) ? -R[(size_t)col * ldr + row] / R[(size_t)col * ldr + col] : 0.0;
 }
 
+// The whole prepared factor written by one CTA (same values as prep_value element by element): a warp takes an
+// off-diagonal pair (K, J) at a time, so the pair index is decoded once per 64 elements, not once per element.
+// *bad_col: a column with a zero / non-finite diagonal, or left untouched.
+__device__ __forceinline__ void prep_cta(const double* R, int ldr, int n, int nB, double* out, int* bad_col)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int npair = nB * (nB - 1) / 2;
+    int J = 1, base = 0;                                   // base = J (J - 1) / 2
+    for (int pair = warp; pair < npair; pair += nwarp) {
+        while (base + J <= pair) { base += J; ++J; }
+        const int K = pair - base;
+        const int col = 8 * J + (g >> 1) + 4 * (g & 1), r0 = 8 * K + t, r1 = r0 + 4;
+        double2 v;
+        v.x = (r0 < n && col < n) ? -R[(size_t)col * ldr + r0] : 0.0;
+        v.y = (r1 < n && col < n) ? -R[(size_t)col * ldr + r1] : 0.0;
+        *reinterpret_cast<double2*>(out + (size_t)pair * 64 + 2 * lane) = v;
+    }
+    const size_t doff = prep_diag_offset(nB);
+    for (int e = threadIdx.x; e < PREP_DIAG * nB; e += blockDim.x) out[doff + e] = prep_value(R, ldr, n, nB, doff + e, bad_col);
+}
+
 // launchers (each returns the number of kernel launches it enqueued)
 int launch_prep_R(const double* R, int n, double* Rprep, int n16, Status* st, int err_code, cudaStream_t s);
 int upload_diag(const double* prep, int n16, int fac, cudaStream_t s);      // prepared diagonal blocks -> constant memory
@@ -106,10 +128,8 @@ __device__ __forceinline__ void k2_prepare(const double* Rs, int n, double* RsPr
 {
     if (!RsPrep) return;
     __syncthreads();
-    const int nB = n16 >> 3;
-    const size_t total = prep_diag_offset(nB) + (size_t)PREP_DIAG * nB;
     int bad = -1;
-    for (size_t o = threadIdx.x; o < total; o += blockDim.x) RsPrep[o] = prep_value(Rs, n, n, nB, o, &bad);
+    prep_cta(Rs, n, n, n16 >> 3, RsPrep, &bad);
     if (bad >= 0) report(st, 2, bad);
 }
 
