@@ -38,18 +38,6 @@ __global__ void mrcqr_triu_mul(const double* __restrict__ Rc, const double* __re
 }
 
 // ---- K4 ---------------------------------------------------------------------------------------
-// 1/sqrt(x) for a positive finite double: hardware seed + two Newton steps (a few ulp; the pivot's own
-// rounding error is of the same size).  Short dependent chain: it sits on the critical path of every pivot.
-__device__ __forceinline__ double rsqrt_fast(double x)
-{
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double h = 0.5 * x;
-    y = y * fma(-h * y, y, 1.5);
-    y = y * fma(-h * y, y, 1.5);
-    return y;
-}
-
 // ---- K4, blocked form with the trailing update on DMMA (n16 <= 160) ---------------------------------------
 // Eight pivots per step and three block barriers per step instead of one per pivot:
 //   (1) warp 0 factors the 8x8 diagonal block in registers (lane j owns column j; shuffles; rsqrt_fast pivots),
@@ -340,9 +328,7 @@ mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __re
         const double sigma = warp_sum(sig_l);
         double beta = alpha, cf = 0.0;
         if (sigma != 0.0) {
-            const double nrm = sqrt(fma(alpha, alpha, sigma));
-            beta = (alpha >= 0.0) ? -nrm : nrm;
-            cf = 1.0 / (beta * (beta - alpha));
+            householder_coeffs(alpha, sigma, beta, cf);
         }
 #pragma unroll
         for (int r = 0; r < RPL; ++r) {

@@ -144,9 +144,7 @@ mrcqr_k2_blocked(double* __restrict__ As, int s, int n, double* __restrict__ bet
                 const double sigma = t2[0], alpha = t2[1];
                 double beta = alpha, c = 0.0;
                 if (sigma != 0.0) {
-                    const double nrm = sqrt(fma(alpha, alpha, sigma));
-                    beta = (alpha >= 0.0) ? -nrm : nrm;
-                    c = 1.0 / (beta * (beta - alpha));
+                    householder_coeffs(alpha, sigma, beta, c);
                 }
                 vd[j] = alpha - beta; cf[j] = c;
 #pragma unroll

@@ -86,9 +86,7 @@ __device__ __forceinline__ void bt_householder(const double* As, int s, int n, d
         const double sigma = bt_warp_sum(sig_l);
         double beta = alpha, cf = 0.0;
         if (sigma != 0.0) {
-            const double nrm = sqrt(fma(alpha, alpha, sigma));
-            beta = (alpha >= 0.0) ? -nrm : nrm;
-            cf = 1.0 / (beta * (beta - alpha));
+            householder_coeffs(alpha, sigma, beta, cf);
         }
 #pragma unroll
         for (int r = 0; r < RPL; ++r) {

@@ -69,6 +69,39 @@ __device__ __forceinline__ double prep_value(const double* R, int ldr, int n, in
     return (row < n && col < n) ? -R[(size_t)col * ldr + row] / R[(size_t)col * ldr + col] : 0.0;
 }
 
+// 1/sqrt(x) and 1/x for a positive, finite, normal double: hardware seed + two Newton steps (a few ulp).  They sit on
+// the serial chain of every Cholesky pivot and every Householder reflector, where the correctly rounded sqrt / division
+// routines cost 150-250 cycles each.
+__device__ __forceinline__ double rsqrt_fast(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double h = 0.5 * x;
+    y = y * fma(-h * y, y, 1.5);
+    y = y * fma(-h * y, y, 1.5);
+    return y;
+}
+__device__ __forceinline__ double rcp_fast(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    y = fma(y, fma(-x, y, 1.0), y);
+    y = fma(y, fma(-x, y, 1.0), y);
+    return y;
+}
+// Householder coefficients of a column with pivot alpha and sigma = sum of squares below it (sigma > 0):
+// beta = -sign(alpha) sqrt(alpha^2 + sigma), c = 1 / (beta (beta - alpha)).  Falls back to the exact routines outside the
+// range where the approximations are safe.
+__device__ __forceinline__ void householder_coeffs(double alpha, double sigma, double& beta, double& c)
+{
+    const double x = fma(alpha, alpha, sigma);
+    double nrm;
+    if (x > 1e-280 && x < 1e280) nrm = x * rsqrt_fast(x); else nrm = sqrt(x);
+    beta = (alpha >= 0.0) ? -nrm : nrm;
+    const double d = beta * (beta - alpha);
+    c = (d > 1e-280 && d < 1e280) ? rcp_fast(d) : 1.0 / d;
+}
+
 // The whole prepared factor written by one CTA (same values as prep_value element by element): a warp takes an
 // off-diagonal pair (K, J) at a time, so the pair index is decoded once per 64 elements, not once per element.
 // *bad_col: a column with a zero / non-finite diagonal, or left untouched.
