@@ -53,7 +53,10 @@ def ncu_traffic(config, kernel):
         d = json.load(open(TRAFFIC_FILE))
         if d.get("src_sha16") != source_sha16():
             return None
-        return d["configs"][config][kernel]["dram_bytes_per_launch"]
+        for name, rec in sorted(d["configs"][config].items()):      # names carry their template arguments: match the prefix
+            if name == kernel or name.startswith(kernel + "<") or name.startswith(kernel):
+                return rec["dram_bytes_per_launch"]
+        return None
     except Exception:
         return None
 
@@ -342,9 +345,10 @@ def dominant_kernel(cfg, stages, hbm_peak, how):
         ach = dom_bytes / (dom_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % how}
-    tkey = {"mrcqr_k3_gram": "mrcqr_k3_gram", "mrcqr_k5_formq": "mrcqr_k5_formq", "mrcqr_syrk": "mrcqr_syrk"}.get(kname, "mrcqr_panel_pass")
+    tkey = {"mrcqr_k3_gram": "mrcqr_k3_gram", "mrcqr_k5_formq": "mrcqr_k5_formq", "mrcqr_syrk": "mrcqr_syrk"}.get(
+        kname, "mrcqr_panel_pass<0" if stage == "k3_gram" else "mrcqr_panel_pass<1")
     traffic = ncu_traffic(cfg["name"], tkey)
-    if traffic is not None and tkey == "mrcqr_panel_pass":
+    if traffic is not None and tkey.startswith("mrcqr_panel_pass"):
         traffic *= (n + 63) // 64                       # the capture holds the mean per launch; the solve is that many launches
     roof.update({"traffic": traffic, "kernel": kname, "stage": stage, "kernel_ms": dom_ms, "algorithmic_bytes": dom_bytes,
                  "algorithmic_flops": dom_flops, "hbm_gbs_achieved": dom_bytes / (dom_ms * 1e-3) / 1e9,
