@@ -469,3 +469,22 @@ def test_two_contexts_factor_concurrently(orc):
     # the default context is untouched and still works
     Q, R = B.mrcqr_factor(mats[0], jobs[0][2], 2 * jobs[0][1], 5)
     assert torch.equal(Q, ref[0][0])
+
+
+@pytest.mark.parametrize("prec,tol", [(64, 1e-12), (32, 5e-5), (16, 1e-2)])
+def test_radix16_sketch_unaligned_operands(orc, prec, tol):
+    """The register radix-16 form of K1 (m >= 8192) on an A whose columns start on an odd element and whose leading
+    dimension is odd: the 8-byte load path.  Same sketch as the aligned matrix, bit for bit, and within tolerance of the oracle."""
+    m, n, s = 1 << 14, 5, 40
+    A0 = inputs.make_A(m, n, 2, 11, 12, "cuda")
+    signs, idx = orc.draw(m, s, 4)
+    dsigns, didx = draw_to_dev(signs, idx)
+    _, As0 = B.mrcqr_sketch(A0, prec, dsigns, didx, want_As=True)
+    buf = torch.zeros(n * (m + 3) + 1, dtype=torch.float64, device="cuda")
+    view = buf[1:1 + n * (m + 3)].view(n, m + 3)[:, :m]
+    view.copy_(A0)
+    assert view.data_ptr() % 16 == 8 and view.stride(0) % 2 == 1
+    _, As1 = B.mrcqr_sketch(view, prec, dsigns, didx, want_As=True)
+    assert torch.equal(As0, As1)
+    As_o = orc.sketch(np.asfortranarray(to_np(A0)), signs, idx)
+    assert relf(to_np(As1), As_o) <= tol
