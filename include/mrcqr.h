@@ -56,7 +56,8 @@ enum {
     MRCQR_ERR_SINGULAR  = 2,  /* R_s has a zero / non-finite diagonal: A rank deficient   */
     MRCQR_ERR_BREAKDOWN = 3,  /* Cholesky pivot <= 0 or NaN; index: mrcqr_last_info() */
     MRCQR_ERR_CUDA      = 4,  /* CUDA runtime error, or no device                                        */
-    MRCQR_ERR_NOT_ORTHOGONAL = 5  /* mrcqr_factor_auto: ||I - Q^T Q||_F > tol even with the FP64 sketch       */
+    MRCQR_ERR_NOT_ORTHOGONAL = 5, /* mrcqr_factor_auto: ||I - Q^T Q||_F > tol even with the FP64 sketch       */
+    MRCQR_ERR_TOO_LARGE = 6   /* mrcqr_orth_error_noalloc: the problem exceeds its fixed static scratch       */
 };
 
 /*
@@ -180,6 +181,23 @@ int mrcqr_last_timing(float* ms_out_host);
  * Returns 0 or -1 m, -2 n, -3 ldq, -4 Q, -5 err_host, 4.
  */
 int mrcqr_orth_error(int64_t m, int n, int64_t ldq, const double* Q, double* err_host, void* stream);
+
+/*
+ * The same quantity for callers that must not allocate (stream capture, serving loops, harnesses that forbid
+ * cudaMalloc): the kernels of mrcqr_orth_error in the same order (bit-identical result), their scratch (one Gram
+ * partial per SYRK CTA, the 128 x 128 Gram matrix) in a static device array of 20 054 016 bytes (19.1 MiB) that every
+ * GPU which loads the library holds until the process exits.  Limit: n <= MRCQR_NOALLOC_N_MAX, any m >= n; a larger n
+ * (or a device with more than 151 SMs) returns MRCQR_ERR_TOO_LARGE before anything is launched.
+ * err: ONE double, DEVICE (written by the last kernel).  G: nullable, DEVICE, n x n, ld n, receives Q^T Q (full
+ * symmetric).  The call uses no context and no workspace, calls no cudaMalloc / cudaFree / allocating routine, copies
+ * nothing to the host and does not synchronise: it enqueues 3 (4 with G) kernels on `stream` and returns; a failure of
+ * a kernel on the device surfaces at the caller's next synchronisation.  Every call shares the array (it needs no
+ * clearing: each call overwrites what it reads): calls that OVERLAP on the GPU race on it, serialise them.  The first
+ * call on a device resolves the array's device address (cudaGetSymbolAddress, that device current).
+ * Returns 0 or -1 m, -2 n < 1, -3 ldq, -4 Q, -5 err, MRCQR_ERR_CUDA, MRCQR_ERR_TOO_LARGE.
+ */
+#define MRCQR_NOALLOC_N_MAX 128
+int mrcqr_orth_error_noalloc(int64_t m, int n, int64_t ldq, const double* Q, double* err, double* G, void* stream);
 
 /*
  * Self-correcting MRCQR ("the remedy is to rerun MRCQR at the next higher precision level"):

