@@ -348,6 +348,123 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
     asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
+// ---- all panels of a solve in ONE launch (n16 a multiple of 64) ------------------------------------------
+// The per-panel launches above re-read the p panels solved before panel p from DRAM (each is m x 64 doubles, far beyond
+// L2): 10 panel reads per solve at n = 256 where 4 would do.  Here a warp takes its 32-row slab through ALL panels before
+// it moves on: the solved panels it sweeps over were written by itself a few microseconds earlier and come back from L2
+// (st.cg / ld.cg: kept in L2, not in L1), so a solve reads its source once and writes its result once.  Same warp
+// program per (slab, panel) step as mrcqr_panel_pass; the landing zone receives the NEXT step's panel (same rows, next
+// panel; after the last panel the next round's first).  Diagonal blocks: FusedFactor (c_diag, uploaded once per solve).
+template <int FAC, int NPMAX>
+__global__ void __launch_bounds__(PP_NW * 32, PP_CTAS)
+mrcqr_panel_fused(int64_t m, int n, int NP, const double* __restrict__ src, int64_t lds,
+                  const double2* __restrict__ frag, double* dst, int64_t ldd, int64_t nslabs)
+{
+    extern __shared__ __align__(16) double Ysm[];
+    constexpr int RG = 4, SR = 32, LDS_ = SR + 4, PB = 8;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    double* slab = Ysm + (size_t)warp * (8 * PB) * LDS_;
+    double* scr = Ysm + (size_t)PP_NW * (8 * PB) * LDS_ + (size_t)warp * 8 * LDS_;
+    double2* Bsm = reinterpret_cast<double2*>(Ysm + (size_t)PP_NW * (8 * PB + 8) * LDS_);   // [2][PB][PP_KC][32]
+    double* yw = slab + t * LDS_ + g;
+    const int ncols_last = n - 64 * (NP - 1);
+    auto stage_chunk = [&](int c, int P0) {          // block rows [4c, 4c+4) x the PB block columns of panel P0 / 8
+        double2* dstb = Bsm + (size_t)(c & 1) * PB * PP_KC * 32;
+        for (int e = tid; e < PB * PP_KC * 32; e += PP_NW * 32) {
+            const int J = e / (PP_KC * 32), kl = (e / 32) % PP_KC, ln = e & 31;
+            const int Kg = PP_KC * c + kl;
+            if (Kg < P0) cp_async16(dstb + e, fragpair(frag, Kg, P0 + J, ln), 16);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    auto request = [&](int64_t i, int p) {           // panel p of slab i into the landing zone (one commit group)
+        if (i < nslabs) {
+            const int nc = (p == NP - 1) ? ncols_last : 64;
+            if (nc < 64) zero_pad_columns<SR>(slab, nc, 64, lane);
+            load_slab<SR, true>(slab, src + (size_t)(64 * p) * (size_t)lds, lds, m, nc, i * SR, lane);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    const int64_t rounds = (nslabs + (int64_t)gridDim.x * PP_NW - 1) / ((int64_t)gridDim.x * PP_NW);
+    __syncwarp();
+    request((int64_t)blockIdx.x * PP_NW + warp, 0);
+    for (int64_t r = 0; r < rounds; ++r) {
+        const int64_t i = (r * gridDim.x + blockIdx.x) * PP_NW + warp;
+        const bool active = i < nslabs;
+        const int64_t row0 = i * SR;
+        const int64_t inext = ((r + 1) * gridDim.x + blockIdx.x) * PP_NW + warp;
+        for (int p = 0; p < NP; ++p) {
+            const int P0 = 8 * p, nchunks = 2 * p;   // P0 / PP_KC
+            const int ncols = (p == NP - 1) ? ncols_last : 64;
+            const FusedFactor<FAC, NPMAX> fac{frag, p};
+            __syncthreads();                         // previous step done with both chunk buffers; its stores are visible
+            if (nchunks > 0) stage_chunk(0, P0);
+            const double* yp = dst + (size_t)t * (size_t)ldd + row0 + g;
+            double a0[RG], a1[RG];
+            if (P0 > 0 && active) {
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) { a0[rg] = __ldcg(yp + 8 * rg); a1[rg] = __ldcg(yp + (size_t)4 * ldd + 8 * rg); }
+            }
+            if (nchunks > 0) asm volatile("cp.async.wait_group 1;" ::: "memory");     // own panel landed (requested a step ago)
+            else asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncwarp();
+            double acc[RG][PB][2];
+            if (active) {
+#pragma unroll
+                for (int J = 0; J < PB; ++J)
+#pragma unroll
+                    for (int rg = 0; rg < RG; ++rg) {
+                        acc[rg][J][0] = yw[(8 * J) * LDS_ + 8 * rg];
+                        acc[rg][J][1] = yw[(8 * J + 4) * LDS_ + 8 * rg];
+                    }
+            }
+            __syncwarp();                            // every lane has its fragments: the landing zone is free again
+            auto prefetch = [&]() { if (p + 1 < NP) request(i, p + 1); else request(inext, 0); };
+            if (nchunks == 0) prefetch();
+            for (int c = 0; c < nchunks; ++c) {
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+                __syncthreads();                     // chunk c visible; everyone is done with chunk c-1
+                if (c + 1 < nchunks) stage_chunk(c + 1, P0);
+                else prefetch();
+                if (active) {
+                    const double2* bs = Bsm + (size_t)(c & 1) * PB * PP_KC * 32 + lane;
+                    for (int kl = 0; kl < PP_KC; ++kl) {
+                        const int Kg = PP_KC * c + kl;
+                        double n0[RG], n1[RG];
+                        const int Kn = (Kg + 1 < P0) ? Kg + 1 : Kg;
+                        const double* yn = yp + (size_t)(8 * Kn) * (size_t)ldd;
+#pragma unroll
+                        for (int rg = 0; rg < RG; ++rg) { n0[rg] = __ldcg(yn + 8 * rg); n1[rg] = __ldcg(yn + (size_t)4 * ldd + 8 * rg); }
+#pragma unroll
+                        for (int J = 0; J < PB; ++J) {
+                            const double2 b = bs[(J * PP_KC + kl) * 32];
+#pragma unroll
+                            for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a0[rg], b.x);
+#pragma unroll
+                            for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], a1[rg], b.y);
+                        }
+#pragma unroll
+                        for (int rg = 0; rg < RG; ++rg) { a0[rg] = n0[rg]; a1[rg] = n1[rg]; }
+                    }
+                }
+            }
+            if (active) {
+                double* out = dst + (size_t)(64 * p) * (size_t)ldd + row0 + lane;      // lane = row of the slab
+                auto sink = [&](int Kg, const double (&y)[8]) {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int col = 8 * (Kg - P0) + j;
+                        if (col < ncols) __stcg(out + (size_t)col * (size_t)ldd, y[j]);
+                    }
+                };
+                panel_core<RG, PB>(acc, ScratchXpose<RG>(scr, lane), fac, P0, lane, sink);
+            }
+        }
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+}
+
 // G16[i,j] (i <= j) = sum over the CTA partials in a FIXED order (deterministic split-m reduction):
 // thread (element, q) adds the partials q, q+32, q+64, ... in ascending order; the 32 per-thread sums of
 // an element are combined by a fixed binary tree in shared memory.  32 elements x 32 lanes per CTA;
@@ -496,7 +613,20 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
     int64_t grid = (nslabs + nw - 1) / nw;
     if (grid > PP_CTAS * num_sms()) grid = PP_CTAS * num_sms();
     int launches = 0;
-    for (int P0 = 0; P0 < nB; P0 += 8) {
+    const int NPF = nB / 8;                          // full 8-block panels: ONE launch (mrcqr_panel_fused)
+    if (NPF > 0) {
+        const int smem = nw * (8 * 8 + 8) * 36 * 8 + 2 * 8 * PP_KC * 512;
+        const int nf = n < 64 * NPF ? n : 64 * NPF;
+#define PF_GO(FAC_, NPM_)                                                                           \
+        { auto k = mrcqr_panel_fused<FAC_, NPM_>;                                                   \
+          cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);               \
+          k<<<(int)grid, nw * 32, smem, s>>>(m, nf, NPF, src, lds, frag, dstp, ldd, nslabs); }
+        if (NPF <= 4) { if (fac == 0) PF_GO(0, 4) else PF_GO(1, 4) }
+        else { if (fac == 0) PF_GO(0, 8) else PF_GO(1, 8) }
+#undef PF_GO
+        ++launches;
+    }
+    for (int P0 = 8 * NPF; P0 < nB; P0 += 8) {       // the ragged last panel (2, 4 or 6 blocks): a launch of its own
         const int pb = (nB - P0 >= 8) ? 8 : nB - P0;
         int ncols = n - 8 * P0;
         if (ncols > 8 * pb) ncols = 8 * pb;
@@ -510,7 +640,7 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
           cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);               \
           k<<<(int)grid, nw * 32, smem, s>>>(m, ncols, P0, own, lds, dstp, ldd, frag, out, ldd, nslabs); }
 #define PP_CALL(PB_) { if (fac == 0) PP_GO(0, PB_) else PP_GO(1, PB_) }
-        if (pb == 8) PP_CALL(8) else if (pb == 6) PP_CALL(6) else if (pb == 4) PP_CALL(4) else PP_CALL(2)
+        if (pb == 6) PP_CALL(6) else if (pb == 4) PP_CALL(4) else PP_CALL(2)
 #undef PP_CALL
 #undef PP_GO
         ++launches;

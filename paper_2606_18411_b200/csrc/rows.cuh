@@ -145,6 +145,7 @@ struct ConstFactor {
     const double2* __restrict__ frag;
     __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const { return __ldg(fragpair(frag, Kg, Jg, lane)); }
     __device__ __forceinline__ const double* diag(int Kg) const { return &c_diag[FAC][Kg * PREP_DIAG]; }
+    __device__ __forceinline__ void substitute(double (&y)[8], int P0, int K) const { diag_substitute(y, diag(P0 + K)); }
 };
 #endif
 #ifndef MRCQR_NO_CONST_DIAG
@@ -157,6 +158,28 @@ struct PanelFactor {
     const double2* __restrict__ frag; int P0;
     __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const { return __ldg(fragpair(frag, Kg, Jg, lane)); }
     __device__ __forceinline__ const double* diag(int Kg) const { return &c_pdiag[FAC][(Kg - P0) * PREP_DIAG]; }
+    __device__ __forceinline__ void substitute(double (&y)[8], int, int K) const { diag_substitute(y, &c_pdiag[FAC][K * PREP_DIAG]); }
+};
+// FusedFactor: all panels of a solve in ONE launch (mrcqr_panel_fused): the panel index p is a run-time value, so the
+// substitution of block K of panel p is picked by a warp-uniform switch among NPMAX copies whose coefficients are
+// compile-time offsets into c_diag[FAC] (instruction operands again, not indexed constant loads).
+template <int FAC, int NPMAX>
+struct FusedFactor {
+    const double2* __restrict__ frag; int p;
+    __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const { return __ldg(fragpair(frag, Kg, Jg, lane)); }
+    __device__ __forceinline__ void substitute(double (&y)[8], int, int K) const
+    {
+        switch (p) {
+            case 0: diag_substitute(y, &c_diag[FAC][(0 + K) * PREP_DIAG]); break;
+            case 1: diag_substitute(y, &c_diag[FAC][(8 + K) * PREP_DIAG]); break;
+            case 2: diag_substitute(y, &c_diag[FAC][(16 + K) * PREP_DIAG]); break;
+            case 3: diag_substitute(y, &c_diag[FAC][(24 + K) * PREP_DIAG]); break;
+            case 4: if (NPMAX > 4) diag_substitute(y, &c_diag[FAC][((NPMAX > 4 ? 32 : 0) + K) * PREP_DIAG]); break;
+            case 5: if (NPMAX > 4) diag_substitute(y, &c_diag[FAC][((NPMAX > 4 ? 40 : 0) + K) * PREP_DIAG]); break;
+            case 6: if (NPMAX > 4) diag_substitute(y, &c_diag[FAC][((NPMAX > 4 ? 48 : 0) + K) * PREP_DIAG]); break;
+            default: if (NPMAX > 4) diag_substitute(y, &c_diag[FAC][((NPMAX > 4 ? 56 : 0) + K) * PREP_DIAG]); break;
+        }
+    }
 };
 #endif
 struct SmemFactor {
@@ -164,6 +187,7 @@ struct SmemFactor {
     __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const
     { return *reinterpret_cast<const double2*>(prep + 2 * ((size_t)(Jg * (Jg - 1) / 2 + Kg) * 32 + lane)); }
     __device__ __forceinline__ const double* diag(int Kg) const { return prep + prep_diag_offset(nB) + Kg * PREP_DIAG; }
+    __device__ __forceinline__ void substitute(double (&y)[8], int P0, int K) const { diag_substitute(y, diag(P0 + K)); }
 };
 
 // ---- where a block goes between its DMMA (accumulator) form and its one-thread-per-row form -------
@@ -232,7 +256,7 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
             }
         }
         if (xp.row_active()) {
-            diag_substitute(y, fac.diag(P0 + K));
+            fac.substitute(y, P0, K);
 #pragma unroll
             for (int j = 0; j < 8; ++j) *xp.rowp(P0 + K, j) = y[j];
             sink(P0 + K, y);

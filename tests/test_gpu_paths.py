@@ -90,6 +90,10 @@ def test_fft_sketch_tile_widths_match_oracle(orc, m, n, s, prec, tol):
     (1 << 12, 240, 8, 64),     # n16 = 240: panels 8, 8, 8, 6
     (1 << 11, 400, 4, 32),     # P = 4 SYRK blocks, 7 panels
     (1 << 11, 512, 5, 64),     # the largest n
+    (1 << 12, 256, 7, 64),     # n16 % 64 == 0: all panels of a solve in one launch (mrcqr_panel_fused), 4 panels
+    (1 << 12, 250, 5, 32),     # the same with a ragged last panel (58 columns)
+    (1 << 12, 180, 4, 32),     # 3 panels (n16 = 192), last one ragged
+    (1 << 11, 500, 3, 64),     # 8 panels, last one ragged
 ])
 def test_store_y_path_factorization(orc, m, n, expo, prec):
     AT = inputs.make_A(m, n, expo, 500 + n, 501 + n, "cuda")
