@@ -321,16 +321,19 @@ def time_point(B, AT, QT, R, cfg, steps, warmup, stream, sampler=None, barrier=N
 def dominant_kernel(cfg, stages, hbm_peak, how):
     """The kernel with the largest share of the step and its roofline (DESIGN.md section 5 states the per-row figures).
     n <= 128: K3 (8n bytes, 2n^2 flops per row) or K5 (16n bytes, 2n^2 flops per row), one launch = all m rows.
-    n > 128: one triangular solve = ceil(n/64) panel-pass launches (n^2 flops, 16n bytes per row over those launches) or
-    the SYRK launch (n^2 flops, 8n bytes per row); `kernel_ms` is the duration of those launches together."""
+    n > 128: one triangular solve = one mrcqr_panel_fused launch over the full 64-column panels (+ one mrcqr_panel_pass
+    launch for a ragged last panel; n^2 flops, 16n bytes per row) or the SYRK launch (n^2 flops, 8n bytes per row);
+    `kernel_ms` is the duration of the stage."""
     m, n = cfg["m"], cfg["n"]
     if n <= 128:
         cand = {"k3_gram": ("mrcqr_k3_gram", 8.0 * m * n, 2.0 * m * n * n),
                 "k5_form_q": ("mrcqr_k5_formq", 16.0 * m * n, 2.0 * m * n * n)}
     else:
-        cand = {"k3_gram": ("mrcqr_panel_pass<0> (solve with R_s, %d launches)" % ((n + 63) // 64), 16.0 * m * n, 1.0 * m * n * n),
+        ragged = ((n + 15) // 16 * 16) % 64 != 0
+        tail = (lambda f: " + mrcqr_panel_pass<%d> for the ragged last panel" % f if ragged else "")
+        cand = {"k3_gram": ("mrcqr_panel_fused<0> (solve with R_s, all full panels in one launch)" + tail(0), 16.0 * m * n, 1.0 * m * n * n),
                 "gram_reduce": ("mrcqr_syrk", 8.0 * m * n, 1.0 * m * n * n),
-                "k5_form_q": ("mrcqr_panel_pass<1> (solve with R_c, %d launches)" % ((n + 63) // 64), 16.0 * m * n, 1.0 * m * n * n)}
+                "k5_form_q": ("mrcqr_panel_fused<1> (solve with R_c, all full panels in one launch)" + tail(1), 16.0 * m * n, 1.0 * m * n * n)}
     stage = max(cand, key=lambda k: stages[k])
     kname, dom_bytes, dom_flops = cand[stage]
     dom_ms = stages[stage]
@@ -346,10 +349,11 @@ def dominant_kernel(cfg, stages, hbm_peak, how):
         roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % how}
     tkey = {"mrcqr_k3_gram": "mrcqr_k3_gram", "mrcqr_k5_formq": "mrcqr_k5_formq", "mrcqr_syrk": "mrcqr_syrk"}.get(
-        kname, "mrcqr_panel_pass<0" if stage == "k3_gram" else "mrcqr_panel_pass<1")
+        kname, "mrcqr_panel_fused<0" if stage == "k3_gram" else "mrcqr_panel_fused<1")
     traffic = ncu_traffic(cfg["name"], tkey)
-    if traffic is not None and tkey.startswith("mrcqr_panel_pass"):
-        traffic *= (n + 63) // 64                       # the capture holds the mean per launch; the solve is that many launches
+    if traffic is not None and tkey.startswith("mrcqr_panel_fused") and ((n + 15) // 16 * 16) % 64 != 0:
+        rest = ncu_traffic(cfg["name"], tkey.replace("fused", "pass"))      # the ragged last panel's own launch
+        traffic = None if rest is None else traffic + rest
     roof.update({"traffic": traffic, "kernel": kname, "stage": stage, "kernel_ms": dom_ms, "algorithmic_bytes": dom_bytes,
                  "algorithmic_flops": dom_flops, "hbm_gbs_achieved": dom_bytes / (dom_ms * 1e-3) / 1e9,
                  "traffic_source": "profiles/r02_traffic.json (ncu --set full of these kernel sources)" if traffic is not None

@@ -357,7 +357,7 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
 // panel; after the last panel the next round's first).  Diagonal blocks: FusedFactor (c_diag, uploaded once per solve).
 template <int FAC, int NPMAX>
 __global__ void __launch_bounds__(PP_NW * 32, PP_CTAS)
-mrcqr_panel_fused(int64_t m, int n, int NP, const double* __restrict__ src, int64_t lds,
+mrcqr_panel_fused(int64_t m, int n, int NP, const double* src, int64_t lds,      // src == dst for the in-place solve
                   const double2* __restrict__ frag, double* dst, int64_t ldd, int64_t nslabs)
 {
     extern __shared__ __align__(16) double Ysm[];
