@@ -6,8 +6,8 @@
 // the Q buffer), this kernel forms G = Y^T Y from it, and stage 2b solves in place (SURVEY.md 8(f)
 // "store-Y": 3 m n^2 flops instead of 4 m n^2; Y costs one write and 1 + reads of 8 m n bytes).
 //
-// G is cut into 128 x 128 blocks (I <= J); a CTA owns one block and one contiguous range of rows
-// (deterministic split of m), streams 32-row chunks of the two 128-column panels of Y through a
+// G is cut into 128 x 128 blocks (I <= J); a CTA owns one block and a strided set of the 32-row chunks
+// (deterministic split of m: chunk c belongs to CTA c mod k of its block), streams 32-row chunks of the two 128-column panels of Y through a
 // triple-buffered shared-memory tile (cp.async, one barrier per chunk) and accumulates on DMMA: 8 warps as 4 x 2, each
 // 32 x 64 of the block (4 x 8 accumulators, 12 fragment loads per 32 DMMA).  Accumulator chains are
 // flushed to the CTA's partial every 1024 rows (reading R7); a reduction kernel adds the
@@ -39,8 +39,7 @@ __device__ __forceinline__ void sy_cp16(void* dst, const void* src, int bytes)
 struct SyrkParams {
     int64_t m, ldy;
     int n, n16, P, pairs;
-    int ks_diag, ks_off;              // row ranges per diagonal / off-diagonal block (a diagonal block costs 18/32)
-    int64_t rows_diag, rows_off;      // rows per range, multiples of SY_KC
+    int ks_diag, ks_off;              // CTAs (strided sets of 32-row chunks) per diagonal / off-diagonal block (a diagonal block costs 18/32)
     int vec;
 };
 
@@ -116,12 +115,13 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
     sy_pair(pair, I, J);
     const bool diag = (I == J);
     const int wi = warp & 3, wj = warp >> 2;
-    const int64_t mpad = (p.m + SY_KC - 1) / SY_KC * SY_KC;
-    const int64_t rps = diag ? p.rows_diag : p.rows_off;
-    const int64_t k0 = (int64_t)ks_id * rps;
-    int64_t k1 = k0 + rps;
-    if (k1 > mpad) k1 = mpad;
-    const int nchunks = k1 > k0 ? (int)((k1 - k0) / SY_KC) : 0;
+    // This CTA's chunks are ks_id, ks_id + ks_n, ks_id + 2 ks_n, ... of the m / 32 chunks (a strided, not a contiguous,
+    // range): every block type then sweeps the rows at the same pace (the split equalises their finishing times), the CTAs
+    // of the diagonal and of the off-diagonal blocks that need the same panel chunk ask for it within microseconds of each
+    // other, and the second one finds it in L2 (contiguous ranges read every panel of Y twice from DRAM).
+    const int64_t chunks = (p.m + SY_KC - 1) / SY_KC;
+    const int nchunks = chunks > ks_id ? (int)((chunks - ks_id + ks_n - 1) / ks_n) : 0;
+    auto chunk_row = [&](int c) { return ((int64_t)ks_id + (int64_t)c * ks_n) * SY_KC; };
     double* part = partials + (size_t)blockIdx.x * SY_B * SY_B;
 
     unsigned maskI = 0, maskJ = 0;
@@ -132,8 +132,8 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
     }
     auto issue = [&](int c) {                        // chunk c -> stage c % 3
         double* st = sy_sm + (size_t)(c % 3) * 2 * PAN;
-        sy_load_panel(st, p, Y, I, k0 + (int64_t)c * SY_KC, tid, maskI);
-        if (!diag) sy_load_panel(st + PAN, p, Y, J, k0 + (int64_t)c * SY_KC, tid, maskJ);
+        sy_load_panel(st, p, Y, I, chunk_row(c), tid, maskI);
+        if (!diag) sy_load_panel(st + PAN, p, Y, J, chunk_row(c), tid, maskJ);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     // three stages, ONE barrier per chunk: the barrier of iteration c also proves that every warp is done
@@ -213,7 +213,7 @@ mrcqr_syrk(SyrkParams p, const double* __restrict__ Y, double* __restrict__ part
     if (nchunks == 0) flush();                               // an empty range still owns a (zero) partial
 }
 
-// G16[i,j] (i <= j) = sum over the row ranges of block (I,J), fixed order (32 lanes of ranges + binary tree)
+// G16[i,j] (i <= j) = sum over the CTAs (chunk sets) of block (I,J), fixed order (32 lanes of ranges + binary tree)
 __global__ void __launch_bounds__(1024)
 mrcqr_syrk_reduce(SyrkParams p, const double* __restrict__ partials, double* __restrict__ G16)
 {
@@ -269,8 +269,6 @@ static SyrkParams syrk_params(int64_t m, int n, int n16)
     if (ko > chunks) ko = (int)chunks;
     if (kd > chunks) kd = (int)chunks;
     p.ks_diag = kd; p.ks_off = ko > 0 ? ko : 1;
-    p.rows_diag = (chunks + kd - 1) / kd * SY_KC;
-    p.rows_off = (chunks + p.ks_off - 1) / p.ks_off * SY_KC;
     return p;
 }
 
