@@ -397,7 +397,7 @@ mrcqr_panel_fused(int64_t m, int n, int NP, const double* src, int64_t lds,     
         for (int p = 0; p < NP; ++p) {
             const int P0 = 8 * p, nchunks = 2 * p;   // P0 / PP_KC
             const int ncols = (p == NP - 1) ? ncols_last : 64;
-            const FusedFactor<FAC, NPMAX> fac{frag, p};
+            const FusedFactor<FAC, NPMAX> fac(frag, p, lane);
             __syncthreads();                         // previous step done with both chunk buffers; its stores are visible
             if (nchunks > 0) stage_chunk(0, P0);
             const double* yp = dst + (size_t)t * (size_t)ldd + row0 + g;
@@ -450,13 +450,15 @@ mrcqr_panel_fused(int64_t m, int n, int NP, const double* src, int64_t lds,     
                 }
             }
             if (active) {
-                double* out = dst + (size_t)(64 * p) * (size_t)ldd + row0 + lane;      // lane = row of the slab
-                auto sink = [&](int Kg, const double (&y)[8]) {
+                double* o = dst + (size_t)(64 * p) * (size_t)ldd + row0 + lane;        // lane = row of the slab
+                int left = ncols;                    // columns of the panel not yet stored (blocks arrive in order)
+                auto sink = [&](int, const double (&y)[8]) {
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const int col = 8 * (Kg - P0) + j;
-                        if (col < ncols) __stcg(out + (size_t)col * (size_t)ldd, y[j]);
+                    for (int j = 0; j < 8; ++j) {    // one running pointer: no per-column address arithmetic
+                        if (j < left) __stcg(o, y[j]);
+                        o += ldd;
                     }
+                    left -= 8;
                 };
                 panel_core<RG, PB>(acc, ScratchXpose<RG>(scr, lane), fac, P0, lane, sink);
             }

@@ -146,6 +146,7 @@ struct ConstFactor {
     __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const { return __ldg(fragpair(frag, Kg, Jg, lane)); }
     __device__ __forceinline__ const double* diag(int Kg) const { return &c_diag[FAC][Kg * PREP_DIAG]; }
     __device__ __forceinline__ void substitute(double (&y)[8], int P0, int K) const { diag_substitute(y, diag(P0 + K)); }
+    __device__ __forceinline__ double2 pair_in(int P0, int K, int J, int lane) const { return pair(P0 + K, P0 + J, lane); }
 };
 #endif
 #ifndef MRCQR_NO_CONST_DIAG
@@ -159,6 +160,7 @@ struct PanelFactor {
     __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const { return __ldg(fragpair(frag, Kg, Jg, lane)); }
     __device__ __forceinline__ const double* diag(int Kg) const { return &c_pdiag[FAC][(Kg - P0) * PREP_DIAG]; }
     __device__ __forceinline__ void substitute(double (&y)[8], int, int K) const { diag_substitute(y, &c_pdiag[FAC][K * PREP_DIAG]); }
+    __device__ __forceinline__ double2 pair_in(int P0_, int K, int J, int lane) const { return pair(P0_ + K, P0_ + J, lane); }
 };
 // FusedFactor: all panels of a solve in ONE launch (mrcqr_panel_fused): the panel index p is a run-time value, so the
 // substitution of block K of panel p is picked by a warp-uniform switch among NPMAX copies whose coefficients are
@@ -166,7 +168,14 @@ struct PanelFactor {
 template <int FAC, int NPMAX>
 struct FusedFactor {
     const double2* __restrict__ frag; int p;
+    const double2* __restrict__ own;          // fragpair(frag, P0, P0, lane): the panel's own pairs start here
+    unsigned jstride;                         // 32 P0: pair (P0 + K, P0 + J) sits at own + J jstride + 32 (J (J - 1) / 2 + K)
+    __device__ __forceinline__ FusedFactor(const double2* f, int p_, int lane)
+        : frag(f), p(p_), own(f + ((size_t)(8 * p_) * (8 * p_ - 1) / 2 + 8 * p_) * 32 + lane), jstride(32u * 8u * (unsigned)p_) {}
     __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const { return __ldg(fragpair(frag, Kg, Jg, lane)); }
+    // in-panel pair with compile-time K, J: one multiply-add on the address instead of the triangular index arithmetic
+    __device__ __forceinline__ double2 pair_in(int, int K, int J, int) const
+    { return __ldg(own + (size_t)jstride * (unsigned)J + (unsigned)(32 * (J * (J - 1) / 2 + K))); }
     __device__ __forceinline__ void substitute(double (&y)[8], int, int K) const
     {
         switch (p) {
@@ -188,6 +197,7 @@ struct SmemFactor {
     { return *reinterpret_cast<const double2*>(prep + 2 * ((size_t)(Jg * (Jg - 1) / 2 + Kg) * 32 + lane)); }
     __device__ __forceinline__ const double* diag(int Kg) const { return prep + prep_diag_offset(nB) + Kg * PREP_DIAG; }
     __device__ __forceinline__ void substitute(double (&y)[8], int P0, int K) const { diag_substitute(y, diag(P0 + K)); }
+    __device__ __forceinline__ double2 pair_in(int P0, int K, int J, int lane) const { return pair(P0 + K, P0 + J, lane); }
 };
 
 // ---- where a block goes between its DMMA (accumulator) form and its one-thread-per-row form -------
@@ -236,7 +246,7 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
         // keep the compiler from hoisting it): an L1 miss then hides under the substitution
         // (panel passes only: K3 / K5 run more warps on fewer registers and lose by the longer live range)
         double2 bnext = make_double2(0.0, 0.0);
-        if (X::REUSE && K + 1 < PB) bnext = fac.pair(P0 + K, P0 + K + 1, lane);
+        if (X::REUSE && K + 1 < PB) bnext = fac.pair_in(P0, K, K + 1, lane);
 #pragma unroll
         for (int rg = 0; rg < RG; ++rg) { *xp.accp(P0 + K, rg, 0) = acc[rg][K][0]; *xp.accp(P0 + K, rg, 1) = acc[rg][K][1]; }
         __syncwarp();
@@ -248,7 +258,7 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
         if (K > 0) {
 #pragma unroll
             for (int J = K + 1; J < PB; ++J) {
-                const double2 b = fac.pair(P0 + K - 1, P0 + J, lane);
+                const double2 b = fac.pair_in(P0, K - 1, J, lane);
 #pragma unroll
                 for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][J], ap0[rg], b.x);
 #pragma unroll
@@ -269,7 +279,7 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
             for (int rg = 0; rg < RG; ++rg) { acc[rg][K][0] = ap0[rg]; acc[rg][K][1] = ap1[rg]; }
         }
         if (K + 1 < PB) {
-            if (!X::REUSE) bnext = fac.pair(P0 + K, P0 + K + 1, lane);
+            if (!X::REUSE) bnext = fac.pair_in(P0, K, K + 1, lane);
 #pragma unroll
             for (int rg = 0; rg < RG; ++rg) dmma884(acc[rg][K + 1], ap0[rg], bnext.x);
 #pragma unroll
