@@ -273,12 +273,19 @@ def max_over_ranks(value, device="cpu"):
     return float(t.item())
 
 
-def floors(m, n, hbm_peak):
+def stores_y(n):
+    """The library's default form of stage 2 (include/mrcqr.h, mrcqr_set_store_y): store-Y from n16 = 112 on."""
+    return (n + 15) // 16 * 16 >= 112
+
+
+def floors(m, n, hbm_peak, store_y=None):
     """Algorithmic work of one factorization (SURVEY.md 8(d)): 32 m n bytes (3 reads of A + 1 write of Q) for every n;
-    4 m n^2 flops in the recompute form (n <= 128), 3 m n^2 in the store-Y form (n > 128: its extra write + read of Y is
+    4 m n^2 flops in the fused (recompute) form, 3 m n^2 in the store-Y form (its extra write + read of Y is
     traffic, not algorithm).  Returns (bytes, flops, hbm floor ms, fp64 floor ms)."""
     alg_bytes = 32.0 * m * n
-    flops = (3.0 if n > 128 else 4.0) * m * n * n
+    if store_y is None:
+        store_y = stores_y(n)
+    flops = (3.0 if store_y else 4.0) * m * n * n
     return alg_bytes, flops, alg_bytes / (hbm_peak * 1e9) * 1e3, flops / (FP64_DMMA_PEAK_TFLOPS * 1e12) * 1e3
 
 
@@ -320,12 +327,12 @@ def time_point(B, AT, QT, R, cfg, steps, warmup, stream, sampler=None, barrier=N
 
 def dominant_kernel(cfg, stages, hbm_peak, how):
     """The kernel with the largest share of the step and its roofline (DESIGN.md section 5 states the per-row figures).
-    n <= 128: K3 (8n bytes, 2n^2 flops per row) or K5 (16n bytes, 2n^2 flops per row), one launch = all m rows.
-    n > 128: one triangular solve = one mrcqr_panel_fused launch over the full 64-column panels (+ one mrcqr_panel_pass
+    Fused form (n16 < 112): K3 (8n bytes, 2n^2 flops per row) or K5 (16n bytes, 2n^2 flops per row), one launch = all m rows.
+    Store-Y form (n16 >= 112): one triangular solve = one mrcqr_panel_fused launch over the full 64-column panels (+ one mrcqr_panel_pass
     launch for a ragged last panel; n^2 flops, 16n bytes per row) or the SYRK launch (n^2 flops, 8n bytes per row);
     `kernel_ms` is the duration of the stage."""
     m, n = cfg["m"], cfg["n"]
-    if n <= 128:
+    if not stores_y(n):
         cand = {"k3_gram": ("mrcqr_k3_gram", 8.0 * m * n, 2.0 * m * n * n),
                 "k5_form_q": ("mrcqr_k5_formq", 16.0 * m * n, 2.0 * m * n * n)}
     else:
@@ -359,6 +366,32 @@ def dominant_kernel(cfg, stages, hbm_peak, how):
                  "traffic_source": "profiles/r02_traffic.json (ncu --set full of these kernel sources)" if traffic is not None
                  else "no ncu capture of these kernel sources / this config on file"})
     return roof
+
+
+def time_forms(B, AT, QT, R, cfg, steps, stream):
+    """ms per factorization with stage 2 forced to each of its two forms (mrcqr_set_store_y 0 / 1); the library's default
+    picks by n16 (store-Y from 112 on)."""
+    import torch
+    out = {}
+    try:
+        for key, mode in (("fused_ms", False), ("store_y_ms", True)):
+            B.mrcqr_set_store_y(mode)
+            for _ in range(3):
+                B.mrcqr_factor(AT, cfg["prec"], cfg["s"], cfg["seed_draw"], QT, R, stream)
+            v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            v0.record(stream)
+            for _ in range(steps):
+                B.mrcqr_factor(AT, cfg["prec"], cfg["s"], cfg["seed_draw"], QT, R, stream)
+            v1.record(stream)
+            torch.cuda.synchronize()
+            out[key] = v0.elapsed_time(v1) / steps
+    finally:
+        B.mrcqr_set_store_y(None)
+    out["default"] = "store_y" if stores_y(cfg["n"]) else "fused"
+    out["note"] = ("fused: Y = A Rs^-1 kept on chip by stage 2a and recomputed by stage 2b (north_star's form: 4 passes, "
+                   "4 m n^2 flops); store_y: written to Q's buffer, Gram from it, solved in place (5 passes, 3 m n^2 flops); "
+                   "default: store_y from n16 = 112 on (measured threshold)")
+    return out
 
 
 def point_json(cfg, ms, stages, hbm_peak, clocks=None):
@@ -442,22 +475,8 @@ def run_ours(args):
     total_ms = max_over_ranks(total_ms, "cuda")
     ms = total_ms / args.steps
 
-    # ---- variant: store-Y form of stage 2 for n <= 128 (n > 128 always stores Y) ----
-    variants = None
-    if n <= 128:
-        B.mrcqr_set_store_y(True)
-        for _ in range(3):
-            B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
-        v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        v0.record(stream)
-        for _ in range(args.steps):
-            B.mrcqr_factor(AT, prec, s, seed, QT, R, stream)
-        v1.record(stream)
-        torch.cuda.synchronize()
-        B.mrcqr_set_store_y(False)
-        variants = {"store_y_ms": v0.elapsed_time(v1) / args.steps,
-                    "note": "mrcqr_set_store_y(1): Y = A Rs^-1 written to Q's buffer by stage 2a, solved in place by stage 2b "
-                            "(5 passes, 3 m n^2 flops) instead of kept on chip and recomputed (4 passes, 4 m n^2)"}
+    # ---- both forms of stage 2 where the library chooses (n16 <= 128) ----
+    variants = time_forms(B, AT, QT, R, cfg, args.steps, stream) if n <= 128 else None
 
     # ---- end to end: HOST buffers through mrcqr_factor_host (H2D + D2H inside the timed region) ----
     A_host = torch.empty((n, m), dtype=torch.float64, pin_memory=True)
@@ -495,7 +514,10 @@ def run_ours(args):
             psamp = ClockSampler(local)
             psteps = max(1, min(args.steps, 10))
             ptot, _, pstages = time_point(B, PA, PQ, PR, pc, psteps, 3, stream, psamp)
-            points.append(point_json(pc, ptot / psteps, pstages, hbm_peak, psamp.stop()))
+            pj = point_json(pc, ptot / psteps, pstages, hbm_peak, psamp.stop())
+            if pc["n"] <= 128:
+                pj["forms"] = time_forms(B, PA, PQ, PR, pc, psteps, stream)
+            points.append(pj)
             del PA, PQ
             torch.cuda.empty_cache()
 
@@ -518,8 +540,8 @@ def run_ours(args):
                              "fp64_frac": flops / (ms * 1e-3) / 1e12 / FP64_DMMA_PEAK_TFLOPS,
                              "hbm_floor_ms": t_hbm, "fp64_floor_ms": t_f64, "binding_frac": max(t_hbm, t_f64) / ms,
                              "stage_ms": stages,
-                             "extra_traffic": "store-Y form (n > 128): +16 m n bytes (Y written by solve 1, read by the SYRK) "
-                                              "beyond the 32 m n algorithmic bytes" if n > 128 else None},
+                             "extra_traffic": "store-Y form: +16 m n bytes (Y written by solve 1, read by the SYRK) "
+                                              "beyond the 32 m n algorithmic bytes" if stores_y(n) else None},
                 "variants": variants, "roofline": roof, "cpu_baseline": cpu,
                 "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": 8 * m * n,
                         "d2h_bytes_per_step": 8 * m * n + 8 * n * n, "steps": e2e_steps},
@@ -565,7 +587,7 @@ def run_sweep(args):
         e1.record()
         torch.cuda.synchronize()
         tot = e0.elapsed_time(e1) / args.steps
-        flop = (3.0 if n > 128 else 4.0) * m * n * n
+        flop = (3.0 if stores_y(n) else 4.0) * m * n * n
         print("| %s | %d | %d | fp%d | %.3f | %.3f | %.3f | %.3f | %.3f | %.3f | %.3f | %.3f | %.1e | %.1e |" % (
             name, m, n, cfg["prec"], tot, acc["k1_srtt"], acc["k2_sketch_qr"], acc["k3_gram"], acc["gram_reduce"] + acc["k4_chol"],
             acc["k5_form_q"], 32.0 * m * n / (hbm_peak * 1e9) * 1e3, flop / (FP64_DMMA_PEAK_TFLOPS * 1e12) * 1e3,

@@ -75,7 +75,7 @@ def lib():
 EXPORTS = ["mrcqr_create", "mrcqr_set_current", "mrcqr_destroy", "mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
            "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim",
-           "mrcqr_orth_error_noalloc"]
+           "mrcqr_orth_error_noalloc", "mrcqr_last_used_store_y"]
 
 STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "gram_reduce", "k4_chol", "k5_form_q"]
 
@@ -336,9 +336,14 @@ def mrcqr_set_sketch_reim(on):
     _reim = bool(on)
 
 
-def mrcqr_set_store_y(on):
-    """Store-Y variant of stage 2 also for n <= 128 (default off: Y stays on chip and is recomputed)."""
-    lib().mrcqr_set_store_y(1 if on else 0)
+def mrcqr_set_store_y(mode):
+    """Form of stage 2 for n16 <= 128: None = by the measured threshold (default: store-Y from n16 = 112 on), False = always
+    fused (Y stays on chip and is recomputed: north_star's form), True = always store-Y."""
+    lib().mrcqr_set_store_y(-1 if mode is None else (1 if mode else 0))
+
+
+def mrcqr_last_used_store_y():
+    return bool(lib().mrcqr_last_used_store_y())
 
 
 def mrcqr_set_timing(on):

@@ -82,12 +82,13 @@ struct Ctx {
     int* bcodes = nullptr; int* h_bcodes = nullptr; size_t bcodes_cap = 0;   // mrcqr_factor_batched: (code, info) per problem, device + pinned
     bool timing = false; cudaEvent_t ev[8] = {}; bool ev_ok = false; float stage_ms[8] = {};
     bool have_device = false, probed = false;
-    bool store_y = false;                    // mrcqr_set_store_y: store-Y variant also for n16 <= 128
+    int store_y = -1;                        // mrcqr_set_store_y: -1 by measured threshold, 0 never for n16 <= 128, 1 always
+    bool last_store_y = false;               // what the last mrcqr_factor did
     bool reim = false;                       // mrcqr_set_sketch_reim: Re+Im sketch (2s rows)
     // mrcqr_set_graph: the whole enqueue sequence of mrcqr_factor captured once per (shape, buffers) and replayed
     bool use_graph = false;
     cudaGraphExec_t gexec = nullptr; int glaunches = 0; uint64_t* h_seed = nullptr;
-    struct { int64_t m, lda; int n, prec, s; const void *A, *Q, *R, *ws, *hidx; bool store_y, reim; } gkey = {};
+    struct { int64_t m, lda; int n, prec, s; const void *A, *Q, *R, *ws, *hidx; int store_y; bool reim; } gkey = {};
 };
 // Every entry point works on the calling thread's CURRENT context: the process default one, or the handle made current
 // with mrcqr_set_current (mrcqr_create / mrcqr_destroy).  A context owns its workspace, staging buffers, settings,
@@ -180,6 +181,7 @@ static bool is_pow2(int64_t m) { return m > 0 && (m & (m - 1)) == 0; }
 static bool prec_ok(int p) { return p == 16 || p == 32 || p == 64; }
 constexpr int N_MAX = 512;
 constexpr int S_MAX = 4096;
+constexpr int STORE_Y_AUTO_N16 = 112;    // n16 from which the store-Y form of stage 2 is the faster one (measured, see enqueue_stage23)
 
 // enqueue helpers shared by the stage calls and mrcqr_factor ----------------------------------------
 static int enqueue_sketch(const Layout& L, int64_t m, int n, int64_t lda, const double* A, int prec, int s,
@@ -418,7 +420,8 @@ static bool timing_events()
 }
 
 extern "C" int mrcqr_set_timing(int on) { g.timing = (on != 0); return 0; }
-extern "C" int mrcqr_set_store_y(int on) { g.store_y = (on != 0); return 0; }
+extern "C" int mrcqr_set_store_y(int mode) { g.store_y = mode < 0 ? -1 : (mode != 0); return 0; }
+extern "C" int mrcqr_last_used_store_y(void) { return g.last_store_y ? 1 : 0; }
 extern "C" int mrcqr_set_sketch_reim(int on) { g.reim = (on != 0); return 0; }
 extern "C" int mrcqr_set_graph(int on) { g.use_graph = (on != 0); if (!on) drop_graph(); return 0; }
 
@@ -447,15 +450,24 @@ static int enqueue_stage23(const Layout& L, int64_t m, int n, int64_t lda, const
         GateScope gate(st);
         k += upload_diag(RsPrep, n16, 0, st);
         if (tm) cudaEventRecord(g.ev[3], st);
-        const bool store_y = n16 > 128;          // Gram of a stored Y (k3_syrk.cu): Y = A Rs^-1 lives in the Q buffer
-        const bool panels = store_y && panel_pass_usable(m, n, A, lda, Q, ldq);
+        // Gram of a stored Y (k3_syrk.cu): Y = A Rs^-1 lives in the Q buffer.  Always for n16 > 128 (the Gram matrix no
+        // longer fits one SM).  For n16 <= 128 by the switch: 1 always, 0 never (north_star's form: Y never written,
+        // recomputed bit-identically by K5), -1 (default) from the measured threshold STORE_Y_AUTO_N16 on: the store-Y
+        // form does 3 m n^2 flops against 4 m n^2 and wins once the FP64 pipe, not HBM, is what binds (
+        // m = 2^21: n16 = 96 3.92 vs 4.30 ms, n16 = 112 5.09 vs 4.80, n16 = 128 6.78 vs 5.09).  The panel kernels need
+        // aligned operands and m % 32 == 0; without them the switch = 1 keeps K3 with a Y dump + K5 in place.
+        const bool panels_ok = panel_pass_usable(m, n, A, lda, Q, ldq);
+        const bool want_y = g.store_y > 0 || (g.store_y < 0 && n16 >= STORE_Y_AUTO_N16);
+        const bool store_y = n16 > 128 || (want_y && panels_ok);
+        g.last_store_y = store_y || g.store_y > 0;
+        const bool panels = store_y && panels_ok;
         if (store_y) {
             if (panels) k += launch_panel_solve(m, n, 0, A, lda, RsPrep, Q, ldq, st);
             else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 1, st);
             if (tm) cudaEventRecord(g.ev[4], st);
             k += launch_syrk(m, n, ldq, Q, part, n16, G16, st);
         } else {
-            k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, g.store_y ? Q : nullptr, ldq, st);
+            k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, g.store_y > 0 ? Q : nullptr, ldq, st);
             if (tm) cudaEventRecord(g.ev[4], st);
             k += launch_reduce_partials(part, np, n, n16, G16, st);
         }
@@ -465,7 +477,7 @@ static int enqueue_stage23(const Layout& L, int64_t m, int n, int64_t lda, const
         if (tm) cudaEventRecord(g.ev[6], st);
         if (panels) k += launch_panel_solve(m, n, 1, Q, ldq, RcPrep, Q, ldq, st);                // q = y Rc^-1 in place
         else if (store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);
-        else if (g.store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);  // variant: stored Y
+        else if (g.store_y > 0) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);  // variant: stored Y
         else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 3, st);        // Alg.1 step 3
         if (tm) cudaEventRecord(g.ev[7], st);
     }

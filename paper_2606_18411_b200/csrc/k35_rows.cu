@@ -602,7 +602,8 @@ int launch_k5_formq(int64_t m, int n, int64_t lda, const double* A, const double
 // Requires 16-byte aligned operands and m % 32 == 0 (the caller falls back to the slab kernel otherwise).
 bool panel_pass_usable(int64_t m, int n, const double* src, int64_t lds, const double* dstp, int64_t ldd)
 {
-    return round_up(n, 16) > 128 && (m % 32 == 0) && vec_ok(src, lds) && vec_ok(dstp, ldd);
+    (void)n;
+    return (m % 32 == 0) && vec_ok(src, lds) && vec_ok(dstp, ldd);
 }
 
 int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds, const double* prep,

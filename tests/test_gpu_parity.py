@@ -295,7 +295,11 @@ def test_factor_equals_its_stages_on_the_oracle_draw(orc, m, n, s, prec):
     """mrcqr_factor(seed) is bit for bit the composition sketch(oracle.draw) -> precondition_gram -> form_q: every
     kernel is deterministic, so equality holds iff the device-drawn sign words and bins equal the oracle's."""
     AT = inputs.make_A(m, n, 3, 800 + n, 801 + n, "cuda")
-    QT, R = B.mrcqr_factor(AT, prec, s, 77)
+    B.mrcqr_set_store_y(False)        # the stage calls are the fused form of stage 2; mrcqr_factor's default stores Y from n16 = 112 on
+    try:
+        QT, R = B.mrcqr_factor(AT, prec, s, 77)
+    finally:
+        B.mrcqr_set_store_y(None)
     signs, idx = orc.draw(m, s, 77)
     dsigns, didx = draw_to_dev(signs, idx)
     Rs, _ = B.mrcqr_sketch(AT, prec, dsigns, didx)

@@ -123,19 +123,42 @@ def test_store_y_path_is_deterministic_and_handles_strides(orc):
     assert np.linalg.norm(Q4n - to_np(Q1)) <= 10 * kappa * n * U
 
 
-@pytest.mark.parametrize("m,n,prec", [(1 << 14, 64, 16), (1 << 13, 100, 32), (1 << 13, 20, 64)])
-def test_store_y_variant_below_128_columns(orc, m, n, prec):
-    """mrcqr_set_store_y(1): stage 2a writes Y into Q's buffer, stage 2b solves it in place.
-    Same factorization as the default (recompute) form: the stored Y is the Y the Gram matrix saw, so Q is
-    bit-identical to the default path's."""
-    AT = inputs.make_A(m, n, 4, 900 + n, 901 + n, "cuda")
-    Q0, R0 = B.mrcqr_factor(AT, prec, 2 * n, 31)
-    B.mrcqr_set_store_y(True)
+@pytest.mark.parametrize("m,n,prec,aligned", [(1 << 14, 64, 16, True), (1 << 13, 100, 32, True), (1 << 13, 20, 64, True),
+                                              (1 << 14, 128, 32, True), (1 << 13, 100, 32, False), (1 << 13, 20, 64, False)])
+def test_both_forms_of_stage2_below_128_columns(orc, m, n, prec, aligned):
+    """mrcqr_set_store_y: 0 = fused form (north_star's: Y stays on chip, K5 recomputes it), 1 = store-Y
+    form (stage 2a writes Y into Q's buffer, stage 2b solves it in place), default = store-Y from n16 = 112 on.
+    Both forms against the oracle.  Aligned operands take the kernels of the n16 > 128 path for store-Y (panel solves +
+    SYRK): the same factorization up to the rounding of a differently ordered Gram sum.  Operands the panel kernels cannot
+    take (A starting on an odd element) keep K3 with a Y dump + K5 in place: the stored Y is the Y the Gram matrix saw,
+    so Q is bit-identical to the fused form's."""
+    A0 = inputs.make_A(m, n, 4, 900 + n, 901 + n, "cuda")
+    if aligned:
+        AT = A0
+    else:
+        buf = torch.empty((n, m + 2), dtype=torch.float64, device="cuda")
+        AT = buf[:, 1:m + 1]
+        AT.copy_(A0)
+    n16 = (n + 15) // 16 * 16
     try:
-        Q1, R1 = factor_parity(orc, AT, 2 * n, 31, prec)
-    finally:
         B.mrcqr_set_store_y(False)
-    assert torch.equal(Q0, Q1) and torch.equal(R0, R1)
+        Q0, R0 = factor_parity(orc, AT, 2 * n, 31, prec)
+        assert not B.mrcqr_last_used_store_y()
+        B.mrcqr_set_store_y(True)
+        Q1, R1 = factor_parity(orc, AT, 2 * n, 31, prec)
+        assert B.mrcqr_last_used_store_y()
+        B.mrcqr_set_store_y(None)
+        Q2, R2 = B.mrcqr_factor(AT, prec, 2 * n, 31)
+        assert B.mrcqr_last_used_store_y() == (aligned and n16 >= 112)      # the measured threshold (include/mrcqr.h)
+    finally:
+        B.mrcqr_set_store_y(None)
+    assert torch.equal(Q2, Q1 if (aligned and n16 >= 112) else Q0)
+    if aligned:
+        kappa = np.linalg.cond(to_np(R0))
+        assert np.linalg.norm(to_np(Q1) - to_np(Q0)) <= 10 * kappa * n * U
+        assert np.linalg.norm(to_np(R1) - to_np(R0)) <= 10 * kappa * n * U * np.linalg.norm(to_np(R0))
+    else:
+        assert torch.equal(Q0, Q1) and torch.equal(R0, R1)
 
 
 def test_large_n_kernels_report_breakdown(orc):
