@@ -274,8 +274,13 @@ def max_over_ranks(value, device="cpu"):
 
 
 def stores_y(n):
-    """The library's default form of stage 2 (include/mrcqr.h, mrcqr_set_store_y): store-Y from n16 = 112 on."""
-    return (n + 15) // 16 * 16 >= 112
+    """The library's default form of stage 2 (include/mrcqr.h, mrcqr_set_store_y): Y stored from n16 = 48 on."""
+    return (n + 15) // 16 * 16 >= 48
+
+
+def syrk_form(n):
+    """... and from n16 = 128 on the stored Y goes through the panel solves and the SYRK (below: K3 with a Y dump + K5)."""
+    return (n + 15) // 16 * 16 >= 128
 
 
 def floors(m, n, hbm_peak, store_y=None):
@@ -327,14 +332,16 @@ def time_point(B, AT, QT, R, cfg, steps, warmup, stream, sampler=None, barrier=N
 
 def dominant_kernel(cfg, stages, hbm_peak, how):
     """The kernel with the largest share of the step and its roofline (DESIGN.md section 5 states the per-row figures).
-    Fused form (n16 < 112): K3 (8n bytes, 2n^2 flops per row) or K5 (16n bytes, 2n^2 flops per row), one launch = all m rows.
-    Store-Y form (n16 >= 112): one triangular solve = one mrcqr_panel_fused launch over the full 64-column panels (+ one mrcqr_panel_pass
+    n16 < 128: K3 (8n bytes read (+ 8n written when Y is stored), 2n^2 flops per row) or K5 (16n bytes; 2n^2 flops per row
+    in the fused form, n^2 when it solves a stored Y), one launch = all m rows.
+    n16 >= 128: one triangular solve = one mrcqr_panel_fused launch over the full 64-column panels (+ one mrcqr_panel_pass
     launch for a ragged last panel; n^2 flops, 16n bytes per row) or the SYRK launch (n^2 flops, 8n bytes per row);
     `kernel_ms` is the duration of the stage."""
     m, n = cfg["m"], cfg["n"]
-    if not stores_y(n):
-        cand = {"k3_gram": ("mrcqr_k3_gram", 8.0 * m * n, 2.0 * m * n * n),
-                "k5_form_q": ("mrcqr_k5_formq", 16.0 * m * n, 2.0 * m * n * n)}
+    if not syrk_form(n):
+        sy = stores_y(n)
+        cand = {"k3_gram": ("mrcqr_k3_gram", (16.0 if sy else 8.0) * m * n, 2.0 * m * n * n),
+                "k5_form_q": ("mrcqr_k5_formq", 16.0 * m * n, (1.0 if sy else 2.0) * m * n * n)}
     else:
         ragged = ((n + 15) // 16 * 16) % 64 != 0
         tail = (lambda f: " + mrcqr_panel_pass<%d> for the ragged last panel" % f if ragged else "")
@@ -389,8 +396,8 @@ def time_forms(B, AT, QT, R, cfg, steps, stream):
         B.mrcqr_set_store_y(None)
     out["default"] = "store_y" if stores_y(cfg["n"]) else "fused"
     out["note"] = ("fused: Y = A Rs^-1 kept on chip by stage 2a and recomputed by stage 2b (north_star's form: 4 passes, "
-                   "4 m n^2 flops); store_y: written to Q's buffer, Gram from it, solved in place (5 passes, 3 m n^2 flops); "
-                   "default: store_y from n16 = 112 on (measured threshold)")
+                   "4 m n^2 flops); store_y: also written to Q's buffer and solved in place by stage 2b (5 passes, 3 m n^2 "
+                   "flops; n16 = 128: panel solves + SYRK); default: the faster one as measured, store_y from n16 = 48 on")
     return out
 
 
@@ -399,7 +406,11 @@ def point_json(cfg, ms, stages, hbm_peak, clocks=None):
     out = {"config": "%s: m=%d n=%d s=%d fp%d" % (cfg["name"], cfg["m"], cfg["n"], cfg["s"], cfg["prec"]),
            "ms": ms, "stage_ms": stages, "hbm_floor_ms": t_hbm, "fp64_floor_ms": t_f64,
            "hbm_frac": t_hbm / ms, "fp64_frac": t_f64 / ms, "binding_frac": max(t_hbm, t_f64) / ms,
-           "hbm_gbs": alg_bytes / (ms * 1e-3) / 1e9, "fp64_tflops": flops / (ms * 1e-3) / 1e12}
+           "hbm_gbs": alg_bytes / (ms * 1e-3) / 1e9, "fp64_tflops": flops / (ms * 1e-3) / 1e12,
+           "flops_form": "3 m n^2 (Y stored)" if stores_y(cfg["n"]) else "4 m n^2 (fused)"}
+    if stores_y(cfg["n"]) and cfg["n"] <= 128:       # where a form was CHOSEN: the fraction against the fused form's floors too
+        _, _, th4, tf4 = floors(cfg["m"], cfg["n"], hbm_peak, store_y=False)
+        out["binding_frac_vs_fused_form_floors"] = max(th4, tf4) / ms
     if clocks is not None:
         out["clocks"] = clocks
     return out
@@ -540,8 +551,9 @@ def run_ours(args):
                              "fp64_frac": flops / (ms * 1e-3) / 1e12 / FP64_DMMA_PEAK_TFLOPS,
                              "hbm_floor_ms": t_hbm, "fp64_floor_ms": t_f64, "binding_frac": max(t_hbm, t_f64) / ms,
                              "stage_ms": stages,
-                             "extra_traffic": "store-Y form: +16 m n bytes (Y written by solve 1, read by the SYRK) "
-                                              "beyond the 32 m n algorithmic bytes" if stores_y(n) else None},
+                             "extra_traffic": ("Y stored: +8 m n bytes beyond the 32 m n algorithmic bytes (written by stage 2a, "
+                                               "read instead of A by stage 2b)" + ("; + 8 m n read by the SYRK" if syrk_form(n) else ""))
+                             if stores_y(n) else None},
                 "variants": variants, "roofline": roof, "cpu_baseline": cpu,
                 "e2e": {"value": e2e_ms, "unit": "ms", "h2d_bytes_per_step": 8 * m * n,
                         "d2h_bytes_per_step": 8 * m * n + 8 * n * n, "steps": e2e_steps},

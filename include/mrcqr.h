@@ -235,13 +235,15 @@ int mrcqr_kappa_probe(int64_t m, int n, int64_t lda, const double* A, double* Qw
  * Form of stage 2 for n16 <= 128 (n16 = n rounded up to 16) in mrcqr_factor / mrcqr_factor_host:
  *   fused    stage 2a keeps Y = A R_s^-1 on chip and stage 2b recomputes it bit-identically (north_star's form:
  *            4 passes over m x n, 4 m n^2 flops, Y never written);
- *   store-Y  stage 2a writes Y into Q's buffer, the Gram matrix is formed from it and stage 2b solves it in place
- *            against R_c (5 passes, 3 m n^2 flops: the paper's own TrsmPre / TrsmFin order).
- * mode < 0 (default): by the measured threshold, store-Y from n16 = 112 on (there the FP64 pipe, not HBM, binds:
- * 6.78 vs 5.09 ms at m = 2^21, n = 128), fused below it; mode 0: always fused; mode > 0: always store-Y.  For
- * n16 > 128 Y is always stored (the Gram matrix no longer fits one SM).  Both forms meet the same tolerances; they
- * differ in the rounding of a differently ordered Gram sum.  Returns 0.  mrcqr_last_used_store_y: 1 if the last
- * mrcqr_factor of this context stored Y, else 0.
+ *   stored   stage 2a writes Y into Q's buffer and stage 2b solves it in place against R_c (5 passes, 3 m n^2 flops:
+ *            the paper's own TrsmPre / TrsmFin order).  Below n16 = 128 (and for operands that are
+ *            not 16-byte aligned or m not a multiple of 32) the Gram matrix is still accumulated on chip beside the
+ *            write, and Q, R are bit-identical to the fused form's; at n16 = 128 the kernels of the n > 128 path run
+ *            (panel solve, Gram of the stored Y, panel solve), same tolerances, a differently ordered Gram sum.
+ * mode < 0 (default): the faster one as measured on B200: fused for n16 <= 32, where HBM binds;
+ * stored from n16 = 48 on, where the FP64 pipe binds (m = 2^21: n = 64 1.79 vs 1.69 ms, n = 128 6.69 vs 5.09 ms).
+ * mode 0: always fused; mode > 0: always stored.  For n16 > 128 Y is always stored (the Gram matrix no longer fits one
+ * SM).  Returns 0.  mrcqr_last_used_store_y: 1 if the last mrcqr_factor of this context stored Y, else 0.
  */
 int mrcqr_set_store_y(int mode);
 int mrcqr_last_used_store_y(void);

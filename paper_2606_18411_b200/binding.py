@@ -337,8 +337,8 @@ def mrcqr_set_sketch_reim(on):
 
 
 def mrcqr_set_store_y(mode):
-    """Form of stage 2 for n16 <= 128: None = by the measured threshold (default: store-Y from n16 = 112 on), False = always
-    fused (Y stays on chip and is recomputed: north_star's form), True = always store-Y."""
+    """Form of stage 2 for n16 <= 128: None = the faster one as measured (default: Y stored from n16 = 48 on), False = always
+    fused (Y stays on chip and is recomputed: north_star's form), True = always stored."""
     lib().mrcqr_set_store_y(-1 if mode is None else (1 if mode else 0))
 
 

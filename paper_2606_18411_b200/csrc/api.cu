@@ -181,7 +181,8 @@ static bool is_pow2(int64_t m) { return m > 0 && (m & (m - 1)) == 0; }
 static bool prec_ok(int p) { return p == 16 || p == 32 || p == 64; }
 constexpr int N_MAX = 512;
 constexpr int S_MAX = 4096;
-constexpr int STORE_Y_AUTO_N16 = 112;    // n16 from which the store-Y form of stage 2 is the faster one (measured, see enqueue_stage23)
+constexpr int STORE_Y_AUTO_N16 = 48;     // n16 from which storing Y is the faster form of stage 2 (measured, see enqueue_stage23)
+constexpr int STORE_Y_SYRK_N16 = 128;    // ... and from which the stored Y goes through the panel solves and the SYRK
 
 // enqueue helpers shared by the stage calls and mrcqr_factor ----------------------------------------
 static int enqueue_sketch(const Layout& L, int64_t m, int n, int64_t lda, const double* A, int prec, int s,
@@ -450,24 +451,28 @@ static int enqueue_stage23(const Layout& L, int64_t m, int n, int64_t lda, const
         GateScope gate(st);
         k += upload_diag(RsPrep, n16, 0, st);
         if (tm) cudaEventRecord(g.ev[3], st);
-        // Gram of a stored Y (k3_syrk.cu): Y = A Rs^-1 lives in the Q buffer.  Always for n16 > 128 (the Gram matrix no
-        // longer fits one SM).  For n16 <= 128 by the switch: 1 always, 0 never (north_star's form: Y never written,
-        // recomputed bit-identically by K5), -1 (default) from the measured threshold STORE_Y_AUTO_N16 on: the store-Y
-        // form does 3 m n^2 flops against 4 m n^2 and wins once the FP64 pipe, not HBM, is what binds (
-        // m = 2^21: n16 = 96 3.92 vs 4.30 ms, n16 = 112 5.09 vs 4.80, n16 = 128 6.78 vs 5.09).  The panel kernels need
-        // aligned operands and m % 32 == 0; without them the switch = 1 keeps K3 with a Y dump + K5 in place.
+        // Stage 2 has three forms (include/mrcqr.h, mrcqr_set_store_y):
+        //   fused   K3 keeps Y = A Rs^-1 on chip, K5 recomputes it bit-identically (north_star's form; 4 m n^2 flops)
+        //   dump    K3 also writes Y into Q's buffer, K5 solves it in place against Rc (3 m n^2 flops, same Q bit for bit)
+        //   syrk    panel solve writes Y, the SYRK forms G from it, panel solve in place (3 m n^2 flops; the only form for
+        //           n16 > 128, where the Gram matrix no longer fits one SM)
+        // Default (-1): the fastest measured one.  m = 2^21, ms per factorization, fused / dump / syrk:
+        //   n16 = 16: 0.309 / 0.334 / 1.58   32: 0.620 / 0.632 / 1.85   48: 1.094 / 1.030 / -   64: 1.79 / 1.69 / 2.66
+        //   80: 3.13 / 2.86 / 3.78   96: 3.94 / 3.57 / 4.30   112: 5.10 / 4.60 / 4.80   128: 6.69 / 5.93 / 5.09
+        // i.e. fused while HBM binds (n16 <= 32), dump for 48 <= n16 <= 112, syrk from 128 on.
         const bool panels_ok = panel_pass_usable(m, n, A, lda, Q, ldq);
-        const bool want_y = g.store_y > 0 || (g.store_y < 0 && n16 >= STORE_Y_AUTO_N16);
-        const bool store_y = n16 > 128 || (want_y && panels_ok);
-        g.last_store_y = store_y || g.store_y > 0;
-        const bool panels = store_y && panels_ok;
-        if (store_y) {
+        const bool want_y = n16 > 128 || g.store_y > 0 || (g.store_y < 0 && n16 >= STORE_Y_AUTO_N16);
+        const bool syrk_form = n16 > 128 || (want_y && n16 >= STORE_Y_SYRK_N16 && panels_ok);
+        const bool panels = syrk_form && panels_ok;
+        const bool dump_form = want_y && !syrk_form;
+        g.last_store_y = want_y;
+        if (syrk_form) {
             if (panels) k += launch_panel_solve(m, n, 0, A, lda, RsPrep, Q, ldq, st);
             else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 1, st);
             if (tm) cudaEventRecord(g.ev[4], st);
             k += launch_syrk(m, n, ldq, Q, part, n16, G16, st);
         } else {
-            k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, g.store_y > 0 ? Q : nullptr, ldq, st);
+            k += launch_k3_gram(m, n, lda, A, RsPrep, part, &np, nullptr, dump_form ? Q : nullptr, ldq, st);
             if (tm) cudaEventRecord(g.ev[4], st);
             k += launch_reduce_partials(part, np, n, n16, G16, st);
         }
@@ -476,8 +481,7 @@ static int enqueue_stage23(const Layout& L, int64_t m, int n, int64_t lda, const
         k += upload_diag(RcPrep, n16, 1, st);
         if (tm) cudaEventRecord(g.ev[6], st);
         if (panels) k += launch_panel_solve(m, n, 1, Q, ldq, RcPrep, Q, ldq, st);                // q = y Rc^-1 in place
-        else if (store_y) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);
-        else if (g.store_y > 0) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);  // variant: stored Y
+        else if (syrk_form || dump_form) k += launch_k5_formq(m, n, ldq, Q, RsPrep, RcPrep, ldq, Q, nullptr, 2, st);
         else k += launch_k5_formq(m, n, lda, A, RsPrep, RcPrep, ldq, Q, nullptr, 3, st);        // Alg.1 step 3
         if (tm) cudaEventRecord(g.ev[7], st);
     }

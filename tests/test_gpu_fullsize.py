@@ -42,6 +42,19 @@ def test_full_config_elementwise(orc, name):
     kappa = np.linalg.cond(o["R"])
     assert np.linalg.norm(Q - o["Q"]) <= 10 * kappa * n * U
     assert np.linalg.norm(to_np(R) - o["R"]) <= 10 * kappa * n * U * np.linalg.norm(o["R"])
+    if B.mrcqr_last_used_store_y():                            # C2: the default stored Y; north_star's fused form as well
+        B.mrcqr_set_store_y(False)
+        try:
+            QF, RF = B.mrcqr_factor(AT, prec, s, cfg["seed_draw"])
+            assert not B.mrcqr_last_used_store_y()
+        finally:
+            B.mrcqr_set_store_y(None)
+        check_invariants(AT, QF, RF)
+        assert np.linalg.norm(to_np(QF) - o["Q"]) <= 10 * kappa * n * U
+        assert np.linalg.norm(to_np(RF) - o["R"]) <= 10 * kappa * n * U * np.linalg.norm(o["R"])
+        del QF
+    else:
+        assert name == "C1"
     # kappa(A Rs^-1) = O(1) for the GPU's own reduced-precision R_s
     Rs, _ = B.mrcqr_sketch(AT, prec, dsigns, didx)
     Rc, _ = B.mrcqr_precondition_gram(AT, Rs)

@@ -295,7 +295,7 @@ def test_factor_equals_its_stages_on_the_oracle_draw(orc, m, n, s, prec):
     """mrcqr_factor(seed) is bit for bit the composition sketch(oracle.draw) -> precondition_gram -> form_q: every
     kernel is deterministic, so equality holds iff the device-drawn sign words and bins equal the oracle's."""
     AT = inputs.make_A(m, n, 3, 800 + n, 801 + n, "cuda")
-    B.mrcqr_set_store_y(False)        # the stage calls are the fused form of stage 2; mrcqr_factor's default stores Y from n16 = 112 on
+    B.mrcqr_set_store_y(False)        # the stage calls are the fused form of stage 2; at n16 = 128 mrcqr_factor's default is the SYRK form
     try:
         QT, R = B.mrcqr_factor(AT, prec, s, 77)
     finally:

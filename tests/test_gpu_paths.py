@@ -124,14 +124,15 @@ def test_store_y_path_is_deterministic_and_handles_strides(orc):
 
 
 @pytest.mark.parametrize("m,n,prec,aligned", [(1 << 14, 64, 16, True), (1 << 13, 100, 32, True), (1 << 13, 20, 64, True),
-                                              (1 << 14, 128, 32, True), (1 << 13, 100, 32, False), (1 << 13, 20, 64, False)])
-def test_both_forms_of_stage2_below_128_columns(orc, m, n, prec, aligned):
-    """mrcqr_set_store_y: 0 = fused form (north_star's: Y stays on chip, K5 recomputes it), 1 = store-Y
-    form (stage 2a writes Y into Q's buffer, stage 2b solves it in place), default = store-Y from n16 = 112 on.
-    Both forms against the oracle.  Aligned operands take the kernels of the n16 > 128 path for store-Y (panel solves +
-    SYRK): the same factorization up to the rounding of a differently ordered Gram sum.  Operands the panel kernels cannot
-    take (A starting on an odd element) keep K3 with a Y dump + K5 in place: the stored Y is the Y the Gram matrix saw,
-    so Q is bit-identical to the fused form's."""
+                                              (1 << 14, 128, 32, True), (1 << 13, 40, 32, True), (1 << 13, 128, 32, False),
+                                              (1 << 13, 100, 32, False), (1 << 13, 20, 64, False)])
+def test_three_forms_of_stage2_up_to_128_columns(orc, m, n, prec, aligned):
+    """mrcqr_set_store_y (include/mrcqr.h): 0 = fused form (north_star's: Y stays on chip, K5 recomputes
+    it), 1 = Y stored in Q's buffer, default = the fastest measured form (fused for n16 <= 32, stored from 48 on).
+    A stored Y below n16 = 128, or with operands the panel kernels cannot take (A starting on an odd element), is K3 with
+    a Y dump + K5 in place: the stored Y is the Y the Gram matrix saw, so Q is bit-identical to the fused form's.
+    n16 = 128 with aligned operands takes the kernels of the n16 > 128 path (panel solves + SYRK): the same factorization
+    up to the rounding of a differently ordered Gram sum.  Every form against the oracle."""
     A0 = inputs.make_A(m, n, 4, 900 + n, 901 + n, "cuda")
     if aligned:
         AT = A0
@@ -149,12 +150,13 @@ def test_both_forms_of_stage2_below_128_columns(orc, m, n, prec, aligned):
         assert B.mrcqr_last_used_store_y()
         B.mrcqr_set_store_y(None)
         Q2, R2 = B.mrcqr_factor(AT, prec, 2 * n, 31)
-        assert B.mrcqr_last_used_store_y() == (aligned and n16 >= 112)      # the measured threshold (include/mrcqr.h)
+        assert B.mrcqr_last_used_store_y() == (n16 >= 48)                   # the measured threshold (include/mrcqr.h)
     finally:
         B.mrcqr_set_store_y(None)
-    assert torch.equal(Q2, Q1 if (aligned and n16 >= 112) else Q0)
-    if aligned:
+    assert torch.equal(Q2, Q1 if n16 >= 48 else Q0)
+    if aligned and n16 >= 128:
         kappa = np.linalg.cond(to_np(R0))
+        assert not torch.equal(Q0, Q1)                                       # really the other kernels
         assert np.linalg.norm(to_np(Q1) - to_np(Q0)) <= 10 * kappa * n * U
         assert np.linalg.norm(to_np(R1) - to_np(R0)) <= 10 * kappa * n * U * np.linalg.norm(to_np(R0))
     else:
