@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 import torch
 
-from helpers import U, draw_to_dev, to_np
+from helpers import U, draw_to_dev, gpu_residual_fro, to_np
 from paper_2606_18411_b200 import binding as B
 from paper_2606_18411_b200 import inputs
 from test_gpu_parity import factor_parity, relf
@@ -256,6 +256,29 @@ def test_factor_auto_escalates_only_when_needed(orc):
     Az = A.copy(); Az[:, 31] = 0.0; Az = Az[:, :31]
     rc, used, orth = B.mrcqr_factor_auto(torch.from_numpy(np.ascontiguousarray(Az.T)).cuda(), B.FP32, 62, 3, check=False)
     assert rc == 0 or rc in (2, 3)
+
+
+@pytest.mark.parametrize("m,n", [(32 * 1301, 192), (32 * 1301, 136), (32 * 2500, 128), (32 * 1301 + 8, 200)])
+def test_panel_kernels_over_several_rounds(orc, m, n):
+    """The panel kernels give every warp slab after slab (296 CTAs x 4 warps of 32 rows): m = 32 x 1301 is a second round
+    that only some warps take part in, with the landing zone re-requested across rounds; n = 192: three full panels in the
+    fused launch; n = 136: two full panels + a ragged one in its own launch; n = 128: the SYRK form below 128 < n;
+    m not a multiple of 32: the slab-kernel fallback.  CholQR2 (mrcqr_cholqr, any m) on a well-conditioned A against
+    numpy's QR: two passes through solve -> Gram -> Cholesky -> solve, the second one in place."""
+    gen = torch.Generator(device="cuda").manual_seed(n + m)
+    AT = torch.randn((n, m), dtype=torch.float64, device="cuda", generator=gen)
+    AT[: n // 2] *= 1e-2                                                  # kappa ~ 1e2: CholQR2 territory
+    QT, R = B.mrcqr_cholqr(AT, 2)
+    assert B.mrcqr_orth_error(QT) <= 1e-13
+    assert gpu_residual_fro(AT, QT, R) <= 1e-13
+    Rn = to_np(R)
+    assert np.all(np.diag(Rn) > 0) and np.array_equal(np.tril(Rn, -1), np.zeros((n, n)))
+    Rref = torch.linalg.qr(AT.T.contiguous(), mode="r").R
+    Rref = Rref * torch.sign(torch.diagonal(Rref)).unsqueeze(1)          # positive diagonal: the unique R
+    kappa = float(torch.linalg.cond(Rref))
+    assert float((R.T - Rref).norm()) <= 10 * kappa * n * U * float(Rref.norm())
+    Q2, R2 = B.mrcqr_cholqr(AT, 2)
+    assert torch.equal(QT, Q2) and torch.equal(R, R2)                     # deterministic across launches
 
 
 def test_cholqr_cholqr2_and_the_kappa_probe(orc):
