@@ -355,9 +355,9 @@ mrcqr_panel_pass(int64_t m, int ncols, int P0, const double* __restrict__ own, i
 // (st.cg / ld.cg: kept in L2, not in L1), so a solve reads its source once and writes its result once.  Same warp
 // program per (slab, panel) step as mrcqr_panel_pass; the landing zone receives the NEXT step's panel (same rows, next
 // panel; after the last panel the next round's first).  Diagonal blocks: FusedFactor (c_diag, uploaded once per solve).
-template <int FAC, int NPMAX>
+template <int FAC, int NPMAX, bool RF>
 __global__ void __launch_bounds__(PP_NW * 32, PP_CTAS)
-mrcqr_panel_fused(int64_t m, int n, int NP, const double* src, int64_t lds,      // src == dst for the in-place solve
+mrcqr_panel_fused(int64_t m, int n, int B0arg, int NP, const double* src, int64_t lds,   // src == dst for the in-place solve
                   const double2* __restrict__ frag, double* dst, int64_t ldd, int64_t nslabs)
 {
     extern __shared__ __align__(16) double Ysm[];
@@ -368,7 +368,9 @@ mrcqr_panel_fused(int64_t m, int n, int NP, const double* src, int64_t lds,     
     double* scr = Ysm + (size_t)PP_NW * (8 * PB) * LDS_ + (size_t)warp * 8 * LDS_;
     double2* Bsm = reinterpret_cast<double2*>(Ysm + (size_t)PP_NW * (8 * PB + 8) * LDS_);   // [2][PB][PP_KC][32]
     double* yw = slab + t * LDS_ + g;
-    const int ncols_last = n - 64 * (NP - 1);
+    const int B0 = RF ? B0arg : 0;                   // RF (ragged first): a panel of B0 = 2, 4 or 6 blocks was solved before this launch
+    const int C0 = 8 * B0;                           // first column of the first full panel (a ragged panel of B0 blocks precedes it)
+    const int ncols_last = n - C0 - 64 * (NP - 1);
     auto stage_chunk = [&](int c, int P0) {          // block rows [4c, 4c+4) x the PB block columns of panel P0 / 8
         double2* dstb = Bsm + (size_t)(c & 1) * PB * PP_KC * 32;
         for (int e = tid; e < PB * PP_KC * 32; e += PP_NW * 32) {
@@ -382,7 +384,7 @@ mrcqr_panel_fused(int64_t m, int n, int NP, const double* src, int64_t lds,     
         if (i < nslabs) {
             const int nc = (p == NP - 1) ? ncols_last : 64;
             if (nc < 64) zero_pad_columns<SR>(slab, nc, 64, lane);
-            load_slab<SR, true>(slab, src + (size_t)(64 * p) * (size_t)lds, lds, m, nc, i * SR, lane);
+            load_slab<SR, true>(slab, src + (size_t)(C0 + 64 * p) * (size_t)lds, lds, m, nc, i * SR, lane);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
@@ -395,9 +397,9 @@ mrcqr_panel_fused(int64_t m, int n, int NP, const double* src, int64_t lds,     
         const int64_t row0 = i * SR;
         const int64_t inext = ((r + 1) * gridDim.x + blockIdx.x) * PP_NW + warp;
         for (int p = 0; p < NP; ++p) {
-            const int P0 = 8 * p, nchunks = 2 * p;   // P0 / PP_KC
+            const int P0 = B0 + 8 * p, nchunks = (P0 + PP_KC - 1) / PP_KC;
             const int ncols = (p == NP - 1) ? ncols_last : 64;
-            const FusedFactor<FAC, NPMAX> fac(frag, p, lane);
+            const FusedFactor<FAC, NPMAX> fac(frag, B0, p, lane);
             __syncthreads();                         // previous step done with both chunk buffers; its stores are visible
             if (nchunks > 0) stage_chunk(0, P0);
             const double* yp = dst + (size_t)t * (size_t)ldd + row0 + g;
@@ -429,7 +431,8 @@ mrcqr_panel_fused(int64_t m, int n, int NP, const double* src, int64_t lds,     
                 else prefetch();
                 if (active) {
                     const double2* bs = Bsm + (size_t)(c & 1) * PB * PP_KC * 32 + lane;
-                    for (int kl = 0; kl < PP_KC; ++kl) {
+                    const int kend = (RF && P0 - PP_KC * c < PP_KC) ? P0 - PP_KC * c : PP_KC;     // !RF: P0 is a multiple of PP_KC
+                    for (int kl = 0; kl < kend; ++kl) {
                         const int Kg = PP_KC * c + kl;
                         double n0[RG], n1[RG];
                         const int Kn = (Kg + 1 < P0) ? Kg + 1 : Kg;
@@ -450,7 +453,7 @@ mrcqr_panel_fused(int64_t m, int n, int NP, const double* src, int64_t lds,     
                 }
             }
             if (active) {
-                double* o = dst + (size_t)(64 * p) * (size_t)ldd + row0 + lane;        // lane = row of the slab
+                double* o = dst + (size_t)(C0 + 64 * p) * (size_t)ldd + row0 + lane;   // lane = row of the slab
                 int left = ncols;                    // columns of the panel not yet stored (blocks arrive in order)
                 auto sink = [&](int, const double (&y)[8]) {
 #pragma unroll
@@ -616,36 +619,37 @@ int launch_panel_solve(int64_t m, int n, int fac, const double* src, int64_t lds
     int64_t grid = (nslabs + nw - 1) / nw;
     if (grid > PP_CTAS * num_sms()) grid = PP_CTAS * num_sms();
     int launches = 0;
-    const int NPF = nB / 8;                          // full 8-block panels: ONE launch (mrcqr_panel_fused)
-    if (NPF > 0) {
-        const int smem = nw * (8 * 8 + 8) * 36 * 8 + 2 * 8 * PP_KC * 512;
-        const int nf = n < 64 * NPF ? n : 64 * NPF;
-#define PF_GO(FAC_, NPM_)                                                                           \
-        { auto k = mrcqr_panel_fused<FAC_, NPM_>;                                                   \
-          cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);               \
-          k<<<(int)grid, nw * 32, smem, s>>>(m, nf, NPF, src, lds, frag, dstp, ldd, nslabs); }
-        if (NPF <= 4) { if (fac == 0) PF_GO(0, 4) else PF_GO(1, 4) }
-        else { if (fac == 0) PF_GO(0, 8) else PF_GO(1, 8) }
-#undef PF_GO
-        ++launches;
-    }
-    for (int P0 = 8 * NPF; P0 < nB; P0 += 8) {       // the ragged last panel (2, 4 or 6 blocks): a launch of its own
-        const int pb = (nB - P0 >= 8) ? 8 : nB - P0;
-        int ncols = n - 8 * P0;
-        if (ncols > 8 * pb) ncols = 8 * pb;
+    const int NPF = nB / 8, RB = nB % 8;             // full 8-block panels; blocks of the ragged panel (0, 2, 4 or 6)
+    // The ragged panel comes FIRST (blocks [0, RB)): it then needs no left-looking sweep, and the full panels that follow
+    // share one launch in which a slab's solved panels come back from L2.  (Ragged last, in a launch of its own, re-read all
+    // the solved panels from DRAM for a handful of columns: 1.2 ms for 16 columns at m = 2^21, n = 208.)
+    if (RB > 0) {
+        const int pb = RB;
+        const int ncols = n < 8 * pb ? n : 8 * pb;
         const int smem = nw * (8 * pb + 8) * 36 * 8 + 2 * pb * PP_KC * 512;
-        cudaMemcpyToSymbolAsync(c_pdiag, prep + prep_diag_offset(nB) + (size_t)P0 * PREP_DIAG, sizeof(double) * PREP_DIAG * pb,
+        cudaMemcpyToSymbolAsync(c_pdiag, prep + prep_diag_offset(nB), sizeof(double) * PREP_DIAG * pb,
                                 sizeof(double) * (size_t)fac * 8 * PREP_DIAG, cudaMemcpyDeviceToDevice, s);
-        const double* own = src + (size_t)(8 * P0) * (size_t)lds;
-        double* out = dstp + (size_t)(8 * P0) * (size_t)ldd;
 #define PP_GO(FAC_, PB_)                                                                            \
         { auto k = mrcqr_panel_pass<FAC_, PB_>;                                                     \
           cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);               \
-          k<<<(int)grid, nw * 32, smem, s>>>(m, ncols, P0, own, lds, dstp, ldd, frag, out, ldd, nslabs); }
+          k<<<(int)grid, nw * 32, smem, s>>>(m, ncols, 0, src, lds, dstp, ldd, frag, dstp, ldd, nslabs); }
 #define PP_CALL(PB_) { if (fac == 0) PP_GO(0, PB_) else PP_GO(1, PB_) }
         if (pb == 6) PP_CALL(6) else if (pb == 4) PP_CALL(4) else PP_CALL(2)
 #undef PP_CALL
 #undef PP_GO
+        ++launches;
+    }
+    if (NPF > 0) {
+        const int smem = nw * (8 * 8 + 8) * 36 * 8 + 2 * 8 * PP_KC * 512;
+#define PF_GO3(FAC_, NPM_, RF_)                                                                     \
+        { auto k = mrcqr_panel_fused<FAC_, NPM_, RF_>;                                              \
+          cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);               \
+          k<<<(int)grid, nw * 32, smem, s>>>(m, n, RB, NPF, src, lds, frag, dstp, ldd, nslabs); }
+#define PF_GO(FAC_, NPM_) { if (RB > 0) PF_GO3(FAC_, NPM_, true) else PF_GO3(FAC_, NPM_, false) }
+        if (NPF <= 4) { if (fac == 0) PF_GO(0, 4) else PF_GO(1, 4) }
+        else { if (fac == 0) PF_GO(0, 8) else PF_GO(1, 8) }
+#undef PF_GO3
+#undef PF_GO
         ++launches;
     }
     return launches;

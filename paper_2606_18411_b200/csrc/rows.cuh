@@ -27,7 +27,7 @@ namespace mrcqr {
 // [0..8) 1/R[j,j], then -R[j,jj] for j < jj, j-major.  Constant memory: the thread-per-row
 // substitution reads them with warp-uniform addresses, off the shared-memory pipe.
 #ifndef MRCQR_NO_CONST_DIAG
-__constant__ double c_diag[2][PREP_MAX_NB * PREP_DIAG];
+__constant__ __align__(16) double c_diag[2][PREP_MAX_NB * PREP_DIAG];
 #endif
 
 __host__ __device__ constexpr int diag_off(int j, int jj) { return 8 + j * 7 - j * (j - 1) / 2 + (jj - j - 1); }
@@ -168,10 +168,12 @@ struct PanelFactor {
 template <int FAC, int NPMAX>
 struct FusedFactor {
     const double2* __restrict__ frag; int p;
+    const double* dbase;                      // &c_diag[FAC][B0 * PREP_DIAG]: the panels start at block B0 (a ragged panel may come first)
     const double2* __restrict__ own;          // fragpair(frag, P0, P0, lane): the panel's own pairs start here
     unsigned jstride;                         // 32 P0: pair (P0 + K, P0 + J) sits at own + J jstride + 32 (J (J - 1) / 2 + K)
-    __device__ __forceinline__ FusedFactor(const double2* f, int p_, int lane)
-        : frag(f), p(p_), own(f + ((size_t)(8 * p_) * (8 * p_ - 1) / 2 + 8 * p_) * 32 + lane), jstride(32u * 8u * (unsigned)p_) {}
+    __device__ __forceinline__ FusedFactor(const double2* f, int B0, int p_, int lane)
+        : frag(f), p(p_), dbase(&c_diag[FAC][B0 * PREP_DIAG]),
+          own(f + ((size_t)(B0 + 8 * p_) * (B0 + 8 * p_ - 1) / 2 + B0 + 8 * p_) * 32 + lane), jstride(32u * (unsigned)(B0 + 8 * p_)) {}
     __device__ __forceinline__ double2 pair(int Kg, int Jg, int lane) const { return __ldg(fragpair(frag, Kg, Jg, lane)); }
     // in-panel pair with compile-time K, J: one multiply-add on the address instead of the triangular index arithmetic
     __device__ __forceinline__ double2 pair_in(int, int K, int J, int) const
@@ -179,14 +181,14 @@ struct FusedFactor {
     __device__ __forceinline__ void substitute(double (&y)[8], int, int K) const
     {
         switch (p) {
-            case 0: diag_substitute(y, &c_diag[FAC][(0 + K) * PREP_DIAG]); break;
-            case 1: diag_substitute(y, &c_diag[FAC][(8 + K) * PREP_DIAG]); break;
-            case 2: diag_substitute(y, &c_diag[FAC][(16 + K) * PREP_DIAG]); break;
-            case 3: diag_substitute(y, &c_diag[FAC][(24 + K) * PREP_DIAG]); break;
-            case 4: if (NPMAX > 4) diag_substitute(y, &c_diag[FAC][((NPMAX > 4 ? 32 : 0) + K) * PREP_DIAG]); break;
-            case 5: if (NPMAX > 4) diag_substitute(y, &c_diag[FAC][((NPMAX > 4 ? 40 : 0) + K) * PREP_DIAG]); break;
-            case 6: if (NPMAX > 4) diag_substitute(y, &c_diag[FAC][((NPMAX > 4 ? 48 : 0) + K) * PREP_DIAG]); break;
-            default: if (NPMAX > 4) diag_substitute(y, &c_diag[FAC][((NPMAX > 4 ? 56 : 0) + K) * PREP_DIAG]); break;
+            case 0: diag_substitute(y, dbase + (0 + K) * PREP_DIAG); break;
+            case 1: diag_substitute(y, dbase + (8 + K) * PREP_DIAG); break;
+            case 2: diag_substitute(y, dbase + (16 + K) * PREP_DIAG); break;
+            case 3: diag_substitute(y, dbase + (24 + K) * PREP_DIAG); break;
+            case 4: if (NPMAX > 4) diag_substitute(y, dbase + (32 + K) * PREP_DIAG); break;
+            case 5: if (NPMAX > 4) diag_substitute(y, dbase + (40 + K) * PREP_DIAG); break;
+            case 6: if (NPMAX > 4) diag_substitute(y, dbase + (48 + K) * PREP_DIAG); break;
+            default: if (NPMAX > 4) diag_substitute(y, dbase + (56 + K) * PREP_DIAG); break;
         }
     }
 };
