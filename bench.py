@@ -335,7 +335,7 @@ def dominant_kernel(cfg, stages, hbm_peak, how):
     n16 < 128: K3 (8n bytes read (+ 8n written when Y is stored), 2n^2 flops per row) or K5 (16n bytes; 2n^2 flops per row
     in the fused form, n^2 when it solves a stored Y), one launch = all m rows.
     n16 >= 128: one triangular solve = one mrcqr_panel_fused launch over the full 64-column panels (+ one mrcqr_panel_pass
-    launch for a ragged last panel; n^2 flops, 16n bytes per row) or the SYRK launch (n^2 flops, 8n bytes per row);
+    launch for a ragged first panel; n^2 flops, 16n bytes per row) or the SYRK launch (n^2 flops, 8n bytes per row);
     `kernel_ms` is the duration of the stage."""
     m, n = cfg["m"], cfg["n"]
     if not syrk_form(n):
@@ -344,7 +344,7 @@ def dominant_kernel(cfg, stages, hbm_peak, how):
                 "k5_form_q": ("mrcqr_k5_formq", 16.0 * m * n, (1.0 if sy else 2.0) * m * n * n)}
     else:
         ragged = ((n + 15) // 16 * 16) % 64 != 0
-        tail = (lambda f: " + mrcqr_panel_pass<%d> for the ragged last panel" % f if ragged else "")
+        tail = (lambda f: " + mrcqr_panel_pass<%d> for the ragged first panel" % f if ragged else "")
         cand = {"k3_gram": ("mrcqr_panel_fused<0> (solve with R_s, all full panels in one launch)" + tail(0), 16.0 * m * n, 1.0 * m * n * n),
                 "gram_reduce": ("mrcqr_syrk", 8.0 * m * n, 1.0 * m * n * n),
                 "k5_form_q": ("mrcqr_panel_fused<1> (solve with R_c, all full panels in one launch)" + tail(1), 16.0 * m * n, 1.0 * m * n * n)}
@@ -366,7 +366,7 @@ def dominant_kernel(cfg, stages, hbm_peak, how):
         kname, "mrcqr_panel_fused<0" if stage == "k3_gram" else "mrcqr_panel_fused<1")
     traffic = ncu_traffic(cfg["name"], tkey)
     if traffic is not None and tkey.startswith("mrcqr_panel_fused") and ((n + 15) // 16 * 16) % 64 != 0:
-        rest = ncu_traffic(cfg["name"], tkey.replace("fused", "pass"))      # the ragged last panel's own launch
+        rest = ncu_traffic(cfg["name"], tkey.replace("fused", "pass"))      # the ragged first panel's own launch
         traffic = None if rest is None else traffic + rest
     roof.update({"traffic": traffic, "kernel": kname, "stage": stage, "kernel_ms": dom_ms, "algorithmic_bytes": dom_bytes,
                  "algorithmic_flops": dom_flops, "hbm_gbs_achieved": dom_bytes / (dom_ms * 1e-3) / 1e9,
