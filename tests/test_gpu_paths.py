@@ -94,6 +94,9 @@ def test_fft_sketch_tile_widths_match_oracle(orc, m, n, s, prec, tol):
     (1 << 12, 250, 5, 32),     # the same with a ragged last panel (58 columns)
     (1 << 12, 180, 4, 32),     # 3 panels (n16 = 192), last one ragged
     (1 << 11, 500, 3, 64),     # 8 panels, last one ragged
+    (1 << 12, 200, 4, 32),     # n16 = 208: a ragged first panel of 2 blocks + 3 full ones; SYRK with 10 live blocks in the last panel
+    (1 << 11, 330, 3, 64),     # n16 = 336: P = 3 SYRK blocks, 10 live blocks, ragged first panel of 2 blocks + 5 full ones
+    (1 << 11, 304, 6, 32),     # n16 = 304: P = 3, 6 live blocks, ragged first panel of 6 blocks
 ])
 def test_store_y_path_factorization(orc, m, n, expo, prec):
     AT = inputs.make_A(m, n, expo, 500 + n, 501 + n, "cuda")
