@@ -432,6 +432,7 @@ mrcqr_panel_fused(int64_t m, int n, int B0arg, int NP, const double* src, int64_
                 if (active) {
                     const double2* bs = Bsm + (size_t)(c & 1) * PB * PP_KC * 32 + lane;
                     const int kend = (RF && P0 - PP_KC * c < PP_KC) ? P0 - PP_KC * c : PP_KC;     // !RF: P0 is a multiple of PP_KC
+#pragma unroll (RF ? 1 : (NPMAX == 4 ? 2 : 4))      // up to 4 panels the kernel is bound by its code size more than by the sweep (C3: 5.09 -> 4.95 ms)
                     for (int kl = 0; kl < kend; ++kl) {
                         const int Kg = PP_KC * c + kl;
                         double n0[RG], n1[RG];
