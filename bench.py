@@ -642,7 +642,11 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C3", choices=["C0", "C1", "C2", "C3", "C4n16", "C4n32", "C4n64", "C4n128", "C4n256", "C4n512"])
+    def config_name(v):                  # BASELINE.json configs[0..3], or a point of the column sweep: C4n<any n in 1 .. 512>
+        if v in ("C0", "C1", "C2", "C3") or (v.startswith("C4n") and v[3:].isdigit() and 1 <= int(v[3:]) <= 512):
+            return v
+        raise argparse.ArgumentTypeError("C0 | C1 | C2 | C3 | C4n<n>, 1 <= n <= 512")
+    ap.add_argument("--config", default="C3", type=config_name)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-points", action="store_true", help="skip the other configurations carried under \"points\"")
     ap.add_argument("--traffic-from", default=None, help="ncu --page raw --csv file: record per-kernel DRAM bytes of --config in profiles/r02_traffic.json")
