@@ -1,9 +1,13 @@
 // k35_rows.cu -- the two passes over A that dominate MRCQR ("TRSM x2" is 56-74 %
 // of the paper's runtime):
 //   K3  mrcqr_k3_gram   Algorithm 2 step 7 fused with Algorithm 1 step 1:
-//                       per row y = a Rs^-1 (solve_slab), G += y^T y on DMMA; Y never leaves the SM.
-//   K5  mrcqr_k5_formq  Algorithm 1 step 3: y recomputed bit-identically,
-//                       q = y Rc^-1, Q streamed out.  Warps are fully independent (no CTA barrier).
+//                       per row y = a Rs^-1 (solve_slab), G += y^T y on DMMA; Y never leaves the SM
+//                       (fused form), or is also written to Q's buffer (dump form, n16 >= 48 by default).
+//   K5  mrcqr_k5_formq  Algorithm 1 step 3: y recomputed bit-identically (fused form) or
+//                       read back (dump form), q = y Rc^-1, Q streamed out.  Warps are fully independent.
+//   mrcqr_panel_fused / mrcqr_panel_pass  the triangular solves of the store-Y form (n16 >= 128): 64-column
+//                       panels in accumulator registers, all full panels of a solve in one launch.
+// Which form runs for which n: api.cu, enqueue_stage23.
 // Persistent CTAs, static slab -> warp map, so every sum has a fixed order: results are
 // deterministic run to run.
 #include "rows.cuh"
@@ -219,8 +223,10 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
     }
 }
 
-// ---- panel passes (n16 > 128, store-Y form) -------------------------------------------------------------
-// One launch solves ONE panel of PB <= 8 column blocks for all rows: every warp streams 32-row slabs
+// ---- panel kernels (store-Y form) -------------------------------------------------------------------------
+// mrcqr_panel_pass: one launch solves ONE panel of PB <= 8 column blocks for all rows (today only the ragged FIRST
+// panel of a solve, PB = 2, 4 or 6, P0 = 0; the full panels share mrcqr_panel_fused below, which is this kernel with a
+// loop over the panels around the body of a round): every warp streams 32-row slabs
 // (RG = 4), keeps the panel in accumulator registers, adds the contributions of the already solved
 // panels with a left-looking sweep whose A fragments come straight from global memory (lane (g, t)
 // reads row g of column t: 64 contiguous bytes per column, every sector fully used; one step
