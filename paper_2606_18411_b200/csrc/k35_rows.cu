@@ -386,11 +386,12 @@ mrcqr_panel_fused(int64_t m, int n, int B0arg, int NP, const double* src, int64_
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
+    const uint64_t once = l2_evict_first_policy();
     auto request = [&](int64_t i, int p) {           // panel p of slab i into the landing zone (one commit group)
         if (i < nslabs) {
             const int nc = (p == NP - 1) ? ncols_last : 64;
             if (nc < 64) zero_pad_columns<SR>(slab, nc, 64, lane);
-            load_slab<SR, true>(slab, src + (size_t)(C0 + 64 * p) * (size_t)lds, lds, m, nc, i * SR, lane);
+            load_slab_once<SR>(slab, src + (size_t)(C0 + 64 * p) * (size_t)lds, lds, m, nc, i * SR, lane, once);   // read once; the solved panels stay in L2
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };

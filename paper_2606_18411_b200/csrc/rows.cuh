@@ -46,6 +46,18 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src,
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gmem_src), "r"(src_bytes) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// the same with an L2 eviction policy (createpolicy): for data that is read once while other lines should stay in L2
+__device__ __forceinline__ void cp_async16_hint(void* smem_dst, const void* gmem_src, int src_bytes, uint64_t policy)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;" ::"r"(d), "l"(gmem_src), "r"(src_bytes), "l"(policy) : "memory");
+}
+__device__ __forceinline__ uint64_t l2_evict_first_policy()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
 
 // Warp-cooperative load of rows [row0, row0+SR) x n columns of A into this warp's slab; zero fill
 // for rows >= m.  The padding columns n..n16-1 are zeroed once by zero_pad_columns().  VEC (A, lda
@@ -73,6 +85,23 @@ __device__ __forceinline__ void load_slab(double* slab, const double* __restrict
             const int64_t r = row0 + rr;
             slab[col * LDS_ + rr] = (r < m) ? __ldcs(A + (size_t)col * (size_t)lda + r) : 0.0;
         }
+    }
+}
+
+// load_slab<SR, true> with every line marked evict-first in L2 (a source that is read exactly once)
+template <int SR>
+__device__ __forceinline__ void load_slab_once(double* slab, const double* __restrict__ A, int64_t lda,
+                                               int64_t m, int n, int64_t row0, int lane, uint64_t policy)
+{
+    constexpr int LDS_ = SR + 4, H = SR / 2;
+    const int64_t left = m - row0;
+#pragma unroll 8
+    for (int e = lane; e < n * H; e += 32) {
+        const int col = e / H, r2 = (e % H) * 2;
+        const int64_t avail = left - r2;
+        const int bytes = avail >= 2 ? 16 : (avail == 1 ? 8 : 0);
+        const double* src = A + (size_t)col * (size_t)lda + row0 + (bytes ? r2 : 0);
+        cp_async16_hint(slab + col * LDS_ + r2, src, bytes, policy);
     }
 }
 
