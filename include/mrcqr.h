@@ -269,6 +269,26 @@ int mrcqr_set_sketch_reim(int on);
  */
 int mrcqr_set_graph(int on);
 
+/*
+ * Calls in flight (repeated-call mode: the QR inside a block-Arnoldi or power-iteration loop, whose
+ * caller does not need the status of one factorization before it enqueues the next).  mrcqr_factor_async takes the
+ * arguments of mrcqr_factor (device pointers, same layouts, same checks), enqueues Algorithm 2 on `stream` and returns
+ * WITHOUT synchronising: 0 = enqueued, < 0 = argument -rc invalid, MRCQR_ERR_CUDA.  Nothing is allocated once the
+ * context's workspace fits the shape and its ring of 8 pinned bin buffers fits s.  Q and R are ready when the work
+ * enqueued on `stream` has run.  Same kernels, same results bit for bit as mrcqr_factor.
+ * The run-time status (MRCQR_ERR_OVERFLOW / _SINGULAR / _BREAKDOWN and its column) is NOT returned per call: the
+ * device status block keeps the FIRST error of the calls in flight, and the later calls still run in full.
+ * mrcqr_wait synchronises the stream of the pending calls, returns that status (0 if every call was clean), writes its
+ * column to *info_host (may be NULL; also mrcqr_last_info) and clears it; with nothing pending it returns 0 at once.
+ * All calls between two waits share the context's workspace and must use ONE stream (a call on another stream, or one
+ * whose workspace must grow, first waits for the pending ones and carries their status over).  Call mrcqr_wait before
+ * any other entry point of the same context: a synchronous entry point drains the pending calls and DROPS their status.
+ * mrcqr_set_timing / mrcqr_set_graph do not apply to these calls.
+ */
+int mrcqr_factor_async(int64_t m, int n, int64_t lda, const double* A, double* Q, double* R,
+                       mrcqr_prec_t sketch_prec, int s, uint64_t seed, void* stream);
+int mrcqr_wait(int* info_host);
+
 /* 1 if the last mrcqr_factor / mrcqr_factor_host call replayed (or captured and replayed) a CUDA graph, else 0. */
 int mrcqr_last_used_graph(void);
 

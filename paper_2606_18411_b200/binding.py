@@ -48,6 +48,8 @@ def lib():
         L.mrcqr_precondition_gram.argtypes = [i64, ci, i64, vp, vp, vp, vp, vp]
         L.mrcqr_form_q.argtypes = [i64, ci, i64, vp, vp, vp, i64, vp, vp, vp]
         L.mrcqr_factor.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64, vp]
+        L.mrcqr_factor_async.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64, vp]
+        L.mrcqr_wait.argtypes = [vp]
         L.mrcqr_factor_batched.argtypes = [ci, i64, ci, i64, i64, vp, i64, vp, vp, ci, ci, u64, vp, vp]
         L.mrcqr_factor_host.argtypes = [i64, ci, i64, vp, vp, vp, ci, ci, u64]
         L.mrcqr_workspace_bytes.restype = C.c_size_t
@@ -66,7 +68,7 @@ def lib():
         L.mrcqr_last_timing.argtypes = [vp]
         for f in ("mrcqr_create", "mrcqr_set_current", "mrcqr_destroy", "mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
                   "mrcqr_factor_host", "mrcqr_last_info", "mrcqr_last_launch_count", "mrcqr_debug_dump_y",
-                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim"):
+                  "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim", "mrcqr_factor_async", "mrcqr_wait"):
             getattr(L, f).restype = ci
         _lib = L
     return _lib
@@ -75,7 +77,7 @@ def lib():
 EXPORTS = ["mrcqr_create", "mrcqr_set_current", "mrcqr_destroy", "mrcqr_draw", "mrcqr_draw_device", "mrcqr_last_used_graph", "mrcqr_factor_batched", "mrcqr_sketch", "mrcqr_precondition_gram", "mrcqr_form_q", "mrcqr_factor",
            "mrcqr_factor_host", "mrcqr_workspace_bytes", "mrcqr_last_info", "mrcqr_last_launch_count",
            "mrcqr_debug_dump_y", "mrcqr_shutdown", "mrcqr_set_timing", "mrcqr_last_timing", "mrcqr_set_store_y", "mrcqr_orth_error", "mrcqr_factor_auto", "mrcqr_cholqr", "mrcqr_kappa_probe", "mrcqr_set_graph", "mrcqr_set_sketch_reim",
-           "mrcqr_orth_error_noalloc", "mrcqr_last_used_store_y"]
+           "mrcqr_orth_error_noalloc", "mrcqr_last_used_store_y", "mrcqr_factor_async", "mrcqr_wait"]
 
 STAGES = ["k1_srtt", "k2_sketch_qr", "prep_rs", "k3_gram", "gram_reduce", "k4_chol", "k5_form_q"]
 
@@ -189,6 +191,23 @@ def mrcqr_factor(AT, prec, s, seed, QT=None, R=None, stream=None, check=True):
         return rc
     _chk(rc)
     return QT, R
+
+
+def mrcqr_factor_async(AT, prec, s, seed, QT, R, stream=None):
+    """mrcqr_factor without the synchronisation: enqueues and returns; the status comes from mrcqr_wait()."""
+    m, n, lda, pA = _mat(AT)
+    _out(QT, AT)
+    _chk(lib().mrcqr_factor_async(m, n, lda, pA, QT.data_ptr(), R.data_ptr(), prec, s, seed, _stream(stream)))
+
+
+def mrcqr_wait(check=True):
+    """Synchronises the pending mrcqr_factor_async calls; returns (code, info) of the first error among them (0, 0 if
+    none) or raises it when check=True."""
+    info = C.c_int(0)
+    rc = lib().mrcqr_wait(C.byref(info))
+    if check:
+        _chk(rc)
+    return rc, info.value
 
 
 def mrcqr_factor_batched(AB, prec, s, seed, QB=None, RB=None, stream=None, check=True):

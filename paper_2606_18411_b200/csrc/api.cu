@@ -71,6 +71,7 @@ static Layout make_layout(int64_t m, int n, int s, int prec)
     return L;
 }
 
+constexpr int ASYNC_RING = 8;          // pinned bin buffers of mrcqr_factor_async calls in flight
 struct Ctx {
     char* ws = nullptr; size_t ws_bytes = 0;
     int* h_status = nullptr;                 // pinned, 2 ints
@@ -89,6 +90,12 @@ struct Ctx {
     bool use_graph = false;
     cudaGraphExec_t gexec = nullptr; int glaunches = 0; uint64_t* h_seed = nullptr;
     struct { int64_t m, lda; int n, prec, s; const void *A, *Q, *R, *ws, *hidx; int store_y; bool reim; } gkey = {};
+    // mrcqr_factor_async: calls in flight.  Each one owns a slot of a ring of pinned bin buffers until the event recorded
+    // behind its host-to-device copy has completed; the run-time status stays in the device status block (first error
+    // wins) until mrcqr_wait reads and clears it.
+    int64_t* h_ring = nullptr; size_t h_ring_cap = 0; int ring_pos = 0;
+    cudaEvent_t ring_ev[ASYNC_RING] = {}; bool ring_busy[ASYNC_RING] = {};
+    int async_pending = 0; cudaStream_t async_stream = nullptr; size_t async_status_off = 0; bool in_async = false;
 };
 // Every entry point works on the calling thread's CURRENT context: the process default one, or the handle made current
 // with mrcqr_set_current (mrcqr_create / mrcqr_destroy).  A context owns its workspace, staging buffers, settings,
@@ -149,6 +156,9 @@ static bool device_ok()
 static bool ensure_ws(size_t bytes)
 {
     if (!g.h_status && cudaMallocHost(&g.h_status, 64) != cudaSuccess) return false;   // [0..1] status, [2..3] a double
+    // a synchronous entry point while mrcqr_factor_async calls are in flight: they finish first (the workspace is shared);
+    // their status is dropped with the pending count, as the header says
+    if (g.async_pending > 0 && !g.in_async) { cudaStreamSynchronize(g.async_stream); g.async_pending = 0; }
     if (bytes <= g.ws_bytes) return true;
     if (g.ws) { cudaDeviceSynchronize(); drop_graph(); cudaFree(g.ws); g.ws = nullptr; g.ws_bytes = 0; }
     if (cudaMalloc(&g.ws, bytes) != cudaSuccess) { cudaGetLastError(); return false; }
@@ -295,6 +305,8 @@ static void free_ctx(Ctx& c)
     if (c.ws) cudaFree(c.ws);
     if (c.h_status) cudaFreeHost(c.h_status);
     if (c.h_idx) cudaFreeHost(c.h_idx);
+    if (c.h_ring) cudaFreeHost(c.h_ring);
+    for (int i = 0; i < ASYNC_RING; ++i) if (c.ring_ev[i]) cudaEventDestroy(c.ring_ev[i]);
     if (c.ev_ok) for (int i = 0; i < 8; ++i) cudaEventDestroy(c.ev[i]);
     if (c.hA) cudaFree(c.hA);
     if (c.hQ) cudaFree(c.hQ);
@@ -491,21 +503,27 @@ static int enqueue_stage23(const Layout& L, int64_t m, int n, int64_t lda, const
 // enqueues steps 1-9 on st.  seed_dev != nullptr: the seed and the bins are read from seed_dev / the pinned
 // staging buffers when the work RUNS (graph capture); otherwise they are taken now.
 static int enqueue_factor(const Layout& L, int64_t m, int n, int64_t lda, const double* A, int64_t ldq, double* Q,
-                          double* R, int prec, int s, uint64_t seed, const uint64_t* seed_dev, cudaStream_t st, bool tm)
+                          double* R, int prec, int s, uint64_t seed, const uint64_t* seed_dev, cudaStream_t st, bool tm,
+                          const int64_t* h_bins = nullptr, bool reset_status = true)
 {
     Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
+    Status* stat0 = reset_status ? stat : nullptr;      // the first kernel clears the status block (not between async calls)
+    if (!h_bins) h_bins = g.h_idx;
     uint64_t* signs = reinterpret_cast<uint64_t*>(g.ws + L.signs);
     int64_t* idx = reinterpret_cast<int64_t*>(g.ws + L.idx);
     double* Rs = reinterpret_cast<double*>(g.ws + L.Rs);
     // Algorithm 2 step 1: bins on the host (s values), sign words on the device (m bits)
-    cudaMemcpyAsync(idx, g.h_idx, sizeof(int64_t) * (size_t)s, cudaMemcpyHostToDevice, st);
+    cudaMemcpyAsync(idx, h_bins, sizeof(int64_t) * (size_t)s, cudaMemcpyHostToDevice, st);
     const int64_t nw = (m + 63) / 64;
-    if (seed_dev) mrcqr_draw_signs_p<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed_dev, nw, signs, stat);
-    else mrcqr_draw_signs<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed, nw, signs, stat);
-    int k = 1;
+    // sign words: by the draw kernel, or (register radix-16 form of K1, seed known now) by K1 itself where it uses them
+    const bool k1_draws = !seed_dev && k1_generates_signs(m, g.reim);
+    int k = 0;
+    if (seed_dev) { mrcqr_draw_signs_p<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed_dev, nw, signs, stat0); k = 1; }
+    else if (!k1_draws) { mrcqr_draw_signs<<<(unsigned)((nw + 255) / 256), 256, 0, st>>>(seed, nw, signs, stat0); k = 1; }
     double* As = reinterpret_cast<double*>(g.ws + L.As);
     if (tm) cudaEventRecord(g.ev[0], st);
-    k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st, g.reim);     // steps 2-4
+    k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st, g.reim,
+                        k1_draws ? &seed : nullptr, reset_status);                                   // steps 2-4
     if (tm) cudaEventRecord(g.ev[1], st);
     k += launch_k2_sketch_qr(As, g.reim ? 2 * s : s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
                              reinterpret_cast<double*>(g.ws + L.betas), stat, st);                              // steps 5-6
@@ -575,6 +593,82 @@ extern "C" int mrcqr_factor(int64_t m, int n, int64_t lda, const double* A, doub
     if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX || (g.reim && 2 * s > S_MAX)) return -8;
     if (!device_ok()) return MRCQR_ERR_CUDA;
     return factor_device(m, n, lda, A, lda, Q, R, (int)sketch_prec, s, seed, (cudaStream_t)stream);
+}
+
+// ---- calls in flight (repeated-call mode) ---------------------------------------------------------
+// mrcqr_factor_async enqueues the same work as mrcqr_factor and returns; mrcqr_wait synchronises and reports.
+static int wait_async(int* info_host)
+{
+    if (g.async_pending == 0) { if (info_host) *info_host = 0; return 0; }
+    cudaStream_t st = g.async_stream;
+    Status* stat = reinterpret_cast<Status*>(g.ws + g.async_status_off);
+    cudaMemcpyAsync(g.h_status, stat, 8, cudaMemcpyDeviceToHost, st);
+    mrcqr_reset_status<<<1, 1, 0, st>>>(stat);
+    g.async_pending = 0;
+    for (int i = 0; i < ASYNC_RING; ++i) g.ring_busy[i] = false;
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) return MRCQR_ERR_CUDA;
+    g.last_info = g.h_status[1];
+    if (info_host) *info_host = g.h_status[1];
+    return g.h_status[0];
+}
+
+extern "C" int mrcqr_wait(int* info_host) { return device_ok() ? wait_async(info_host) : MRCQR_ERR_CUDA; }
+
+extern "C" int mrcqr_factor_async(int64_t m, int n, int64_t lda, const double* A, double* Q, double* R,
+                                  mrcqr_prec_t sketch_prec, int s, uint64_t seed, void* stream)
+{
+    if (n < 1 || n > N_MAX) return -2;
+    if (!is_pow2(m) || m < n || m < 32) return -1;
+    if (lda < m) return -3;
+    if (!A) return -4;
+    if (!Q) return -5;
+    if (!R) return -6;
+    if (!prec_ok((int)sketch_prec)) return -7;
+    if (s <= 0) s = 3 * n;
+    if (s < n || (int64_t)s > m / 2 + 1 || s > S_MAX || (g.reim && 2 * s > S_MAX)) return -8;
+    if (!device_ok()) return MRCQR_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    Layout L = make_layout(m, n, s, (int)sketch_prec);
+    // The calls in flight share the context's workspace, ordered by their stream: another stream, or a workspace that
+    // has to grow (or whose status block would move), first drains what is pending (its status is kept: see below).
+    int carried = 0, carried_info = 0;
+    if (g.async_pending > 0 && (st != g.async_stream || L.total > g.ws_bytes || L.status != g.async_status_off)) {
+        carried = wait_async(&carried_info);
+        if (carried == MRCQR_ERR_CUDA) return carried;
+    }
+    g.in_async = true;
+    const bool ws_ok = ensure_ws(L.total);
+    g.in_async = false;
+    if (!ws_ok) return MRCQR_ERR_CUDA;
+    if ((size_t)s > g.h_ring_cap) {                              // (re)allocate the ring: nothing is in flight on a smaller one
+        if (g.async_pending > 0) { const int c = wait_async(&carried_info); if (c == MRCQR_ERR_CUDA) return c; if (!carried) carried = c; }
+        if (g.h_ring) cudaFreeHost(g.h_ring);
+        g.h_ring = nullptr; g.h_ring_cap = 0;
+        const size_t cap = std::max<size_t>((size_t)s, 256);
+        if (cudaMallocHost(&g.h_ring, sizeof(int64_t) * cap * ASYNC_RING) != cudaSuccess) { cudaGetLastError(); g.h_ring = nullptr; return MRCQR_ERR_CUDA; }
+        g.h_ring_cap = cap;
+    }
+    const int slot = g.ring_pos;
+    g.ring_pos = (g.ring_pos + 1) % ASYNC_RING;
+    if (!g.ring_ev[slot] && cudaEventCreateWithFlags(&g.ring_ev[slot], cudaEventDisableTiming) != cudaSuccess) return MRCQR_ERR_CUDA;
+    if (g.ring_busy[slot] && cudaEventSynchronize(g.ring_ev[slot]) != cudaSuccess) return MRCQR_ERR_CUDA;   // its copy has run
+    int64_t* bins = g.h_ring + (size_t)slot * g.h_ring_cap;
+    draw_bins_host(m, s, seed, bins);
+    Status* stat = reinterpret_cast<Status*>(g.ws + L.status);
+    if (g.async_pending == 0) {
+        mrcqr_reset_status<<<1, 1, 0, st>>>(stat);
+        if (carried) {                                           // an error of the drained calls is not lost
+            g.h_status[4] = carried; g.h_status[5] = carried_info;      // pinned; rewritten only after another drain (a sync)
+            cudaMemcpyAsync(stat, g.h_status + 4, 8, cudaMemcpyHostToDevice, st);
+        }
+    }
+    const int k = enqueue_factor(L, m, n, lda, A, lda, Q, R, (int)sketch_prec, s, seed, nullptr, st, false, bins, false);
+    // the bins are on the device once the first kernels have run; the slot is free from this event on
+    cudaEventRecord(g.ring_ev[slot], st);
+    g.ring_busy[slot] = true;
+    g.async_stream = st; g.async_status_off = L.status; ++g.async_pending;
+    g.last_launches = k; g.last_graph = false;
+    return cudaGetLastError() == cudaSuccess ? 0 : MRCQR_ERR_CUDA;
 }
 
 // ||I - Q^T Q||_F on the device: DMMA SYRK of Q (deterministic row split, chains flushed every 1024 rows) + norm

@@ -23,6 +23,7 @@
 // T = float serves p = FP16 (inputs and outputs rounded to FP16, FP32 arithmetic) and p = FP32;
 // T = double serves p = FP64.  No fast-math intrinsics: twiddles come from sincospi.
 #include "mrcqr_internal.cuh"
+#include <cstdlib>
 #include <cuda_fp16.h>
 
 namespace mrcqr {
@@ -70,6 +71,10 @@ struct K1Params {
     int vec;                      // A and lda allow 16-byte loads
     int reim;                     // Re+Im variant: 2s sketch rows, Im X[S] below Re X[S]
     int dtab;                     // the per-bin step twiddles W_m^k fit in shared memory (computed once per CTA)
+    // mrcqr_factor (register radix-16 form only): the sign words are splitmix64_at(seed, word) evaluated where they are
+    // used instead of read from the array a draw kernel wrote (a0: the same bits; one launch less), and the
+    // status block is cleared here, by the first kernel of the call
+    int gen_signs; uint64_t seed; Status* st_reset;
 };
 
 template <typename T, int PREC, int W, bool REIM>
@@ -296,6 +301,36 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
     const int col = blockIdx.x / p.chunks, chunk = blockIdx.x % p.chunks;
     const double* colA = A + (size_t)col * (size_t)p.lda;
 
+    const int tile_lo = chunk * p.tiles_per_chunk;
+    const int tile_hi = min(p.tiles_per_col, tile_lo + p.tiles_per_chunk);
+    double2 v[16];
+    unsigned sw = 0;                                                                // sign word of row a = lane % 16 (this half warp's b)
+    // rows a = A0 .. A0+7 of tile tl (the request is split in two so that at most 8 rows are in flight beside a butterfly)
+    auto fetch = [&](int tl, int A0) {
+        const int64_t t2_0 = (int64_t)tl * (2 * F16_W);
+        if (p.vec) {
+            const double2* src = reinterpret_cast<const double2*>(colA + t2_0) + u;
+            const int64_t m2h = p.m2 >> 1;
+#pragma unroll
+            for (int a = 0; a < 8; ++a) v[A0 + a] = __ldcs(src + (int64_t)(16 * (A0 + a) + b) * m2h);
+        } else {
+            const double* src = colA + t2_0 + 2 * u;
+#pragma unroll
+            for (int a = 0; a < 8; ++a) {
+                const int64_t off = (int64_t)(16 * (A0 + a) + b) * p.m2;
+                v[A0 + a] = make_double2(__ldcs(src + off), __ldcs(src + off + 1));
+            }
+        }
+        if (A0 == 0) {                                                              // m2 % 32 == 0: one word per row and tile
+            const int64_t w32 = ((int64_t)(16 * (lane & 15) + b) * p.m2 + t2_0) >> 5;
+            sw = p.gen_signs ? (unsigned)(splitmix64_at(p.seed, (uint64_t)(w32 >> 1)) >> (32 * (int)(w32 & 1))) : __ldg(signs32 + w32);
+        }
+    };
+    if (p.st_reset && blockIdx.x == 0 && tid == 0) { p.st_reset->code = 0; p.st_reset->info = 0; }
+    // the first tile is requested BEFORE the tables below are built: a CTA of a narrow matrix owns only a few tiles
+    // (n = 16: three), and its set-up would otherwise sit in front of the first HBM round trip
+    if (tile_lo < tile_hi) { fetch(tile_lo, 0); fetch(tile_lo, 8); }
+
     for (int e = tid; e < F16_M1; e += F16_NT) {
         double sn, cs;
         sincospi(-2.0 * (double)e / (double)F16_M1, &sn, &cs);
@@ -340,29 +375,6 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
         }
     }
 
-    const int tile_lo = chunk * p.tiles_per_chunk;
-    const int tile_hi = min(p.tiles_per_col, tile_lo + p.tiles_per_chunk);
-    double2 v[16];
-    unsigned sw = 0;                                                                // sign word of row a = lane % 16 (this half warp's b)
-    // rows a = A0 .. A0+7 of tile tl (the request is split in two so that at most 8 rows are in flight beside a butterfly)
-    auto fetch = [&](int tl, int A0) {
-        const int64_t t2_0 = (int64_t)tl * (2 * F16_W);
-        if (p.vec) {
-            const double2* src = reinterpret_cast<const double2*>(colA + t2_0) + u;
-            const int64_t m2h = p.m2 >> 1;
-#pragma unroll
-            for (int a = 0; a < 8; ++a) v[A0 + a] = __ldcs(src + (int64_t)(16 * (A0 + a) + b) * m2h);
-        } else {
-            const double* src = colA + t2_0 + 2 * u;
-#pragma unroll
-            for (int a = 0; a < 8; ++a) {
-                const int64_t off = (int64_t)(16 * (A0 + a) + b) * p.m2;
-                v[A0 + a] = make_double2(__ldcs(src + off), __ldcs(src + off + 1));
-            }
-        }
-        if (A0 == 0) sw = __ldg(signs32 + (((int64_t)(16 * (lane & 15) + b) * p.m2 + t2_0) >> 5));   // m2 % 32 == 0: one word per row and tile
-    };
-    if (tile_lo < tile_hi) { fetch(tile_lo, 0); fetch(tile_lo, 8); }
     for (int tl = tile_lo; tl < tile_hi; ++tl) {
         const int64_t t2_0 = (int64_t)tl * (2 * F16_W);
         Cx<T> x[16];
@@ -444,6 +456,51 @@ __global__ void mrcqr_k1_finalize(K1Params p, const double* __restrict__ partial
     As[e] = v;
 }
 
+// The same for a column cut into MANY chunks (a narrow matrix: n = 16 has 86 of them, and a thread that adds them one after
+// the other waits for one L2 round trip each: 14 us).  32 elements x 32 chunk groups per CTA: group q adds chunks q, q + 32,
+// ... in ascending order, the groups are combined by a fixed binary tree in shared memory (the layout of
+// mrcqr_reduce_partials).  Deterministic; the order differs from the plain loop's only in how the chunks are bracketed.
+template <int PREC>
+__global__ void __launch_bounds__(1024)
+mrcqr_k1_finalize_wide(K1Params p, const double* __restrict__ partial, double* __restrict__ As, Status* st)
+{
+    __shared__ double sm[32][33];
+    const int el = threadIdx.x & 31, q = threadIdx.x >> 5;
+    const int e = blockIdx.x * 32 + el;
+    const int rows = p.reim ? 2 * p.s : p.s, nacc = p.reim ? 2 : 1;
+    const bool live = e < rows * p.n;
+    double acc = 0.0;
+    if (live) {
+        const int r = e % rows, j = e / rows;
+        const int i = r % p.s, part = r / p.s;
+        const size_t cs = (size_t)nacc * p.s;
+        const double* src = partial + ((size_t)j * p.chunks) * cs + (size_t)part * p.s + i;
+        for (int c = q; c < p.chunks; c += 32) acc += src[(size_t)c * cs];
+    }
+    sm[q][el] = acc;
+    __syncthreads();
+#pragma unroll
+    for (int h = 16; h > 0; h >>= 1) {
+        if (q < h) sm[q][el] += sm[q + h][el];
+        __syncthreads();
+    }
+    if (q == 0 && live) {
+        double v = sm[0][el] * sqrt((double)p.s / (double)p.m);
+        if (PREC == 16) v = (double)__half2float(__double2half(v));
+        else if (PREC == 32) v = (double)__double2float_rn(v);
+        if (isnan(v) || isinf(v)) report(st, 1, e / rows);
+        As[e] = v;
+    }
+}
+
+template <int PREC>
+static void k1_finalize(const K1Params& p, const double* partial, double* As, Status* st, cudaStream_t stream)
+{
+    const int total = (p.reim ? 2 : 1) * p.s * p.n;
+    if (p.chunks > 8) mrcqr_k1_finalize_wide<PREC><<<(total + 31) / 32, 1024, 0, stream>>>(p, partial, As, st);
+    else mrcqr_k1_finalize<PREC><<<(total + 255) / 256, 256, 0, stream>>>(p, partial, As, st);
+}
+
 // tile width W of the shared-memory radix-4 form (complex elements = 2W consecutive t2 of one column).  That form now
 // serves only short columns (m < 8192) and the Re+Im variant: 32-wide tiles, narrower ones where the column is too short
 // for them (m >= 32: 2W <= m / 2).
@@ -462,6 +519,7 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec, int re
 {
     K1Params p;
     p.m = m; p.lda = lda; p.n = n; p.s = s; p.reim = reim;
+    p.gen_signs = 0; p.seed = 0; p.st_reset = nullptr;
     const bool f16 = k1_fft16_usable(m, reim);
     const int K1_W = f16 ? F16_W : k1_tile_w(m, prec, s, reim);
     const int m1max = f16 ? F16_M1 : ((prec == 64) ? 128 : 256) * (32 / K1_W);    // 68 KB tile (W = 8: 74 KB)
@@ -471,7 +529,8 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec, int re
     p.m1 = (int)m1; p.m2 = m / m1;
     p.log_m1 = 0; while ((1 << p.log_m1) < p.m1) ++p.log_m1;
     p.tiles_per_col = (int)(p.m2 / (2 * K1_W));
-    int chunks = (12 * num_sms() + n - 1) / n;
+    static const int cps = getenv("MRCQR_K1_CPS") ? atoi(getenv("MRCQR_K1_CPS")) : 12;   // EXPERIMENT
+    int chunks = (cps * num_sms() + n - 1) / n;
     if (chunks > p.tiles_per_col) chunks = p.tiles_per_col;
     if (chunks < 1) chunks = 1;
     p.tiles_per_chunk = (p.tiles_per_col + chunks - 1) / chunks;
@@ -502,7 +561,7 @@ static void k1_launch_t(const K1Params& p_in, const double* A, const uint64_t* s
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int grid = p.n * p.chunks;
     k<<<grid, K1_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
-    mrcqr_k1_finalize<PREC><<<((REIM ? 2 : 1) * p.s * p.n + 255) / 256, 256, 0, stream>>>(p, partial, As, st);
+    k1_finalize<PREC>(p, partial, As, st, stream);
 }
 
 template <typename T, typename ST, int PREC>
@@ -516,16 +575,19 @@ static void k1_launch_fft16(const K1Params& p_in, const double* A, const uint64_
     auto k = mrcqr_k1_fft16<T, ST, PREC>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k<<<p.n * p.chunks, F16_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
-    mrcqr_k1_finalize<PREC><<<(p.s * p.n + 255) / 256, 256, 0, stream>>>(p, partial, As, st);
+    k1_finalize<PREC>(p, partial, As, st, stream);
 }
+
+bool k1_generates_signs(int64_t m, int reim) { return k1_fft16_usable(m, reim); }
 
 int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int s,
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
-                   Status* st, cudaStream_t stream, int reim)
+                   Status* st, cudaStream_t stream, int reim, const uint64_t* gen_seed, bool reset_status)
 {
     double* partial = reinterpret_cast<double*>(k1_work);
     K1Params p = k1_params(m, n, lda, s, prec, reim);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
+    if (gen_seed && k1_generates_signs(m, reim)) { p.gen_signs = 1; p.seed = *gen_seed; p.st_reset = reset_status ? st : nullptr; }
     if (k1_fft16_usable(m, reim)) {
         if (prec == 16) k1_launch_fft16<float, __half2, 16>(p, A, signs, idx, partial, As, st, stream);
         else if (prec == 32) k1_launch_fft16<float, Cx<float>, 32>(p, A, signs, idx, partial, As, st, stream);
