@@ -110,13 +110,18 @@ static inline Ctx& ctx() { return t_current ? *t_current : g_default; }
 // interleave with another context's.  The gate orders such stretches ON THE DEVICE (a stream waits for the event the
 // previous stretch recorded) and on the host (a mutex held while the stretch is enqueued); everything before it (K1, K2)
 // and the batched kernel (coefficients in shared memory) overlap freely.
+// While the process has only its default context (mrcqr_create never called) two stretches cannot be in flight at once
+// (one workspace: its calls are ordered already), and the two stream operations per stretch are skipped: they are part
+// of the gaps between the kernels of a small factorization.  mrcqr_create synchronises the device once and turns them on.
 struct ConstGate {
     std::recursive_mutex mu;                 // recursive: a call that spans two stretches (the debug dump) nests them
     cudaEvent_t ev = nullptr;
     bool pending = false;
+    bool multi = false;                      // a second context exists (or existed)
     void acquire(cudaStream_t st)
     {
         mu.lock();
+        if (!multi) return;
         if (!ev) cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
         cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
         cudaStreamIsCapturing(st, &cs);
@@ -124,10 +129,17 @@ struct ConstGate {
     }
     void release(cudaStream_t st)
     {
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        cudaStreamIsCapturing(st, &cs);
-        if (cs == cudaStreamCaptureStatusNone) { cudaEventRecord(ev, st); pending = true; }
+        if (multi) {
+            cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+            cudaStreamIsCapturing(st, &cs);
+            if (cs == cudaStreamCaptureStatusNone) { cudaEventRecord(ev, st); pending = true; }
+        }
         mu.unlock();
+    }
+    void enable()
+    {
+        std::lock_guard<std::recursive_mutex> lk(mu);
+        if (!multi) { cudaDeviceSynchronize(); cudaGetLastError(); multi = true; }
     }
 };
 static ConstGate g_gate;
@@ -322,6 +334,7 @@ extern "C" void mrcqr_shutdown(void) { free_ctx(ctx()); }
 extern "C" int mrcqr_create(mrcqr_handle_t* handle)
 {
     if (!handle) return -1;
+    g_gate.enable();
     *handle = reinterpret_cast<mrcqr_handle_t>(new Ctx());
     return 0;
 }
@@ -513,7 +526,9 @@ static int enqueue_factor(const Layout& L, int64_t m, int n, int64_t lda, const 
     int64_t* idx = reinterpret_cast<int64_t*>(g.ws + L.idx);
     double* Rs = reinterpret_cast<double*>(g.ws + L.Rs);
     // Algorithm 2 step 1: bins on the host (s values), sign words on the device (m bits)
-    cudaMemcpyAsync(idx, h_bins, sizeof(int64_t) * (size_t)s, cudaMemcpyHostToDevice, st);
+    // ... or, for s <= 256 in front of the register radix-16 K1, not copied at all: they ride in the launch parameters
+    const bool bins_inline = !seed_dev && k1_takes_host_bins(m, s, g.reim);
+    if (!bins_inline) cudaMemcpyAsync(idx, h_bins, sizeof(int64_t) * (size_t)s, cudaMemcpyHostToDevice, st);
     const int64_t nw = (m + 63) / 64;
     // sign words: by the draw kernel, or (register radix-16 form of K1, seed known now) by K1 itself where it uses them
     const bool k1_draws = !seed_dev && k1_generates_signs(m, g.reim);
@@ -523,7 +538,7 @@ static int enqueue_factor(const Layout& L, int64_t m, int n, int64_t lda, const 
     double* As = reinterpret_cast<double*>(g.ws + L.As);
     if (tm) cudaEventRecord(g.ev[0], st);
     k += launch_k1_srtt(m, n, lda, A, prec, s, signs, idx, g.ws + L.k1, As, stat, st, g.reim,
-                        k1_draws ? &seed : nullptr, reset_status);                                   // steps 2-4
+                        k1_draws ? &seed : nullptr, reset_status, bins_inline ? h_bins : nullptr);   // steps 2-4
     if (tm) cudaEventRecord(g.ev[1], st);
     k += launch_k2_sketch_qr(As, g.reim ? 2 * s : s, n, Rs, reinterpret_cast<double*>(g.ws + L.RsPrep), round_up(n, 16),
                              reinterpret_cast<double*>(g.ws + L.betas), stat, st);                              // steps 5-6

@@ -24,6 +24,7 @@
 // T = double serves p = FP64.  No fast-math intrinsics: twiddles come from sincospi.
 #include "mrcqr_internal.cuh"
 #include <cstdlib>
+#include <cstring>
 #include <cuda_fp16.h>
 
 namespace mrcqr {
@@ -63,6 +64,10 @@ __device__ __forceinline__ T diag_cast(double a, unsigned neg)
     return neg ? -v : v;
 }
 
+// s <= K1_INLINE_BINS: mrcqr_factor hands the drawn bins to the register radix-16 kernel as a launch parameter (constant
+// bank) instead of copying them to the device first: one host-to-device copy less in front of a call.
+constexpr int K1_INLINE_BINS = 256;
+struct K1Bins { int64_t v[K1_INLINE_BINS]; };
 struct K1Params {
     int64_t m, lda;
     int n, s, m1, log_m1;
@@ -75,6 +80,7 @@ struct K1Params {
     // used instead of read from the array a draw kernel wrote (a0: the same bits; one launch less), and the
     // status block is cleared here, by the first kernel of the call
     int gen_signs; uint64_t seed; Status* st_reset;
+    int inline_bins;              // the bins are in the K1Bins parameter, idx is not read
 };
 
 template <typename T, int PREC, int W, bool REIM>
@@ -285,9 +291,10 @@ constexpr int F16_W = 16, F16_NT = 256, F16_M1 = 256, F16_LD = F16_W + 1;
 
 template <typename T, typename ST, int PREC>
 __global__ void __launch_bounds__(F16_NT, sizeof(T) == 8 ? F16_DBL_CTAS : 2)
-mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restrict__ signs32,
-               const int64_t* __restrict__ idx, double* __restrict__ partial)
+mrcqr_k1_fft16(K1Params p, const __grid_constant__ K1Bins bins, const double* __restrict__ A,
+               const uint32_t* __restrict__ signs32, const int64_t* __restrict__ idx, double* __restrict__ partial)
 {
+    auto bin_at = [&](int i) -> int64_t { return p.inline_bins ? bins.v[i] : idx[i]; };
     extern __shared__ __align__(16) unsigned char smraw[];
     ST* tile = reinterpret_cast<ST*>(smraw);                                        // [256][17]
     Cx<T>* tw = reinterpret_cast<Cx<T>*>(smraw + (size_t)F16_M1 * F16_LD * sizeof(ST));   // [256]  W_256^e
@@ -338,7 +345,7 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
     }
     for (int e = tid; e < p.s; e += F16_NT) colacc[e] = 0.0;
     for (int i = tid; i < p.s; i += F16_NT) {
-        const int64_t k = idx[i];
+        const int64_t k = bin_at(i);
         Cx<T> d;
         sincospi_t((T)(2.0 * (double)(k & (p.m - 1)) / (double)p.m), &d.y, &d.x);
         dstep[i] = d;
@@ -358,14 +365,14 @@ mrcqr_k1_fft16(K1Params p, const double* __restrict__ A, const uint32_t* __restr
         int myrank[16];                                                            // s <= 4096: at most 16 bins per thread here
         int cnt = 0;
         for (int i = tid; i < p.s; i += F16_NT, ++cnt) {
-            const int k1 = (int)(idx[i] & (F16_M1 - 1));
+            const int k1 = (int)(bin_at(i) & (F16_M1 - 1));
             const int key = (16 * (k1 & 15) + (k1 >> 4)) & (G - 1);
             myrank[cnt & 15] = atomicAdd(&bucket[key], 1);
         }
         __syncthreads();
         cnt = 0;
         for (int i = tid; i < p.s; i += F16_NT, ++cnt) {
-            const int k1 = (int)(idx[i] & (F16_M1 - 1));
+            const int k1 = (int)(bin_at(i) & (F16_M1 - 1));
             const int key = (16 * (k1 & 15) + (k1 >> 4)) & (G - 1);
             const int r = myrank[cnt & 15];
             int pos = 0;
@@ -519,7 +526,7 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec, int re
 {
     K1Params p;
     p.m = m; p.lda = lda; p.n = n; p.s = s; p.reim = reim;
-    p.gen_signs = 0; p.seed = 0; p.st_reset = nullptr;
+    p.gen_signs = 0; p.seed = 0; p.st_reset = nullptr; p.inline_bins = 0;
     const bool f16 = k1_fft16_usable(m, reim);
     const int K1_W = f16 ? F16_W : k1_tile_w(m, prec, s, reim);
     const int m1max = f16 ? F16_M1 : ((prec == 64) ? 128 : 256) * (32 / K1_W);    // 68 KB tile (W = 8: 74 KB)
@@ -529,8 +536,7 @@ static K1Params k1_params(int64_t m, int n, int64_t lda, int s, int prec, int re
     p.m1 = (int)m1; p.m2 = m / m1;
     p.log_m1 = 0; while ((1 << p.log_m1) < p.m1) ++p.log_m1;
     p.tiles_per_col = (int)(p.m2 / (2 * K1_W));
-    static const int cps = getenv("MRCQR_K1_CPS") ? atoi(getenv("MRCQR_K1_CPS")) : 12;   // EXPERIMENT
-    int chunks = (cps * num_sms() + n - 1) / n;
+    int chunks = (12 * num_sms() + n - 1) / n;
     if (chunks > p.tiles_per_col) chunks = p.tiles_per_col;
     if (chunks < 1) chunks = 1;
     p.tiles_per_chunk = (p.tiles_per_col + chunks - 1) / chunks;
@@ -566,32 +572,37 @@ static void k1_launch_t(const K1Params& p_in, const double* A, const uint64_t* s
 
 template <typename T, typename ST, int PREC>
 static void k1_launch_fft16(const K1Params& p_in, const double* A, const uint64_t* signs, const int64_t* idx,
-                            double* partial, double* As, Status* st, cudaStream_t stream)
+                            double* partial, double* As, Status* st, cudaStream_t stream, const int64_t* h_bins)
 {
     K1Params p = p_in;
+    K1Bins bins;                                         // copied into the launch when it is made
+    p.inline_bins = (h_bins && p.s <= K1_INLINE_BINS) ? 1 : 0;
+    if (p.inline_bins) memcpy(bins.v, h_bins, sizeof(int64_t) * (size_t)p.s);
     size_t smem = (size_t)F16_M1 * F16_LD * sizeof(ST) + (size_t)F16_M1 * sizeof(Cx<T>) + (size_t)p.s * sizeof(double);
     p.dtab = 1;
     smem += (size_t)p.s * (sizeof(Cx<T>) + sizeof(int)) + (size_t)((p.s + 7) & ~7) * sizeof(unsigned short);
     auto k = mrcqr_k1_fft16<T, ST, PREC>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    k<<<p.n * p.chunks, F16_NT, smem, stream>>>(p, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
+    k<<<p.n * p.chunks, F16_NT, smem, stream>>>(p, bins, A, reinterpret_cast<const uint32_t*>(signs), idx, partial);
     k1_finalize<PREC>(p, partial, As, st, stream);
 }
 
 bool k1_generates_signs(int64_t m, int reim) { return k1_fft16_usable(m, reim); }
+bool k1_takes_host_bins(int64_t m, int s, int reim) { return k1_fft16_usable(m, reim) && s <= K1_INLINE_BINS; }
 
 int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int s,
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
-                   Status* st, cudaStream_t stream, int reim, const uint64_t* gen_seed, bool reset_status)
+                   Status* st, cudaStream_t stream, int reim, const uint64_t* gen_seed, bool reset_status,
+                   const int64_t* h_bins)
 {
     double* partial = reinterpret_cast<double*>(k1_work);
     K1Params p = k1_params(m, n, lda, s, prec, reim);
     p.vec = ((uintptr_t)A % 16 == 0) && (lda % 2 == 0);
     if (gen_seed && k1_generates_signs(m, reim)) { p.gen_signs = 1; p.seed = *gen_seed; p.st_reset = reset_status ? st : nullptr; }
     if (k1_fft16_usable(m, reim)) {
-        if (prec == 16) k1_launch_fft16<float, __half2, 16>(p, A, signs, idx, partial, As, st, stream);
-        else if (prec == 32) k1_launch_fft16<float, Cx<float>, 32>(p, A, signs, idx, partial, As, st, stream);
-        else k1_launch_fft16<double, Cx<double>, 64>(p, A, signs, idx, partial, As, st, stream);
+        if (prec == 16) k1_launch_fft16<float, __half2, 16>(p, A, signs, idx, partial, As, st, stream, h_bins);
+        else if (prec == 32) k1_launch_fft16<float, Cx<float>, 32>(p, A, signs, idx, partial, As, st, stream, h_bins);
+        else k1_launch_fft16<double, Cx<double>, 64>(p, A, signs, idx, partial, As, st, stream, h_bins);
         return 2;
     }
     const int w = k1_tile_w(m, prec, s, reim);

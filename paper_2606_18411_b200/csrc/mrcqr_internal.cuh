@@ -171,10 +171,13 @@ size_t k1_workspace_bytes(int64_t m, int n, int s, int prec);
 int launch_k1_srtt(int64_t m, int n, int64_t lda, const double* A, int prec, int s,
                    const uint64_t* signs, const int64_t* idx, void* k1_work, double* As,
                    Status* st, cudaStream_t stream, int reim = 0,       // reim: 2s rows, Im X[S] below Re X[S]
-                   const uint64_t* gen_seed = nullptr, bool reset_status = false);
+                   const uint64_t* gen_seed = nullptr, bool reset_status = false, const int64_t* h_bins = nullptr);
+// h_bins != nullptr (HOST pointer, read during the call) and k1_takes_host_bins(m, s, reim): the bins travel as a launch
+// parameter and `idx` is not read.
 // gen_seed != nullptr and k1_generates_signs(m, reim): K1 evaluates the sign words from *gen_seed itself (`signs` is not
 // read) and, with reset_status, clears the status block as the first kernel of the call.
 bool k1_generates_signs(int64_t m, int reim);
+bool k1_takes_host_bins(int64_t m, int s, int reim);
 
 // batched small problems, one CTA per problem (k_batched.cu); codes_dev: batch x 2 ints (code, info)
 bool batched_fused_usable(int64_t m, int n, int s);
