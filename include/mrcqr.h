@@ -73,10 +73,12 @@ enum {
 int mrcqr_draw(int64_t m, int s, uint64_t seed, uint64_t* signs_host, int64_t* idx_host);
 
 /*
- * The same draw (Algorithm 2 step 1) exactly as mrcqr_factor performs it, into DEVICE buffers: the
- * ceil(m/64) sign words by the device kernel of the library, the s bins drawn on the host and copied.  The words
- * and bins are bit-identical to mrcqr_draw's (and the oracle's); the GPU tests pin that.  signs / idx: device.
- * Synchronises the stream.  Returns as mrcqr_draw, or 4.
+ * The same draw (Algorithm 2 step 1) into DEVICE buffers: the ceil(m/64) sign words by the device kernel
+ * of the library, the s bins drawn on the host and copied.  The words and bins are bit-identical to mrcqr_draw's (and
+ * the oracle's); the GPU tests pin that.  mrcqr_factor draws the same words: with this kernel when m < 8192, in the
+ * Re+Im variant and under graph replay, otherwise inside its transform kernel, which evaluates X(word) where it uses
+ * it (the tests require mrcqr_factor to equal, bit for bit, its stage calls run on these buffers).  signs / idx:
+ * device.  Synchronises the stream.  Returns as mrcqr_draw, or 4.
  */
 int mrcqr_draw_device(int64_t m, int s, uint64_t seed, uint64_t* signs, int64_t* idx, void* stream);
 
