@@ -298,21 +298,24 @@ mrcqr_k2_sketch_qr(double* __restrict__ As, int s, int n, int use_smem, double* 
 // shared vector; the warp that owns column j+1 forms v_{j+1} right after updating it.
 // Reflector, unnormalised: v = x - beta e_j (v_j = alpha - beta), H = I - c v v^T, c = 1 / (beta (beta - alpha))
 // (= tau / v_j^2 of the LAPACK form): one square root and one reciprocal per column.
-template <int CPW, int RPL>
-__global__ void __launch_bounds__(SMALL_NT)
+// NW warps per CTA (column c -> warp c % NW): a 32 x 16 sketch (n = 16, s = 2n) runs on 16 warps with one row slot
+// instead of 32 warps with four, i.e. a cheaper barrier and a quarter of the multiply-adds per reflector; the arithmetic
+// of every element is the same (the slots that are gone held exact zeros).
+template <int CPW, int RPL, int NW = 32>
+__global__ void __launch_bounds__(32 * NW)
 mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __restrict__ Rs,
                        double* __restrict__ RsPrep, int n16, Status* st)
 {
     __shared__ double vbuf[2][RPL * 32];
     __shared__ double cbuf[2];
-    __shared__ double betas[32 * CPW];
+    __shared__ double betas[NW * CPW];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     double a[CPW][RPL];
 #pragma unroll
     for (int k = 0; k < CPW; ++k)
 #pragma unroll
         for (int r = 0; r < RPL; ++r) {
-            const int c = warp + 32 * k, i = lane + 32 * r;
+            const int c = warp + NW * k, i = lane + 32 * r;
             a[k][r] = (c < n && i < s) ? As[(size_t)c * s + i] : 0.0;
         }
     // forms the reflector of column j (held in slot k of this warp) and publishes it in buffer j & 1
@@ -360,7 +363,7 @@ mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __re
             for (int k = 0; k < CPW; ++k) w[k] += __shfl_xor_sync(0xffffffffu, w[k], o);
 #pragma unroll
         for (int k = 0; k < CPW; ++k) {
-            const int c = warp + 32 * k;
+            const int c = warp + NW * k;
             if (c > j && c < n) {
                 const double wt = w[k] * cf;
 #pragma unroll
@@ -369,14 +372,14 @@ mrcqr_k2_sketch_qr_reg(const double* __restrict__ As, int s, int n, double* __re
         }
 #pragma unroll
         for (int k = 0; k < CPW; ++k)
-            if (warp + 32 * k == j + 1 && j + 1 < n) make_v(k, j + 1);
+            if (warp + NW * k == j + 1 && j + 1 < n) make_v(k, j + 1);
     }
     __syncthreads();
 #pragma unroll
     for (int k = 0; k < CPW; ++k)
 #pragma unroll
         for (int r = 0; r < RPL; ++r) {
-            const int c = warp + 32 * k, i = lane + 32 * r;
+            const int c = warp + NW * k, i = lane + 32 * r;
             if (c < n && i < n) {
                 double val = (i <= c) ? a[k][r] : 0.0;
                 if (i <= c && betas[i] < 0.0) val = -val;    // sign-normalise row i: diag(Rs) > 0
@@ -419,7 +422,10 @@ int launch_k2_sketch_qr(const double* As, int s_rows, int n, double* Rs, double*
                         double* betas, Status* st, cudaStream_t s)
 {
     if (n <= 64 && s_rows <= 256) {
-        if (n <= 32 && s_rows <= 128) mrcqr_k2_sketch_qr_reg<1, 4><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
+        if (n <= 16 && s_rows <= 32) mrcqr_k2_sketch_qr_reg<1, 1, 16><<<1, 512, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
+        else if (n <= 16 && s_rows <= 64) mrcqr_k2_sketch_qr_reg<1, 2, 16><<<1, 512, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
+        else if (n <= 32 && s_rows <= 64) mrcqr_k2_sketch_qr_reg<1, 2><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
+        else if (n <= 32 && s_rows <= 128) mrcqr_k2_sketch_qr_reg<1, 4><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
         else if (s_rows <= 128) mrcqr_k2_sketch_qr_reg<2, 4><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
         else mrcqr_k2_sketch_qr_reg<2, 8><<<1, SMALL_NT, 0, s>>>(As, s_rows, n, Rs, RsPrep, n16, st);
         return 1;
