@@ -83,6 +83,23 @@ def test_batched_argument_errors():
     assert L.mrcqr_factor_batched(2, 1024, 8, 1024, 8192, p, 8192, p, p, 32, 4, 0, None, None) == -11
 
 
+def test_async_argument_errors():
+    # mrcqr_factor_async checks its arguments like mrcqr_factor and reports them at once (include/mrcqr.h)
+    L = B.lib()
+    p = C.c_void_p(16)            # never dereferenced
+    assert L.mrcqr_factor_async(1000, 8, 1000, p, p, p, 32, 16, 0, None) == -1
+    assert L.mrcqr_factor_async(1024, 0, 1024, p, p, p, 32, 16, 0, None) == -2
+    assert L.mrcqr_factor_async(1024, 8, 1000, p, p, p, 32, 16, 0, None) == -3
+    assert L.mrcqr_factor_async(1024, 8, 1024, None, p, p, 32, 16, 0, None) == -4
+    assert L.mrcqr_factor_async(1024, 8, 1024, p, None, p, 32, 16, 0, None) == -5
+    assert L.mrcqr_factor_async(1024, 8, 1024, p, p, None, 32, 16, 0, None) == -6
+    assert L.mrcqr_factor_async(1024, 8, 1024, p, p, p, 8, 16, 0, None) == -7
+    assert L.mrcqr_factor_async(1024, 8, 1024, p, p, p, 32, 4, 0, None) == -8
+    if not torch.cuda.is_available():
+        assert L.mrcqr_factor_async(1024, 8, 1024, p, p, p, 32, 16, 0, None) == 4     # no device: no fallback
+        assert L.mrcqr_wait(None) == 4
+
+
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-device behaviour")
 def test_no_cpu_fallback_without_device():
     L = B.lib()
