@@ -215,11 +215,44 @@ mrcqr_k5_formq(int64_t m, int n, int n16, int64_t lda, const double* __restrict_
         load_slab<SR, VEC>(slab, A, lda, m, n, row0, lane);
         if (VEC) cp_async_wait_all();
         __syncwarp();
-        if (mode & 1) solve_slab<RG, 0, NBT>(slab, fragS, nB, lane);        // y = a Rs^-1, same code as K3
-        if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); __syncwarp(); }
-        if (mode & 2) solve_slab<RG, 1, NBT>(slab, fragC, nB, lane);        // q = y Rc^-1
-        __syncwarp();
-        if (Q) store_slab<SR, VEC>(slab, Q, ldq, m, n, row0, lane);          // Q = nullptr: the debug dump wants only Y
+        if constexpr (NBT > 0 && NBT <= 8) {
+            // one panel (n16 <= 64): the panel goes into accumulator registers ONCE; the second solve starts from the
+            // fragments the first one left there, and every block of Q leaves for global memory from its row form, so
+            // the slab is not re-read between the solves nor for the store (K5 at n16 = 16 was bound by the
+            // shared-memory pipe: 67 % busy).  Same panel_core, same operations as K3's solve_slab: Y stays bit-identical.
+            const int g = lane >> 2, t = lane & 3;
+            const double* yw = slab + t * LDS_ + g;
+            double acc[RG][NBT][2];
+#pragma unroll
+            for (int J = 0; J < NBT; ++J)
+#pragma unroll
+                for (int rg = 0; rg < RG; ++rg) {
+                    acc[rg][J][0] = yw[(8 * J) * LDS_ + 8 * rg];
+                    acc[rg][J][1] = yw[(8 * J + 4) * LDS_ + 8 * rg];
+                }
+            const SlabXpose<RG> xp(slab, lane);
+            const RowSink rs{Q + row0 + lane, ldq, n, row0 + lane < m};
+            if ((mode & 2) && Q) {
+                if (mode & 1) {
+                    panel_core<RG, NBT, true>(acc, xp, ConstFactor<0>{fragS}, 0, lane, NoSink());      // y = a Rs^-1
+                    if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); }
+                    __syncwarp();
+                }
+                panel_core<RG, NBT, false, true>(acc, xp, ConstFactor<1>{fragC}, 0, lane, rs);         // q = y Rc^-1
+            } else {
+                if (mode & 1) panel_core<RG, NBT>(acc, xp, ConstFactor<0>{fragS}, 0, lane, NoSink());
+                if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); __syncwarp(); }
+                if (mode & 2) solve_slab<RG, 1, NBT>(slab, fragC, nB, lane);
+                __syncwarp();
+                if (Q) store_slab<SR, VEC>(slab, Q, ldq, m, n, row0, lane);
+            }
+        } else {
+            if (mode & 1) solve_slab<RG, 0, NBT>(slab, fragS, nB, lane);        // y = a Rs^-1, same code as K3
+            if (Ydump) { __syncwarp(); store_slab<SR, false>(slab, Ydump, m, m, n, row0, lane); __syncwarp(); }
+            if (mode & 2) solve_slab<RG, 1, NBT>(slab, fragC, nB, lane);        // q = y Rc^-1
+            __syncwarp();
+            if (Q) store_slab<SR, VEC>(slab, Q, ldq, m, n, row0, lane);          // Q = nullptr: the debug dump wants only Y
+        }
     }
 }
 

@@ -257,6 +257,18 @@ struct ScratchXpose {
     __device__ __forceinline__ bool row_active() const { return SR >= 32 || lane < SR; }
 };
 struct NoSink { __device__ __forceinline__ void operator()(int, const double (&)[8]) const {} };
+// RowSink: a solved block leaves for a column-major matrix straight from its row form (lane = row of the slab: 256
+// contiguous bytes per column and warp); out = &Q[row0 + lane], columns >= n and rows >= m are not written.
+struct RowSink {
+    double* out; int64_t ldq; int n; bool row_ok;
+    __device__ __forceinline__ void operator()(int Kg, const double (&y)[8]) const
+    {
+        if (!row_ok) return;
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if (8 * Kg + j < n) __stcs(out + (size_t)(8 * Kg + j) * (size_t)ldq, y[j]);
+    }
+};
 
 // The right-looking sweep inside a panel of PB column blocks starting at global block P0, on the
 // accumulator registers acc[rg][J][e] (matrix column 8(P0+J) + t + 4e of row 8 rg + g).
@@ -266,7 +278,10 @@ struct NoSink { __device__ __forceinline__ void operator()(int, const double (&)
 // with) the dependent fma chain of that step's substitution; only J = K+1 is updated at once.
 // sink(Kg, y) sees every solved block in row form (lane = row of the slab).
 // This is the ONLY place the solve's arithmetic lives: K3 and K5 both run it.
-template <int RG, int PB, typename X, typename F, typename SINK>
+// KEEP: the solved blocks are also left in acc (fragment form), so that a second solve of the same panel can start from
+// the registers.  DROP_LAST: the last block is not written back to its transposition buffer after its substitution (the
+// sink has taken it and no later block needs its fragments).  Neither changes a single floating-point operation.
+template <int RG, int PB, bool KEEP = false, bool DROP_LAST = false, typename X, typename F, typename SINK>
 __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp, const F& fac,
                                            int P0, int lane, const SINK& sink)
 {
@@ -298,14 +313,18 @@ __device__ __forceinline__ void panel_core(double (&acc)[RG][PB][2], const X& xp
         }
         if (xp.row_active()) {
             fac.substitute(y, P0, K);
+            if (!(DROP_LAST && K == PB - 1)) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) *xp.rowp(P0 + K, j) = y[j];
+                for (int j = 0; j < 8; ++j) *xp.rowp(P0 + K, j) = y[j];
+            }
             sink(P0 + K, y);
         }
-        __syncwarp();
+        if (!(DROP_LAST && K == PB - 1)) {
+            __syncwarp();
 #pragma unroll
-        for (int rg = 0; rg < RG; ++rg) { ap0[rg] = *xp.accp(P0 + K, rg, 0); ap1[rg] = *xp.accp(P0 + K, rg, 1); }
-        if (X::REUSE) {
+            for (int rg = 0; rg < RG; ++rg) { ap0[rg] = *xp.accp(P0 + K, rg, 0); ap1[rg] = *xp.accp(P0 + K, rg, 1); }
+        }
+        if (X::REUSE || KEEP) {
 #pragma unroll
             for (int rg = 0; rg < RG; ++rg) { acc[rg][K][0] = ap0[rg]; acc[rg][K][1] = ap1[rg]; }
         }

@@ -102,3 +102,25 @@ def test_async_more_calls_than_ring_slots_and_a_change_of_stream():
     B.mrcqr_factor_async(big, 64, 80, 3, Qa, Ra)
     assert B.mrcqr_wait() == (0, 0)
     assert torch.equal(outs[2][0], ref[1][0]) and torch.equal(Qa, Qb) and torch.equal(Ra, Rb)
+
+
+def test_async_honours_the_switches_of_the_context():
+    # the Re+Im sketch (draw kernel + radix-4 K1) and the forced forms of stage 2 take the same path in flight
+    rng = np.random.default_rng(8)
+    m, n, s = 16384, 48, 96
+    AT = colmajor_to_dev(rng.standard_normal((m, n)))
+    outs = [(torch.empty_like(AT), torch.empty((n, n), dtype=torch.float64, device="cuda")) for _ in range(3)]
+    try:
+        for reim, store in ((True, None), (False, False), (False, True)):
+            B.mrcqr_set_sketch_reim(reim)
+            B.mrcqr_set_store_y(store)
+            Qs, Rs_ = B.mrcqr_factor(AT, 32, s, 11)
+            Qs, Rs_ = Qs.clone(), Rs_.clone()
+            for k in range(3):
+                B.mrcqr_factor_async(AT, 32, s, 11, *outs[k])
+            assert B.mrcqr_wait() == (0, 0)
+            for k in range(3):
+                assert torch.equal(outs[k][0], Qs) and torch.equal(outs[k][1], Rs_)
+    finally:
+        B.mrcqr_set_sketch_reim(False)
+        B.mrcqr_set_store_y(None)
