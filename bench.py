@@ -596,6 +596,45 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# The paper's Table I: MRCQR on an H100 PCIe with cuFFT / cuBLAS / cuSOLVER, m = 2^20,
+# c = 3n, mean of 5 trials, ms, by sketch precision (fp64, fp32, fp16).  Context only: another machine, another build.
+PAPER_TABLE1 = {20: (2.60, 2.33, 2.19), 40: (5.22, 4.71, 4.46), 60: (7.84, 7.06, 6.67), 80: (10.80, 9.77, 9.26),
+                100: (14.05, 12.75, 12.11), 120: (17.18, 15.62, 14.84), 140: (21.15, 19.32, 18.41), 160: (23.64, 21.56, 20.53),
+                180: (27.48, 25.18, 24.00), 200: (31.43, 28.83, 27.50)}
+
+
+def run_table1(args):
+    """--table1: the shapes of the paper's Table I (m = 2^20, n = 20 .. 200, s = 3n, the three sketch precisions) on
+    synthetic matrices of the BASELINE.json recipe (kappa ~ 1e4, seeds 60+n / 61+n / 62+n), ms per factorization
+    (mrcqr_factor, CUDA events, 3 warm-ups + --steps timed), the paper's H100 figure beside each as context."""
+    import torch
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import gpu_orth_error_fro
+    from paper_2606_18411_b200 import binding as B
+    from paper_2606_18411_b200 import inputs
+    m = 1 << 20
+    print("| n | s | fp64 sketch ms (paper, H100 PCIe) | fp32 sketch ms (paper) | fp16 sketch ms (paper) | orth (fp16) |")
+    print("|---|---|---|---|---|---|")
+    for n in sorted(PAPER_TABLE1):
+        AT = inputs.make_A(m, n, 4, 60 + n, 61 + n, "cuda")
+        QT = torch.empty_like(AT)
+        R = torch.empty((n, n), dtype=torch.float64, device="cuda")
+        cells = []
+        for k, prec in enumerate((64, 32, 16)):
+            for _ in range(3):
+                B.mrcqr_factor(AT, prec, 3 * n, 62 + n, QT=QT, R=R)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(args.steps):
+                B.mrcqr_factor(AT, prec, 3 * n, 62 + n, QT=QT, R=R)
+            e1.record()
+            torch.cuda.synchronize()
+            cells.append("%.3f (%.2f)" % (e0.elapsed_time(e1) / args.steps, PAPER_TABLE1[n][k]))
+        print("| %d | %d | %s | %s | %s | %.1e |" % (n, 3 * n, cells[0], cells[1], cells[2], gpu_orth_error_fro(QT)), flush=True)
+        del AT, QT
+    return 0
+
+
 def run_sweep(args):
     """--sweep: BASELINE.json configs[0..3] and the column sweep configs[4] (m = 2^21, n in 16..512, three sketch
     precisions): per-stage CUDA-event times and both roofline floors, one markdown table row per point (not the
@@ -685,11 +724,14 @@ def main():
     ap.add_argument("--traffic-from", default=None, help="ncu --page raw --csv file: record per-kernel DRAM bytes of --config in profiles/r02_traffic.json")
     ap.add_argument("--stability", action="store_true", help="orthogonality / residual vs kappa on the paper's eq.(3) matrices")
     ap.add_argument("--sweep", action="store_true", help="per-stage table over BASELINE.json configs 0-4 instead of the JSON line")
+    ap.add_argument("--table1", action="store_true", help="the shapes of the paper's Table I (m = 2^20, n = 20..200, s = 3n), the paper's H100 figures beside as context")
     args = ap.parse_args()
     if args.traffic_from:
         return write_traffic(args.traffic_from, args.config)
     if args.stability:
         return run_stability(args)
+    if args.table1:
+        return run_table1(args)
     if args.sweep:
         args.steps = min(args.steps, 5)
         return run_sweep(args)
